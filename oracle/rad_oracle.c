@@ -1,0 +1,149 @@
+/*
+ * rad_oracle.c -- fp64 CPU ORACLE for the far-field (Lienard-Wiechert) radiation detector.
+ *
+ * TEST INFRASTRUCTURE ONLY.  Nothing on the product path (paper_2501_03383_b200/) may
+ * include, link, import or call this file; only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs use it.  It shares no code, header,
+ * table or constant generator with the CUDA path.
+ *
+ * What it computes (BASELINE.json north_star; "weighted sum of all
+ * contributions from all particles"; lines 79-81 "at each time step ... sum of the
+ * contributions from all radiating particles ... complex amplitude and phase for each
+ * wavelength and direction"; line 142 "Lienard-Wiechert potential approach [38]";
+ * SURVEY.md section 8(c)):
+ *
+ *   for each call (step t, particles k), each direction n, each frequency w_j:
+ *      d    = 1 - beta_k . n
+ *      a    = w_k * dt * [ n x ((n - beta_k) x betadot_k) ] / d^2          (3-vector)
+ *      tau  = (t0 + t*dt) - (n . r_k)/c
+ *      A[n][j][c] += a_c * (cos(w_j tau) + i sin(w_j tau)),   c in {x,y,z}
+ *   S[n][j] = scale * (|A_x|^2 + |A_y|^2 + |A_z|^2)
+ *
+ * Written exactly in that order with the two explicit cross products, plain double
+ * arithmetic, libm sin/cos, plain summation in particle order; no blocking, no
+ * reordering, no fast-math.  OpenMP only splits the independent (n, j) bins over
+ * threads; every bin's sum is sequential in k, so results do not depend on the
+ * thread count.
+ *
+ * Readings of the paper: Q1 phase sign +i w (t - n.r/c);
+ * Q2 time of step t is t0 + t*dt; Q3 rectangle rule, every term times dt, no window;
+ * Q4 spectrum = scale*|A|^2, default scale e^2/(16 pi^3 eps0 c); Q5 amplitude linear
+ * in the macro weight; Q8 n normalised in fp64; Q9 far field (1/R dropped).
+ *
+ * Pins (tests/test_oracle_pins.py): zero for unaccelerated motion, Dirichlet kernel
+ * (magnitude and complex phase), Doppler-shifted Dirichlet kernel, two-particle
+ * interference, linearity/superposition, cyclotron (Schott) harmonics, SI constant,
+ * mpmath/numpy brute force.  The spectra of the five BASELINE.json configs themselves
+ * have no published values: "parity unpinned" except through those pins.
+ */
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_C_LIGHT 299792458.0 /* m/s, exact (SI) */
+
+/* e^2 / (16 pi^3 eps0 c) in J s, from CODATA-2018 e and eps0 (SURVEY.md Q4 / pin P9). */
+double oracle_default_scale(void)
+{
+    const double e = 1.602176634e-19;     /* C, exact */
+    const double eps0 = 8.8541878128e-12; /* F/m */
+    const double pi = 3.14159265358979323846;
+    return (e * e) / (16.0 * pi * pi * pi * eps0 * ORACLE_C_LIGHT);
+}
+
+int oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+static void cross3(const double a[3], const double b[3], double out[3])
+{
+    out[0] = a[1] * b[2] - a[2] * b[1];
+    out[1] = a[2] * b[0] - a[0] * b[2];
+    out[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+/*
+ * Accumulate one PIC step into A.
+ *   dirs   [n_dir][3]   fp64, any non-zero length (normalised here, Q8)
+ *   omega  [n_omega]    rad/s
+ *   state  10 SoA arrays of length n_part; is_f32 != 0 -> float arrays promoted
+ *          value-for-value to double, else double arrays
+ *   bin_idx optional list of n_bins flat bin indices (dir*n_omega + j) to compute;
+ *          NULL -> all bins.  Bins are independent sums, so a subset is exact.
+ *   A      [n_dir][n_omega][3][2] (re, im) fp64, accumulated in place (only the
+ *          selected bins are touched)
+ * Returns 0, or 1 on a bad argument.
+ */
+int oracle_accumulate_step(int n_dir, const double *dirs, int n_omega, const double *omega,
+                           double dt, double t0, long long step_index, long long n_part,
+                           int is_f32, const void *rx, const void *ry, const void *rz,
+                           const void *bx, const void *by, const void *bz, const void *bdx,
+                           const void *bdy, const void *bdz, const void *w,
+                           long long n_bins, const long long *bin_idx, double *A)
+{
+    if (n_dir <= 0 || n_omega <= 0 || !dirs || !omega || !A || n_part < 0) return 1;
+    const long long total = bin_idx ? n_bins : (long long)n_dir * n_omega;
+    const double t_step = t0 + (double)step_index * dt;
+
+#define LOAD(p, k) (is_f32 ? (double)((const float *)(p))[k] : ((const double *)(p))[k])
+
+#pragma omp parallel for schedule(dynamic, 1)
+    for (long long b = 0; b < total; ++b) {
+        const long long flat = bin_idx ? bin_idx[b] : b;
+        const int id = (int)(flat / n_omega);
+        const int j = (int)(flat % n_omega);
+        double n[3] = {dirs[3 * id + 0], dirs[3 * id + 1], dirs[3 * id + 2]};
+        const double nn = sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+        n[0] /= nn; n[1] /= nn; n[2] /= nn;
+        const double om = omega[j];
+        double acc[6] = {0, 0, 0, 0, 0, 0};
+        for (long long k = 0; k < n_part; ++k) {
+            const double r[3] = {LOAD(rx, k), LOAD(ry, k), LOAD(rz, k)};
+            const double be[3] = {LOAD(bx, k), LOAD(by, k), LOAD(bz, k)};
+            const double bd[3] = {LOAD(bdx, k), LOAD(bdy, k), LOAD(bdz, k)};
+            const double wk = LOAD(w, k);
+            const double d = 1.0 - (be[0] * n[0] + be[1] * n[1] + be[2] * n[2]);
+            const double nmb[3] = {n[0] - be[0], n[1] - be[1], n[2] - be[2]};
+            double inner[3], outer[3];
+            cross3(nmb, bd, inner);   /* (n - beta) x betadot        */
+            cross3(n, inner, outer);  /* n x ((n - beta) x betadot)  */
+            const double pre = wk * dt / (d * d);
+            const double tau = t_step - (n[0] * r[0] + n[1] * r[1] + n[2] * r[2]) / ORACLE_C_LIGHT;
+            const double ph = om * tau;
+            const double cs = cos(ph), sn = sin(ph);
+            for (int c = 0; c < 3; ++c) {
+                const double a = pre * outer[c];
+                acc[2 * c + 0] += a * cs;
+                acc[2 * c + 1] += a * sn;
+            }
+        }
+        double *dst = A + (size_t)flat * 6;
+        for (int c = 0; c < 6; ++c) dst[c] += acc[c];
+    }
+#undef LOAD
+    return 0;
+}
+
+/* S[n][j] = scale * sum_c |A_c|^2 ; scale == 0 -> SI default (Q4). */
+int oracle_spectrum(long long n_bins_total, const double *A, double scale, double *S)
+{
+    if (!A || !S || n_bins_total < 0) return 1;
+    const double sc = (scale == 0.0) ? oracle_default_scale() : scale;
+    for (long long b = 0; b < n_bins_total; ++b) {
+        const double *a = A + (size_t)b * 6;
+        double s = 0.0;
+        for (int c = 0; c < 6; ++c) s += a[c] * a[c];
+        S[b] = sc * s;
+    }
+    return 0;
+}

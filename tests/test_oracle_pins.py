@@ -1,0 +1,315 @@
+"""Pins for the fp64 oracle (oracle/rad_oracle.c) -- CPU only.
+
+The paper prints no worked numerical example for the radiation detector (PAPER.md has
+no equation for it), so every pin is a closed form, an invariant or a
+brute force, as BASELINE.json north_star prescribes ("zero output for unaccelerated
+straight-line motion; cyclotron lines at harmonics of w_c for helical motion; exact
+linearity in particle weights and superposition across particles and steps; brute-force
+agreement on tiny inputs").  Pin numbers follow SURVEY.md section 8(c).
+Each pin is chosen so that a plausible slip (dropped dt, wrong sign of the phase, wrong
+power of (1 - beta.n), transposed cross product, metres vs c) fails at least one of them.
+"""
+import numpy as np
+import pytest
+from scipy import special
+
+C = 299792458.0
+
+
+def _run(oracle_mod, dirs, omega, dt, steps, t0=0.0, scale=1.0, bins=None):
+    """steps: iterable of (step_index, state list)."""
+    o = oracle_mod.Oracle(dirs, omega, dt, t0=t0, scale=scale, bins=bins)
+    for t, st in steps:
+        o.accumulate_step(t, *st)
+    return o
+
+
+def _const_state(r0, beta, bdot, w=1.0, dtype=np.float64):
+    vals = list(r0) + list(beta) + list(bdot) + [w]
+    return [np.array([v], dtype=dtype) for v in vals]
+
+
+DIRS = np.array([[1.0, 0.0, 0.0], [0.0, 0.0, 2.0], [0.3, -0.5, 0.8], [-0.6, 0.64, 0.48],
+                 [0.1, 0.2, -0.97]])
+UNIT = DIRS / np.linalg.norm(DIRS, axis=1, keepdims=True)
+OMEGA = np.array([3.0e14, 1.0e15, 2.7e15, 8.1e15, 3.3e16])
+DT = 2.0e-17
+
+
+# ------------------------------------------------------------------------------ P1 zero
+def test_p1_unaccelerated_motion_gives_exact_zero(oracle_mod):
+    rng = np.random.default_rng(1)
+    n = 50
+    beta = rng.uniform(-0.5, 0.5, (3, n))
+    r0 = rng.uniform(0, 1e-5, (3, n))
+    steps = []
+    for t in range(7):
+        r = r0 + C * beta * t * DT
+        steps.append((t, [r[0], r[1], r[2], beta[0], beta[1], beta[2],
+                          np.zeros(n), np.zeros(n), np.zeros(n), rng.uniform(0.5, 2, n)]))
+    o = _run(oracle_mod, DIRS, OMEGA, DT, steps)
+    assert np.all(o.A == 0.0)
+    assert np.all(o.spectrum() == 0.0)
+
+
+# ----------------------------------------------------------- P2 / P3 Dirichlet kernel
+def _dirichlet(x, T):
+    """sin(T x/2)/sin(x/2)."""
+    return np.sin(T * x / 2.0) / np.sin(x / 2.0)
+
+
+@pytest.mark.parametrize("t0", [0.0, 3.7e-16])
+def test_p2_p3_static_particle_dirichlet_kernel(oracle_mod, t0):
+    r0 = np.array([1.3e-6, -2.1e-6, 0.7e-6])
+    b = np.array([2.0e12, -1.0e12, 0.5e12])
+    w, T = 1.7, 23
+    st = _const_state(r0, (0, 0, 0), b, w)
+    o = _run(oracle_mod, DIRS, OMEGA, DT, [(t, st) for t in range(T)], t0=t0)
+    A = o.amplitude()
+    S = o.spectrum()
+    for i, n in enumerate(UNIT):
+        ndb = n @ b
+        vec = n * ndb - b                       # n x (n x b), written as BAC-CAB
+        for j, om in enumerate(OMEGA):
+            dk = _dirichlet(om * DT, T)
+            # P2: magnitude
+            s_ref = w ** 2 * (b @ b - ndb ** 2) * DT ** 2 * dk ** 2
+            assert S[i, j] == pytest.approx(s_ref, rel=1e-9)
+            # P3: complex amplitude incl. sign of the phase, t0 and n.r/c
+            ph = np.exp(1j * om * (t0 - (n @ r0) / C)) * np.exp(1j * om * (T - 1) * DT / 2.0)
+            a_ref = w * DT * vec * ph * dk
+            assert np.allclose(A[i, j], a_ref, rtol=1e-9, atol=1e-12 * np.abs(a_ref).max())
+
+
+# --------------------------------------------------------- P4 Doppler-shifted Dirichlet
+def test_p4_uniform_motion_with_constant_betadot_doppler(oracle_mod):
+    r0 = np.array([0.4e-6, 0.9e-6, -0.3e-6])
+    beta = np.array([0.31, -0.12, 0.22])
+    b = np.array([-1.0e12, 3.0e12, 2.0e12])
+    w, T = 0.8, 31
+    steps = [(t, _const_state(r0 + C * beta * t * DT, beta, b, w)) for t in range(T)]
+    S = _run(oracle_mod, DIRS, OMEGA, DT, steps).spectrum()
+    for i, n in enumerate(UNIT):
+        d = 1.0 - n @ beta
+        vec = (n - beta) * (n @ b) - b * d     # BAC-CAB of n x ((n-beta) x b)
+        for j, om in enumerate(OMEGA):
+            dk = _dirichlet(om * d * DT, T)    # Doppler: w' = w (1 - n.beta)
+            s_ref = w ** 2 * (vec @ vec) / d ** 4 * DT ** 2 * dk ** 2
+            assert S[i, j] == pytest.approx(s_ref, rel=2e-9)
+
+
+# ------------------------------------------------------------ P5 two-particle interference
+def test_p5_two_displaced_particles_interfere(oracle_mod):
+    r0 = np.array([0.2e-6, 0.1e-6, 0.5e-6])
+    dr = np.array([0.37e-6, -0.81e-6, 0.29e-6])
+    b = np.array([1.0e12, 2.0e12, -0.7e12])
+    T = 9
+    one = [(t, _const_state(r0, (0, 0, 0), b)) for t in range(T)]
+    two_state = [np.array([r0[0], r0[0] + dr[0]]), np.array([r0[1], r0[1] + dr[1]]),
+                 np.array([r0[2], r0[2] + dr[2]])] + [np.zeros(2)] * 3 + \
+                [np.full(2, b[0]), np.full(2, b[1]), np.full(2, b[2]), np.ones(2)]
+    S1 = _run(oracle_mod, DIRS, OMEGA, DT, one).spectrum()
+    S2 = _run(oracle_mod, DIRS, OMEGA, DT, [(t, two_state) for t in range(T)]).spectrum()
+    for i, n in enumerate(UNIT):
+        for j, om in enumerate(OMEGA):
+            fac = 4.0 * np.cos(om * (n @ dr) / (2.0 * C)) ** 2
+            assert S2[i, j] == pytest.approx(S1[i, j] * fac, rel=1e-9, abs=1e-14 * S1.max())
+
+
+# ------------------------------------------------------- P6 linearity and superposition
+def _random_steps(rng, n, T, dtype=np.float64):
+    out = []
+    for t in range(T):
+        st = [rng.uniform(0, 5e-6, n) for _ in range(3)] + \
+             [rng.uniform(-0.4, 0.4, n) for _ in range(3)] + \
+             [rng.uniform(-3e12, 3e12, n) for _ in range(3)] + [rng.uniform(0.5, 2.0, n)]
+        out.append((t, [a.astype(dtype) for a in st]))
+    return out
+
+
+def test_p6_linearity_superposition_split_permutation(oracle_mod):
+    rng = np.random.default_rng(6)
+    steps = _random_steps(rng, 40, 5)
+    base = _run(oracle_mod, DIRS, OMEGA, DT, steps)
+    A0, S0 = base.amplitude(), base.spectrum()
+    # weights scaled by lambda: A -> lambda A, S -> lambda^2 S
+    lam = 3.0
+    scaled = [(t, st[:9] + [lam * st[9]]) for t, st in steps]
+    o = _run(oracle_mod, DIRS, OMEGA, DT, scaled)
+    assert np.allclose(o.amplitude(), lam * A0, rtol=1e-13, atol=0)
+    assert np.allclose(o.spectrum(), lam ** 2 * S0, rtol=1e-12)
+    # particle set split into two calls with the same step_index; and two detectors summed
+    o = oracle_mod.Oracle(DIRS, OMEGA, DT, scale=1.0)
+    oa = oracle_mod.Oracle(DIRS, OMEGA, DT, scale=1.0)
+    ob = oracle_mod.Oracle(DIRS, OMEGA, DT, scale=1.0)
+    for t, st in steps:
+        o.accumulate_step(t, *[a[:17] for a in st])
+        o.accumulate_step(t, *[a[17:] for a in st])
+        oa.accumulate_step(t, *[a[:17] for a in st])
+        ob.accumulate_step(t, *[a[17:] for a in st])
+    tol = 1e-12 * np.abs(A0).max()
+    assert np.allclose(o.amplitude(), A0, rtol=0, atol=tol)
+    assert np.allclose(oa.amplitude() + ob.amplitude(), A0, rtol=0, atol=tol)
+    # permutation of particles and order of steps
+    perm = rng.permutation(40)
+    o = _run(oracle_mod, DIRS, OMEGA, DT, [(t, [a[perm] for a in st]) for t, st in steps[::-1]])
+    assert np.allclose(o.amplitude(), A0, rtol=0, atol=tol)
+    # bin subset == same bins of the full run, bit for bit; other bins untouched
+    bins = np.array([0, 7, 13, 24])
+    sub = _run(oracle_mod, DIRS, OMEGA, DT, steps, bins=bins)
+    full = base.A.reshape(-1, 3, 2)
+    assert np.array_equal(sub.A.reshape(-1, 3, 2)[bins], full[bins])
+    mask = np.ones(full.shape[0], bool)
+    mask[bins] = False
+    assert np.all(sub.A.reshape(-1, 3, 2)[mask] == 0.0)
+
+
+def test_p6_f32_state_is_promoted_value_for_value(oracle_mod):
+    rng = np.random.default_rng(66)
+    steps32 = _random_steps(rng, 20, 3, dtype=np.float32)
+    steps64 = [(t, [a.astype(np.float64) for a in st]) for t, st in steps32]
+    a32 = _run(oracle_mod, DIRS, OMEGA, DT, steps32).A
+    a64 = _run(oracle_mod, DIRS, OMEGA, DT, steps64).A
+    assert np.array_equal(a32, a64)
+
+
+# ------------------------------------------------------- P7 cyclotron (Schott) harmonics
+@pytest.mark.parametrize("beta_par", [0.0, 0.05, -0.3])
+def test_p7_cyclotron_lines_match_schott_formula(oracle_mod, beta_par):
+    """Single helical electron, M whole gyro-periods, integer steps per period: at
+    w_m = m w_c / (1 - beta_par cos th) the raw |A|^2 equals
+    (2 pi M m)^2 / D^2 [ bp^2 J_m'(x)^2 + ((cos th - beta_par)/sin th)^2 J_m(x)^2 ],
+    x = m bp sin th / D  (Schott / Bekefi; SURVEY.md pin P7)."""
+    wc, bp, M, spp = 1.0e14, 0.1, 3, 40
+    dt = 2.0 * np.pi / wc / spp
+    phi0, r0 = 0.83, np.array([0.3e-6, -0.2e-6, 0.6e-6])
+    rho = C * bp / wc
+    steps = []
+    for t in range(M * spp):
+        ph = wc * t * dt + phi0
+        r = r0 + np.array([rho * (np.sin(ph) - np.sin(phi0)),
+                           rho * (-np.cos(ph) + np.cos(phi0)), C * beta_par * t * dt])
+        steps.append((t, _const_state(r, (bp * np.cos(ph), bp * np.sin(ph), beta_par),
+                                      (-wc * bp * np.sin(ph), wc * bp * np.cos(ph), 0.0))))
+    for theta, az in [(0.4, 0.3), (1.1, -2.0), (np.pi / 2, 1.0), (2.5, 0.1)]:
+        n = np.array([np.sin(theta) * np.cos(az), np.sin(theta) * np.sin(az), np.cos(theta)])
+        D = 1.0 - beta_par * np.cos(theta)
+        ms = np.arange(1, 5)
+        om = ms * wc / D
+        S = _run(oracle_mod, n[None, :], om, dt, steps).spectrum()[0]
+        x = ms * bp * np.sin(theta) / D
+        ref = (2 * np.pi * M * ms) ** 2 / D ** 2 * (
+            bp ** 2 * special.jvp(ms, x) ** 2
+            + ((np.cos(theta) - beta_par) / np.sin(theta)) ** 2 * special.jv(ms, x) ** 2)
+        assert np.allclose(S, ref, rtol=1e-9)
+
+
+def test_p7_off_harmonic_frequencies_are_dark(oracle_mod):
+    """Between the lines (w = (m+1/2) w_c, whole number of periods M even) the sum over
+    periods cancels: |A|^2 is many orders below the neighbouring line."""
+    wc, bp, M, spp = 1.0e14, 0.1, 4, 40
+    dt = 2.0 * np.pi / wc / spp
+    rho = C * bp / wc
+    steps = []
+    for t in range(M * spp):
+        ph = wc * t * dt
+        steps.append((t, _const_state((rho * np.sin(ph), -rho * np.cos(ph), 0.0),
+                                      (bp * np.cos(ph), bp * np.sin(ph), 0.0),
+                                      (-wc * bp * np.sin(ph), wc * bp * np.cos(ph), 0.0))))
+    n = np.array([[np.sin(1.0), 0.0, np.cos(1.0)]])
+    S = _run(oracle_mod, n, np.array([1.0, 1.5, 2.0, 2.5]) * wc, dt, steps).spectrum()[0]
+    assert S[1] < 1e-20 * S[0] and S[3] < 1e-20 * S[2]
+
+
+# --------------------------------------------------------------------- P8 brute force
+def test_p8_bruteforce_numpy_complex128(oracle_mod):
+    rng = np.random.default_rng(8)
+    T, N = 6, 12
+    steps = _random_steps(rng, N, T)
+    t0 = 1.1e-16
+    o = _run(oracle_mod, DIRS, OMEGA, DT, steps, t0=t0)
+    ref = np.zeros((len(DIRS), len(OMEGA), 3), dtype=np.complex128)
+    for t, st in steps:
+        r, be, bd, w = np.stack(st[0:3], 1), np.stack(st[3:6], 1), np.stack(st[6:9], 1), st[9]
+        for i, n in enumerate(UNIT):
+            for k in range(N):
+                vec = np.cross(n, np.cross(n - be[k], bd[k]))
+                a = w[k] * vec / (1.0 - be[k] @ n) ** 2
+                tret = t0 + t * DT - (n @ r[k]) / C
+                ref[i] += a[None, :] * np.exp(1j * OMEGA * tret)[:, None] * DT
+    assert np.allclose(o.amplitude(), ref, rtol=0, atol=1e-12 * np.abs(ref).max())
+    assert np.allclose(o.spectrum(), (np.abs(ref) ** 2).sum(-1), rtol=1e-11)
+
+
+def test_p8_bruteforce_mpmath_tiny(oracle_mod):
+    mp = pytest.importorskip("mpmath")
+    mp.mp.dps = 40
+    rng = np.random.default_rng(88)
+    steps = _random_steps(rng, 2, 3)
+    dirs, om = DIRS[2:4], OMEGA[3:5]          # the large-phase bins
+    o = _run(oracle_mod, dirs, om, DT, steps)
+    for i, nraw in enumerate(dirs):
+        nn = [mp.mpf(float(v)) for v in nraw]
+        nrm = mp.sqrt(sum(v * v for v in nn))
+        n = [v / nrm for v in nn]
+        for j, w_j in enumerate(om):
+            acc = [mp.mpc(0)] * 3
+            for t, st in steps:
+                for k in range(2):
+                    r, be, bd = ([mp.mpf(float(st[c + o3][k])) for c in range(3)] for o3 in (0, 3, 6))
+                    wk = mp.mpf(float(st[9][k]))
+                    d = 1 - sum(be[c] * n[c] for c in range(3))
+                    g = [n[c] - be[c] for c in range(3)]
+                    inner = [g[1] * bd[2] - g[2] * bd[1], g[2] * bd[0] - g[0] * bd[2],
+                             g[0] * bd[1] - g[1] * bd[0]]
+                    outer = [n[1] * inner[2] - n[2] * inner[1], n[2] * inner[0] - n[0] * inner[2],
+                             n[0] * inner[1] - n[1] * inner[0]]
+                    tau = mp.mpf(t) * mp.mpf(DT) - sum(n[c] * r[c] for c in range(3)) / mp.mpf(C)
+                    ph = mp.expj(mp.mpf(float(w_j)) * tau)
+                    for c in range(3):
+                        acc[c] += wk * mp.mpf(DT) * outer[c] / d ** 2 * ph
+            got = o.amplitude()[i, j]
+            scale = max(abs(complex(a)) for a in acc)
+            for c in range(3):
+                assert abs(got[c] - complex(acc[c])) <= 1e-11 * scale
+
+
+# ------------------------------------------------------------------------ P9 SI constant
+def test_p9_default_scale_is_e2_over_16pi3eps0c(oracle_mod):
+    assert oracle_mod.default_scale() == pytest.approx(1.949313784587704e-38, rel=1e-9)
+    # scale == 0 selects it
+    st = _const_state((0, 0, 0), (0, 0, 0), (1e12, 0, 0))
+    s_default = _run(oracle_mod, DIRS, OMEGA, DT, [(0, st)], scale=0.0).spectrum()
+    s_unit = _run(oracle_mod, DIRS, OMEGA, DT, [(0, st)], scale=1.0).spectrum()
+    assert np.allclose(s_default, s_unit * 1.949313784587704e-38, rtol=1e-9)
+
+
+# ----------------------------------------------------------------- P10 Larmor / Parseval
+def test_p10_frequency_integral_matches_angular_power(oracle_mod):
+    """int_0^inf S dw = pi * sum_t |n x ((n-beta) x betadot)|^2/(1-beta.n)^5 dt  (raw scale=1),
+    the retarded-time power law (Jackson 14.38): pins the (1-beta.n) powers jointly with P4."""
+    wc, bp, bz, M, spp = 1.0e14, 0.3, 0.2, 4, 1024
+    dt = 2.0 * np.pi / wc / spp
+    rho = C * bp / wc
+    n = np.array([np.sin(0.9) * np.cos(0.4), np.sin(0.9) * np.sin(0.4), np.cos(0.9)])
+    steps, power = [], 0.0
+    for t in range(M * spp):
+        ph = wc * t * dt
+        be = np.array([bp * np.cos(ph), bp * np.sin(ph), bz])
+        bd = np.array([-wc * bp * np.sin(ph), wc * bp * np.cos(ph), 0.0])
+        r = np.array([rho * np.sin(ph), -rho * np.cos(ph), C * bz * t * dt])
+        steps.append((t, _const_state(r, be, bd)))
+        d = 1.0 - be @ n
+        vec = (n - be) * (n @ bd) - bd * d
+        power += (vec @ vec) / d ** 5 * dt
+        if t == 0:
+            jump2 = (vec @ vec) / d ** 6       # |a(tau)|^2 at the window edge, a(tau)=vec/d^3
+    # dense linear grid well past the highest significant harmonic; lines have width
+    # ~ w_c/M, resolved with w_c/(16 M) spacing
+    om = np.arange(1, 16 * M * 40 + 1) * (wc / (16.0 * M))
+    S = _run(oracle_mod, n[None, :], om, dt, steps).spectrum()[0]
+    dw = om[1] - om[0]
+    # the rectangular time window gives |A|^2 a (|J0|^2+|J1|^2)/w^2 tail (J = jump of the
+    # observer-time signal at either edge; equal by periodicity): add it beyond the grid
+    integral = np.sum(S) * dw + 2.0 * jump2 / (om[-1] + 0.5 * dw)
+    assert integral == pytest.approx(np.pi * power, rel=2e-4)
