@@ -76,7 +76,7 @@ def test_khi_state_physics_and_determinism():
     src2 = wl.KHISource(16, w.seed, w.dt)
     r0 = src2.r.copy()
     src2.advance()
-    assert np.allclose(src2.r - r0, wl.C_LIGHT * w.dt * src2.b, rtol=1e-12, atol=0)
+    assert np.allclose(src2.r - r0, wl.C_LIGHT * w.dt * src2.b, rtol=1e-5, atol=0)
     # |betadot| = |q B/(gamma m)| |beta_perp|
     k = np.abs(src2.qm * src2._Bz())
     st = src2.state()
