@@ -1,0 +1,142 @@
+/*
+ * rad.h -- C ABI of the B200-native far-field radiation detector.
+ *
+ * The operation (BASELINE.json north_star; "the far-field radiation
+ * plugin calculates radiation emissions using the Lienard-Wiechert potential approach";
+ * line 74 "a weighted sum of all contributions from all particles"; lines 79-81 "at each
+ * PIConGPU time step ... the sum of the contributions from all radiating particles ...
+ * the complex amplitude and phase for each wavelength and direction"):
+ *
+ *   A(n, w_j) = sum over steps t, particles k of
+ *                 w_k * [ n x ((n - beta_k) x betadot_k) ] / (1 - beta_k.n)^2
+ *                     * exp( i w_j ( t0 + t*dt - n.r_k/c ) ) * dt
+ *   S(n, w_j) = scale * |A(n, w_j)|^2              (d^2 I / dOmega dw)
+ *
+ * on a grid of n_dir observation directions n and n_omega angular frequencies w_j.
+ * Units are SI: r [m], beta = v/c [1], betadot [1/s], omega [rad/s], dt [s];
+ * c = 299 792 458 m/s.  Readings of the paper where it is silent: DESIGN.md.
+ *
+ * Conventions
+ *   - No C++/torch types cross this boundary: plain pointers, sizes and scalars.
+ *     Every pointer argument says HOST or DEVICE.
+ *   - Particle state is structure-of-arrays: 10 arrays (rx ry rz bx by bz bdx bdy bdz w)
+ *     of n_particles elements of `state_dtype` (40 B per particle in fp32).
+ *     The caller owns them; the library never copies (except the *_host entry), frees or
+ *     writes them; they must stay valid until the work queued on `cuda_stream` completes.
+ *   - Every call is asynchronous on `cuda_stream` (a cudaStream_t passed as void*, NULL =
+ *     the legacy default stream) unless it returns data to HOST memory, in which case it
+ *     synchronises that stream before returning.
+ *   - A handle is not thread-safe; distinct handles are independent.  All work of a
+ *     handle must be issued on streams the caller orders correctly (the library adds no
+ *     cross-stream dependency between calls).
+ *   - No exception crosses the ABI.  Every function returns a rad_status; details via
+ *     rad_last_error().  Particle values are not scanned: NaN/Inf or 1 - beta.n = 0 in the
+ *     state give NaN/Inf in the result (documented, caller's responsibility).
+ *   - There is no CPU fallback: without a CUDA device rad_create fails with RAD_ERR_CUDA.
+ */
+#ifndef RAD_H_
+#define RAD_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RAD_API __attribute__((visibility("default")))
+
+typedef struct rad_handle rad_handle; /* opaque, library-owned */
+
+typedef enum {
+    RAD_OK = 0,
+    RAD_ERR_INVALID_ARG = 1, /* NULL/negative/non-finite argument, zero direction, unsorted omega */
+    RAD_ERR_ALLOC = 2,       /* host or device allocation failed */
+    RAD_ERR_CUDA = 3,        /* a CUDA runtime call or kernel launch failed / no device */
+    RAD_ERR_STATE = 4,       /* handle unusable (a previous CUDA error) */
+    RAD_ERR_UNSUPPORTED = 5  /* valid request this build does not implement */
+} rad_status;
+
+typedef enum { RAD_F32 = 0, RAD_F64 = 1 } rad_dtype;
+
+/* rad_config.flags */
+#define RAD_FLAG_DETERMINISTIC 1u /* bit 0: no floating-point atomics; results are
+                                     bit-reproducible run to run (slower, more memory) */
+#define RAD_FLAG_FORCE_GENERAL 2u /* bit 1: never use the uniform-grid recurrence kernel */
+
+typedef struct {
+    uint32_t struct_size;  /* = sizeof(rad_config); ABI versioning                         */
+    int32_t device;        /* CUDA device ordinal                                          */
+    int32_t n_dir;         /* >= 1                                                         */
+    int32_t n_omega;       /* >= 1                                                         */
+    const double *dirs;    /* HOST [n_dir][3]; any non-zero length, normalised in fp64     */
+    const double *omega;   /* HOST [n_omega] rad/s; finite, > 0, strictly increasing       */
+    double dt;             /* s, > 0: the quadrature weight of every term                  */
+    double t0;             /* s: time of step_index 0                                      */
+    double scale;          /* S = scale*|A|^2; 0 -> SI e^2/(16 pi^3 eps0 c) J s            */
+    int32_t state_dtype;   /* rad_dtype of the 10 particle arrays                          */
+    uint32_t flags;        /* RAD_FLAG_*                                                   */
+} rad_config;
+
+/* Create a detector: copies dirs/omega, builds the device tables, zeroes A.
+ * *out is set to NULL on failure. */
+RAD_API rad_status rad_create(const rad_config *cfg, rad_handle **out);
+
+/* A += contributions of n_particles particles at time t0 + step_index*dt.
+ * All 10 arrays DEVICE, `state_dtype` elements, 16-byte aligned not required.
+ * n_particles == 0 is a no-op.  Calls are additive: several calls with the same
+ * step_index superpose (particle subsets), any order of steps gives the same A up to
+ * rounding. */
+RAD_API rad_status rad_accumulate_step(rad_handle *h, int64_t step_index, int64_t n_particles,
+                                       const void *rx, const void *ry, const void *rz,
+                                       const void *bx, const void *by, const void *bz,
+                                       const void *bdx, const void *bdy, const void *bdz,
+                                       const void *w, void *cuda_stream);
+
+/* Same, state in HOST memory (pinned memory makes the copies asynchronous).  The
+ * library stages the arrays through its own double-buffered device buffer: the
+ * host->device copy of one call overlaps the kernels of the previous call.  The host
+ * arrays may be reused as soon as the call returns only if they are pageable; pinned
+ * arrays must stay untouched until `cuda_stream` has passed this call. */
+RAD_API rad_status rad_accumulate_step_host(rad_handle *h, int64_t step_index, int64_t n_particles,
+                                            const void *rx, const void *ry, const void *rz,
+                                            const void *bx, const void *by, const void *bz,
+                                            const void *bdx, const void *bdy, const void *bdz,
+                                            const void *w, void *cuda_stream);
+
+/* out[n_dir][n_omega] (row-major, fp64) = scale * sum_c |A_c|^2.  Non-destructive.
+ * out_on_device != 0: `out` is DEVICE memory, call is asynchronous; else HOST and the
+ * call returns after the data has arrived. */
+RAD_API rad_status rad_spectrum(rad_handle *h, double *out, int out_on_device, void *cuda_stream);
+
+/* out[n_dir][n_omega][3][2] fp64: (re, im) of the x, y, z components of A
+ * ("complex amplitude and phase for each wavelength and direction"). */
+RAD_API rad_status rad_amplitude(rad_handle *h, double *out, int out_on_device, void *cuda_stream);
+
+/* A := A + amp, amp DEVICE [n_dir][n_omega][3][2] fp64 in the rad_amplitude layout.
+ * For the multi-GPU sum: ranks all-reduce rad_amplitude() buffers (amplitudes, not
+ * intensities, must be summed -- PAPER.md line 80 "sum of the contributions from all
+ * radiating particles in the simulation"), rad_reset(), then add the reduced buffer. */
+RAD_API rad_status rad_add_amplitude(rad_handle *h, const double *amp_device, void *cuda_stream);
+
+/* A := 0 (start a new accumulation window). */
+RAD_API rad_status rad_reset(rad_handle *h, void *cuda_stream);
+
+/* Frees everything the handle owns after synchronising the device.  NULL-safe. */
+RAD_API void rad_destroy(rad_handle *h);
+
+/* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
+RAD_API int64_t rad_launch_count(const rad_handle *h);
+
+/* Name of the accumulation kernel variant the last rad_accumulate_step used
+ * ("general", "uniform", ...), static storage. */
+RAD_API const char *rad_kernel_variant(const rad_handle *h);
+
+RAD_API const char *rad_status_string(rad_status s);
+/* Message of the last failing call on this handle (h == NULL: last rad_create failure). */
+RAD_API const char *rad_last_error(const rad_handle *h);
+RAD_API const char *rad_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RAD_H_ */

@@ -1,0 +1,254 @@
+"""Thin ctypes binding of include/rad.h -- argument marshalling only.
+
+Same names as the C ABI (rad_create, rad_accumulate_step, rad_spectrum, ...), plus a small
+`Detector` convenience class that owns a handle.  torch is used for device memory and
+streams only; every step of the path runs in the CUDA kernels of librad.so.  There is no
+CPU fallback: if the library is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+from typing import Optional, Sequence
+
+import numpy as np
+
+_PKG = Path(__file__).resolve().parent
+LIB_PATH = _PKG / "librad.so"
+
+RAD_OK, RAD_ERR_INVALID_ARG, RAD_ERR_ALLOC, RAD_ERR_CUDA, RAD_ERR_STATE, RAD_ERR_UNSUPPORTED = range(6)
+RAD_F32, RAD_F64 = 0, 1
+RAD_FLAG_DETERMINISTIC, RAD_FLAG_FORCE_GENERAL = 1, 2
+
+ABI_SYMBOLS = (
+    "rad_create", "rad_accumulate_step", "rad_accumulate_step_host", "rad_spectrum",
+    "rad_amplitude", "rad_add_amplitude", "rad_reset", "rad_destroy", "rad_launch_count",
+    "rad_kernel_variant", "rad_status_string", "rad_last_error", "rad_version",
+)
+
+
+class rad_config(ctypes.Structure):
+    _fields_ = [
+        ("struct_size", ctypes.c_uint32), ("device", ctypes.c_int32),
+        ("n_dir", ctypes.c_int32), ("n_omega", ctypes.c_int32),
+        ("dirs", ctypes.c_void_p), ("omega", ctypes.c_void_p),
+        ("dt", ctypes.c_double), ("t0", ctypes.c_double), ("scale", ctypes.c_double),
+        ("state_dtype", ctypes.c_int32), ("flags", ctypes.c_uint32),
+    ]
+
+
+class RadError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{status_string(status)}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def load(path: Optional[Path] = None) -> ctypes.CDLL:
+    """Load librad.so (built in-tree by paper_2501_03383_b200.build).  Fails loudly."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    p = Path(path) if path else LIB_PATH
+    if not p.exists():
+        raise FileNotFoundError(
+            f"{p} not found: build it with `python -m paper_2501_03383_b200.build` "
+            "(there is no CPU fallback)")
+    lib = ctypes.CDLL(str(p))
+    vp, i64, dbl = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double
+    lib.rad_create.restype = ctypes.c_int
+    lib.rad_create.argtypes = [ctypes.POINTER(rad_config), ctypes.POINTER(vp)]
+    for name in ("rad_accumulate_step", "rad_accumulate_step_host"):
+        f = getattr(lib, name)
+        f.restype = ctypes.c_int
+        f.argtypes = [vp, i64, i64] + [vp] * 10 + [vp]
+    for name in ("rad_spectrum", "rad_amplitude"):
+        f = getattr(lib, name)
+        f.restype = ctypes.c_int
+        f.argtypes = [vp, vp, ctypes.c_int, vp]
+    lib.rad_add_amplitude.restype = ctypes.c_int
+    lib.rad_add_amplitude.argtypes = [vp, vp, vp]
+    lib.rad_reset.restype = ctypes.c_int
+    lib.rad_reset.argtypes = [vp, vp]
+    lib.rad_destroy.restype = None
+    lib.rad_destroy.argtypes = [vp]
+    lib.rad_launch_count.restype = i64
+    lib.rad_launch_count.argtypes = [vp]
+    for name in ("rad_kernel_variant", "rad_last_error"):
+        f = getattr(lib, name)
+        f.restype = ctypes.c_char_p
+        f.argtypes = [vp]
+    lib.rad_status_string.restype = ctypes.c_char_p
+    lib.rad_status_string.argtypes = [ctypes.c_int]
+    lib.rad_version.restype = ctypes.c_char_p
+    lib.rad_version.argtypes = []
+    if path is None:
+        _lib = lib
+    return lib
+
+
+def status_string(status: int) -> str:
+    return load().rad_status_string(int(status)).decode()
+
+
+def rad_version() -> str:
+    return load().rad_version().decode()
+
+
+def _check(status: int, handle) -> None:
+    if status != RAD_OK:
+        raise RadError(status, (load().rad_last_error(handle) or b"").decode())
+
+
+# ------------------------------------------------------------------ ABI-named functions
+def rad_create(dirs, omega, dt: float, t0: float = 0.0, scale: float = 0.0,
+               state_dtype: int = RAD_F32, flags: int = 0, device: int = 0) -> int:
+    """-> opaque handle (int).  dirs [D,3], omega [W]: HOST fp64 (copied by the library)."""
+    dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
+    omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
+    cfg = rad_config(ctypes.sizeof(rad_config), device, dirs.shape[0], omega.shape[0],
+                     dirs.ctypes.data, omega.ctypes.data, dt, t0, scale, state_dtype, flags)
+    h = ctypes.c_void_p()
+    _check(load().rad_create(ctypes.byref(cfg), ctypes.byref(h)), None)
+    return h.value
+
+
+def rad_accumulate_step(handle: int, step_index: int, n_particles: int, state_ptrs: Sequence[int],
+                        stream: int = 0) -> None:
+    """state_ptrs: 10 DEVICE pointers (rx ry rz bx by bz bdx bdy bdz w)."""
+    _check(load().rad_accumulate_step(handle, step_index, n_particles, *state_ptrs, stream), handle)
+
+
+def rad_accumulate_step_host(handle: int, step_index: int, n_particles: int,
+                             state_ptrs: Sequence[int], stream: int = 0) -> None:
+    """state_ptrs: 10 HOST pointers."""
+    _check(load().rad_accumulate_step_host(handle, step_index, n_particles, *state_ptrs, stream), handle)
+
+
+def rad_spectrum(handle: int, out_ptr: int, out_on_device: bool, stream: int = 0) -> None:
+    _check(load().rad_spectrum(handle, out_ptr, int(out_on_device), stream), handle)
+
+
+def rad_amplitude(handle: int, out_ptr: int, out_on_device: bool, stream: int = 0) -> None:
+    _check(load().rad_amplitude(handle, out_ptr, int(out_on_device), stream), handle)
+
+
+def rad_add_amplitude(handle: int, amp_device_ptr: int, stream: int = 0) -> None:
+    _check(load().rad_add_amplitude(handle, amp_device_ptr, stream), handle)
+
+
+def rad_reset(handle: int, stream: int = 0) -> None:
+    _check(load().rad_reset(handle, stream), handle)
+
+
+def rad_destroy(handle: Optional[int]) -> None:
+    load().rad_destroy(handle)
+
+
+def rad_launch_count(handle: int) -> int:
+    return int(load().rad_launch_count(handle))
+
+
+def rad_kernel_variant(handle: int) -> str:
+    return load().rad_kernel_variant(handle).decode()
+
+
+# ------------------------------------------------------------------ convenience wrapper
+class Detector:
+    """Owns one rad_handle.  State may be torch CUDA tensors (device path) or numpy /
+    pinned torch CPU tensors (host path, copies inside the library)."""
+
+    def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, state_dtype=np.float32, flags=0, device=0):
+        self.D = int(np.asarray(dirs).reshape(-1, 3).shape[0])
+        self.W = int(np.asarray(omega).reshape(-1).shape[0])
+        self.np_dtype = np.dtype(state_dtype)
+        code = {np.dtype(np.float32): RAD_F32, np.dtype(np.float64): RAD_F64}[self.np_dtype]
+        self.device = device
+        self.handle = rad_create(dirs, omega, dt, t0, scale, code, flags, device)
+
+    # -- helpers
+    @staticmethod
+    def _stream() -> int:
+        import torch
+        return int(torch.cuda.current_stream().cuda_stream)
+
+    def _ptrs(self, state, want_cuda: bool):
+        import torch
+        if len(state) != 10:
+            raise ValueError("state must be 10 arrays: rx ry rz bx by bz bdx bdy bdz w")
+        n, ptrs = None, []
+        for a in state:
+            if isinstance(a, torch.Tensor):
+                if a.is_cuda != want_cuda or not a.is_contiguous() or a.dim() != 1:
+                    raise ValueError("state tensors must be 1-D contiguous and on the expected device")
+                if a.element_size() != self.np_dtype.itemsize or not a.dtype.is_floating_point:
+                    raise TypeError("state dtype does not match the detector's state_dtype")
+                ptrs.append(a.data_ptr()); m = a.numel()
+            else:
+                if want_cuda or a.dtype != self.np_dtype or not a.flags.c_contiguous or a.ndim != 1:
+                    raise ValueError("host state must be 1-D contiguous numpy arrays of state_dtype")
+                ptrs.append(a.ctypes.data); m = a.shape[0]
+            if n is not None and m != n:
+                raise ValueError("state arrays differ in length")
+            n = m
+        return n, ptrs
+
+    # -- ABI calls
+    def accumulate_step(self, step_index: int, state) -> None:
+        n, ptrs = self._ptrs(state, want_cuda=True)
+        rad_accumulate_step(self.handle, step_index, n, ptrs, self._stream())
+
+    def accumulate_step_host(self, step_index: int, state) -> None:
+        n, ptrs = self._ptrs(state, want_cuda=False)
+        rad_accumulate_step_host(self.handle, step_index, n, ptrs, self._stream())
+
+    def spectrum(self, out=None):
+        """out: optional torch CUDA fp64 tensor [D, W] (asynchronous); default -> numpy."""
+        if out is not None:
+            rad_spectrum(self.handle, out.data_ptr(), True, self._stream())
+            return out
+        res = np.empty((self.D, self.W), dtype=np.float64)
+        rad_spectrum(self.handle, res.ctypes.data, False, self._stream())
+        return res
+
+    def amplitude(self, out=None):
+        """Complex amplitude; default -> numpy complex128 [D, W, 3]."""
+        if out is not None:
+            rad_amplitude(self.handle, out.data_ptr(), True, self._stream())
+            return out
+        res = np.empty((self.D, self.W, 3, 2), dtype=np.float64)
+        rad_amplitude(self.handle, res.ctypes.data, False, self._stream())
+        return res[..., 0] + 1j * res[..., 1]
+
+    def add_amplitude(self, amp) -> None:
+        rad_add_amplitude(self.handle, amp.data_ptr(), self._stream())
+
+    def reset(self) -> None:
+        rad_reset(self.handle, self._stream())
+
+    @property
+    def launch_count(self) -> int:
+        return rad_launch_count(self.handle)
+
+    @property
+    def kernel_variant(self) -> str:
+        return rad_kernel_variant(self.handle)
+
+    def close(self) -> None:
+        if getattr(self, "handle", None):
+            rad_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()

@@ -1,0 +1,108 @@
+// rad_finalize.cu -- a4: |A|^2 and normalisation, amplitude export /
+// import in Cartesian components, and the deterministic reduction of per-chunk partials.
+// All fp64, one thread per (direction, frequency) bin; bandwidth-trivial (<= a few MB).
+#include "rad_internal.h"
+
+namespace rad {
+
+namespace {
+
+// S[n][j] = scale * (|A1|^2 + |A2|^2); (e1, e2, n) is orthonormal and A . n = 0, so this
+// equals scale * (|Ax|^2 + |Ay|^2 + |Az|^2).
+__global__ void rad_spectrum_kernel(const double *__restrict__ acc, double *__restrict__ out,
+                                    int D, int W, int w_pad, double scale)
+{
+    const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= (long long)D * W) return;
+    const int d = (int)(b / W), j = (int)(b - (long long)d * W);
+    const double2 *a = reinterpret_cast<const double2 *>(acc + ((size_t)d * w_pad + j) * 4);
+    const double2 a1 = a[0], a2 = a[1];
+    out[b] = scale * (a1.x * a1.x + a1.y * a1.y + a2.x * a2.x + a2.y * a2.y);
+}
+
+// A_xyz = A1 e1 + A2 e2  ->  out[n][j][3][2]
+__global__ void rad_amplitude_kernel(const double *__restrict__ acc, const DirRec *__restrict__ dirs,
+                                     const double *__restrict__ basis, double *__restrict__ out,
+                                     int D, int W, int w_pad)
+{
+    const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= (long long)D * W) return;
+    const int d = (int)(b / W), j = (int)(b - (long long)d * W);
+    const double2 *a = reinterpret_cast<const double2 *>(acc + ((size_t)d * w_pad + j) * 4);
+    const double2 a1 = a[0], a2 = a[1];
+    const double *e = basis + (size_t)d * 6;  // fp64 e1, e2
+    double *o = out + (size_t)b * 6;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        o[2 * c + 0] = a1.x * e[c] + a2.x * e[3 + c];
+        o[2 * c + 1] = a1.y * e[c] + a2.y * e[3 + c];
+    }
+}
+
+// A1 += e1 . amp, A2 += e2 . amp
+__global__ void rad_add_amplitude_kernel(double *__restrict__ acc, const double *__restrict__ basis,
+                                         const double *__restrict__ amp, int D, int W, int w_pad)
+{
+    const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= (long long)D * W) return;
+    const int d = (int)(b / W), j = (int)(b - (long long)d * W);
+    const double *e = basis + (size_t)d * 6;
+    const double *in = amp + (size_t)b * 6;
+    double r1 = 0, i1 = 0, r2 = 0, i2 = 0;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        r1 += e[c] * in[2 * c];
+        i1 += e[c] * in[2 * c + 1];
+        r2 += e[3 + c] * in[2 * c];
+        i2 += e[3 + c] * in[2 * c + 1];
+    }
+    double *a = acc + ((size_t)d * w_pad + j) * 4;
+    a[0] += r1; a[1] += i1; a[2] += r2; a[3] += i2;
+}
+
+// deterministic mode: acc[e] += sum over chunks (fixed order) of partial[chunk][e]
+__global__ void rad_reduce_partials_kernel(double *__restrict__ acc, const double *__restrict__ partial,
+                                           long long n_elem, int n_chunks)
+{
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n_elem) return;
+    double s = 0.0;
+    for (int c = 0; c < n_chunks; ++c) s += partial[(size_t)c * n_elem + e];
+    acc[e] += s;
+}
+
+inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) / t); }
+
+}  // namespace
+
+cudaError_t launch_spectrum(const Handle &h, double *out_dev, cudaStream_t s)
+{
+    const long long n = (long long)h.D * h.W;
+    rad_spectrum_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, out_dev, h.D, h.W, h.w_pad, h.scale);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_amplitude(const Handle &h, double *out_dev, cudaStream_t s)
+{
+    const long long n = (long long)h.D * h.W;
+    rad_amplitude_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, h.dirs_d, h.basis_d, out_dev,
+                                                            h.D, h.W, h.w_pad);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_add_amplitude(const Handle &h, const double *amp_dev, cudaStream_t s)
+{
+    const long long n = (long long)h.D * h.W;
+    rad_add_amplitude_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, h.basis_d, amp_dev, h.D,
+                                                                h.W, h.w_pad);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_reduce_partials(const Handle &h, const double *partial, int n_chunks, cudaStream_t s)
+{
+    const long long n = (long long)h.D * h.w_pad * 4;
+    rad_reduce_partials_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, partial, n, n_chunks);
+    return cudaGetLastError();
+}
+
+}  // namespace rad

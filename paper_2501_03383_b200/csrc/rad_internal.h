@@ -1,0 +1,99 @@
+// rad_internal.h -- host/device shared declarations of the CUDA path (NOT part of the ABI).
+//
+// Notation follows BASELINE.json north_star / SURVEY.md section 8: N particles, D directions n,
+// W frequencies w_j = 2 pi f_j, A(n, w_j) complex amplitude, S = scale |A|^2.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "rad.h"
+
+namespace rad {
+
+constexpr double kC = 299792458.0;             // m/s
+constexpr double kTwo32 = 4294967296.0;        // 2^32
+constexpr int kWarpsPerBlock = 4;              // one warp per SM sub-partition
+constexpr int kThreads = 32 * kWarpsPerBlock;
+constexpr int kBatch = 32;                     // particles staged per warp batch (one per lane)
+
+// Per direction (device table).  k = n * (f_unit 2^32 / c): the dot product k.r is the
+// light-travel delay n.r/c measured in units of 2^-32 "unit turns" (phase).
+struct DirRec {
+    double kx, ky, kz;     // fp64: phase path
+    double nx, ny, nz;     // fp64 unit vector: Doppler factor d = 1 - n.beta
+    float nfx, nfy, nfz;   // fp32 copy for n.betadot
+    float e1x, e1y, e1z;   // transverse orthonormal basis, e1 x e2 = n (A is _|_ n exactly)
+    float e2x, e2y, e2z;
+    float pad[3];
+};
+static_assert(sizeof(DirRec) == 96, "DirRec layout");
+
+// Everything the accumulate kernels need, passed by value.
+struct AccumParams {
+    const void *st[10];    // rx ry rz bx by bz bdx bdy bdz w (DEVICE, float or double)
+    long long n_particles;
+    int chunk;             // particles per block (multiple of kBatch)
+    int n_dir, n_omega;    // D, W
+    int w_pad;             // W padded to the frequency tile
+    int n_ftiles;          // frequency tiles per direction group
+    int n_wtiles;          // warp tiles = direction groups * n_ftiles
+    const DirRec *dirs;    // [D]
+    const uint32_t *F;     // [w_pad] integer part of f_j / f_unit
+    const float *Ff;       // [w_pad] (float)F_j
+    const float *fl;       // [w_pad] f_j / f_unit - F_j  in [-0.5, 0.5]
+    double ts32;           // (t0 + step dt) f_unit 2^32
+    float dt;              // quadrature weight
+    double *acc;           // [D][w_pad][4]: A1.re A1.im A2.re A2.im (transverse components)
+    double *partial;       // deterministic mode: [n_chunks][D][w_pad][4], else NULL
+    // uniform-grid variant only
+    double f0_unit, df_unit;  // f_0 / f_unit and (f_1 - f_0)/f_unit
+};
+
+struct Handle;
+
+// kernels/launchers (rad_kernels.cu, rad_finalize.cu)
+cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_f64,
+                              cudaStream_t s, int *n_launches, const char **variant);
+cudaError_t launch_spectrum(const Handle &h, double *out_dev, cudaStream_t s);
+cudaError_t launch_amplitude(const Handle &h, double *out_dev, cudaStream_t s);
+cudaError_t launch_add_amplitude(const Handle &h, const double *amp_dev, cudaStream_t s);
+cudaError_t launch_reduce_partials(const Handle &h, const double *partial, int n_chunks,
+                                   cudaStream_t s);
+
+struct Handle {
+    int device = 0;
+    int D = 0, W = 0, w_pad = 0;
+    int lw = 32, strip = 8;          // lanes along frequency, bins per lane
+    int n_ftiles = 0, n_wtiles = 0;
+    double dt = 0, t0 = 0, scale = 0, f_unit = 0;
+    bool state_f64 = false, deterministic = false, uniform = false;
+    double f0_unit = 0, df_unit = 0;
+    int sm_count = 148;
+    std::vector<double> dirs_h;      // normalised [D][3]
+    std::vector<double> omega_h;
+    DirRec *dirs_d = nullptr;
+    double *basis_d = nullptr;       // [D][6] fp64 e1, e2 (amplitude export/import)
+    uint32_t *F_d = nullptr;
+    float *Ff_d = nullptr, *fl_d = nullptr;
+    double *acc_d = nullptr;         // [D][w_pad][4]
+    double *partial_d = nullptr;     // deterministic workspace
+    size_t partial_bytes = 0;
+    // host-state staging (rad_accumulate_step_host): two device buffers, copy stream
+    void *stage_d[2] = {nullptr, nullptr};
+    size_t stage_bytes[2] = {0, 0};
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr};
+    bool consumed_valid[2] = {false, false};
+    int stage_next = 0;
+    double *out_d = nullptr;         // scratch for HOST-destination results
+    size_t out_bytes = 0;
+    int64_t launches = 0;
+    const char *variant = "none";
+    bool broken = false;
+    std::string err;
+};
+
+}  // namespace rad

@@ -1,0 +1,224 @@
+// rad_kernels.cu -- accumulation kernels (SURVEY.md section 8(a) rows a1, a2, a2', a3) for sm_100a.
+//
+// Mapping ("bin owner"): a thread owns S frequency bins of one direction and keeps their
+// transverse complex amplitudes (A1, A2) in fp32 registers; a warp owns DPW = 32/LW
+// directions x (LW*S) frequencies; the 4 warps of a block own 4 such tiles and share one
+// chunk of particles.  Per batch of 32 particles each lane stages ONE particle for the
+// warp's directions (a1: coalesced SoA loads, fp64 phase set-up, fp32 amplitude) into the
+// warp's private shared-memory records; then all lanes sweep the 32 records (a2), reading
+// them as shared-memory broadcasts.  No block-level barrier anywhere.
+//
+// Phase: turns = f_j tau, tau = t - n.r/c.  With
+// f_j = (F_j + phi_j) f_unit (F_j a 32-bit integer, |phi_j| <= 1/2) and
+// s32 = tau f_unit 2^32 = I + res (I integer, |res| <= 1/2, both from fp64):
+//   frac(turns) = frac( (F_j * (I mod 2^32) mod 2^32) / 2^32  +  F_j res / 2^32  +  phi_j s )
+// The first term is ONE 32-bit integer multiply (wrap-around = exact reduction mod one turn
+// for any |tau|); the other two are O(1/2 turn) and O(tau f_unit) and are added in fp32.
+#include <math_constants.h>
+
+#include "rad_internal.h"
+
+namespace rad {
+
+namespace {
+
+constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: fp64 round-to-integer constant
+constexpr float kTwoPi = 6.283185307179586f;
+constexpr float kUnitToRad = 1.4629180792671596e-09f;  // 2 pi / 2^32
+
+template <typename ST>
+__device__ __forceinline__ ST ld_state(const void *p, long long k)
+{
+    return __ldg(reinterpret_cast<const ST *>(p) + k);
+}
+
+// a1: stage one particle for one direction -> record {T, ql, a1, a2} + sf.
+struct Particle {
+    double rx, ry, rz, bx, by, bz;  // fp64 for the phase and the Doppler factor
+    float bfx, bfy, bfz, bdx, bdy, bdz, wdt;
+};
+
+__device__ __forceinline__ void stage_record(const Particle &p, const DirRec &dr, double ts32,
+                                             float4 &rec, float &sf)
+{
+    // phase: s32 = (t - n.r/c) f_unit 2^32 in fp64, split into integer (mod 2^32) + residual
+    const double s32 = ts32 - fma(dr.kx, p.rx, fma(dr.ky, p.ry, dr.kz * p.rz));
+    const double m = s32 + kMagic;
+    const uint32_t T = (uint32_t)__double2loint(m);
+    const double res = s32 - (m - kMagic);
+    // Doppler factor d = 1 - n.beta in fp64 (no cancellation error for beta -> 1)
+    const double d64 = 1.0 - fma(dr.nx, p.bx, fma(dr.ny, p.by, dr.nz * p.bz));
+    const float d = (float)d64;
+    // amplitude: n x ((n-beta) x bd) = (n-beta)(n.bd) - bd (1-n.beta); it is _|_ n, so its
+    // components on the transverse basis are a_i = -(e_i.beta)(n.bd) - (e_i.bd) d
+    const float g = fmaf(dr.nfx, p.bdx, fmaf(dr.nfy, p.bdy, dr.nfz * p.bdz));
+    const float e1b = fmaf(dr.e1x, p.bfx, fmaf(dr.e1y, p.bfy, dr.e1z * p.bfz));
+    const float e2b = fmaf(dr.e2x, p.bfx, fmaf(dr.e2y, p.bfy, dr.e2z * p.bfz));
+    const float e1d = fmaf(dr.e1x, p.bdx, fmaf(dr.e1y, p.bdy, dr.e1z * p.bdz));
+    const float e2d = fmaf(dr.e2x, p.bdx, fmaf(dr.e2y, p.bdy, dr.e2z * p.bdz));
+    const float inv = 1.0f / d;
+    const float pre = -p.wdt * inv * inv;  // -w dt / d^2
+    rec.x = __uint_as_float(T);
+    rec.y = (float)res * kUnitToRad;
+    rec.z = pre * fmaf(e1b, g, e1d * d);
+    rec.w = pre * fmaf(e2b, g, e2d * d);
+    sf = (float)s32 * kUnitToRad;
+}
+
+template <typename ST>
+__device__ __forceinline__ Particle load_particle(const AccumParams &P, long long k, bool valid)
+{
+    Particle p;
+    if (valid) {
+        const ST rx = ld_state<ST>(P.st[0], k), ry = ld_state<ST>(P.st[1], k),
+                 rz = ld_state<ST>(P.st[2], k);
+        const ST bx = ld_state<ST>(P.st[3], k), by = ld_state<ST>(P.st[4], k),
+                 bz = ld_state<ST>(P.st[5], k);
+        const ST dx = ld_state<ST>(P.st[6], k), dy = ld_state<ST>(P.st[7], k),
+                 dz = ld_state<ST>(P.st[8], k);
+        const ST w = ld_state<ST>(P.st[9], k);
+        p.rx = rx; p.ry = ry; p.rz = rz;
+        p.bx = bx; p.by = by; p.bz = bz;
+        p.bfx = (float)bx; p.bfy = (float)by; p.bfz = (float)bz;
+        p.bdx = (float)dx; p.bdy = (float)dy; p.bdz = (float)dz;
+        p.wdt = (float)w * P.dt;
+    } else {  // padding lane: zero amplitude, harmless phase
+        p.rx = p.ry = p.rz = p.bx = p.by = p.bz = 0.0;
+        p.bfx = p.bfy = p.bfz = p.bdx = p.bdy = p.bdz = p.wdt = 0.0f;
+    }
+    return p;
+}
+
+// a3: fold one thread's fp32 partials into the fp64 accumulator (or the deterministic
+// per-chunk workspace).
+template <int S, int LW>
+__device__ __forceinline__ void fold(const AccumParams &P, const float (&acc)[S][4], int dir,
+                                     int jbase)
+{
+    if (dir >= P.n_dir) return;
+    if (P.partial) {
+        double *dst = P.partial + ((size_t)blockIdx.y * P.n_dir + dir) * (size_t)P.w_pad * 4;
+#pragma unroll
+        for (int i = 0; i < S; ++i) {
+            const int j = jbase + i * LW;
+            double2 *q = reinterpret_cast<double2 *>(dst + (size_t)j * 4);
+            q[0] = make_double2((double)acc[i][0], (double)acc[i][1]);
+            q[1] = make_double2((double)acc[i][2], (double)acc[i][3]);
+        }
+    } else {
+        double *dst = P.acc + (size_t)dir * P.w_pad * 4;
+#pragma unroll
+        for (int i = 0; i < S; ++i) {
+            const int j = jbase + i * LW;
+            if (j < P.n_omega) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) atomicAdd(dst + (size_t)j * 4 + c, (double)acc[i][c]);
+            }
+        }
+    }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// a2: general (non-uniform) frequency grid.  Per update: 1 IMAD + 1 LOP/SHF + 3 FP32 for the
+// phase, FMUL + MUFU.SIN + MUFU.COS, 4 FFMA.
+template <typename ST, int LW, int S, int MINB>
+__global__ void __launch_bounds__(kThreads, MINB) rad_accum_general(const AccumParams P)
+{
+    constexpr int DPW = 32 / LW;
+    __shared__ float4 s_rec[kWarpsPerBlock][kBatch * DPW];
+    __shared__ float s_sf[kWarpsPerBlock][kBatch * DPW];
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int wt = blockIdx.x * kWarpsPerBlock + warp;
+    if (wt >= P.n_wtiles) return;  // whole warp leaves; no block barrier is used below
+    const int dg = wt / P.n_ftiles, ft = wt - dg * P.n_ftiles;
+    const int ld = lane / LW, lf = lane - ld * LW;
+    const int jbase = ft * (LW * S) + lf;
+
+    uint32_t F[S];
+    float Ff[S], fl[S], acc[S][4];
+#pragma unroll
+    for (int i = 0; i < S; ++i) {
+        F[i] = __ldg(P.F + jbase + i * LW);
+        Ff[i] = __ldg(P.Ff + jbase + i * LW);
+        fl[i] = __ldg(P.fl + jbase + i * LW);
+        acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.0f;
+    }
+
+    const long long k0 = (long long)blockIdx.y * P.chunk;
+    const long long k1 = min(P.n_particles, k0 + (long long)P.chunk);
+    float4 *rec = s_rec[warp];
+    float *sfs = s_sf[warp];
+
+    for (long long kb = k0; kb < k1; kb += kBatch) {
+        {  // a1: stage
+            const long long k = kb + lane;
+            const Particle p = load_particle<ST>(P, k, k < k1);
+#pragma unroll
+            for (int dd = 0; dd < DPW; ++dd) {
+                const int dir = min(dg * DPW + dd, P.n_dir - 1);
+                float4 r4;
+                float sf;
+                stage_record(p, P.dirs[dir], P.ts32, r4, sf);
+                rec[lane * DPW + dd] = r4;
+                sfs[lane * DPW + dd] = sf;
+            }
+        }
+        __syncwarp();
+#pragma unroll 2
+        for (int kk = 0; kk < kBatch; ++kk) {  // a2: sweep
+            const float4 r4 = rec[kk * DPW + ld];
+            const float sf = sfs[kk * DPW + ld];
+            const uint32_t T = __float_as_uint(r4.x);
+#pragma unroll
+            for (int i = 0; i < S; ++i) {
+                const uint32_t u = F[i] * T;
+                const float v = __uint_as_float(0x3f800000u | (u >> 9));  // 1 + frac, in turns
+                const float q = fmaf(fl[i], sf, Ff[i] * r4.y);
+                const float x = fmaf(v, kTwoPi, q);
+                float sn, cs;
+                __sincosf(x, &sn, &cs);
+                acc[i][0] = fmaf(r4.z, cs, acc[i][0]);
+                acc[i][1] = fmaf(r4.z, sn, acc[i][1]);
+                acc[i][2] = fmaf(r4.w, cs, acc[i][2]);
+                acc[i][3] = fmaf(r4.w, sn, acc[i][3]);
+            }
+        }
+        __syncwarp();
+    }
+    fold<S, LW>(P, acc, dg * DPW + ld, jbase);
+}
+
+// ------------------------------------------------------------------------------------------
+// Launch logic.
+template <typename ST, int LW, int S, int MINB>
+static cudaError_t launch_general(const AccumParams &p, cudaStream_t s)
+{
+    const int n_chunks = (int)((p.n_particles + p.chunk - 1) / p.chunk);
+    dim3 grid((p.n_wtiles + kWarpsPerBlock - 1) / kWarpsPerBlock, n_chunks);
+    rad_accum_general<ST, LW, S, MINB><<<grid, kThreads, 0, s>>>(p);
+    return cudaGetLastError();
+}
+
+template <typename ST>
+static cudaError_t dispatch_general(const Handle &h, const AccumParams &p, cudaStream_t s)
+{
+    switch (h.lw) {
+        case 32: return launch_general<ST, 32, 8, 4>(p, s);
+        case 16: return launch_general<ST, 16, 8, 4>(p, s);
+        case 8: return launch_general<ST, 8, 8, 4>(p, s);
+        default: return launch_general<ST, 4, 8, 4>(p, s);
+    }
+}
+
+cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_f64,
+                              cudaStream_t s, int *n_launches, const char **variant)
+{
+    *variant = "general";
+    *n_launches = 1;
+    return state_f64 ? dispatch_general<double>(h, p, s) : dispatch_general<float>(h, p, s);
+}
+
+}  // namespace rad

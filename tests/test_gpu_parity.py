@@ -1,0 +1,161 @@
+"""GPU parity: CUDA path (through the C ABI) vs the fp64 oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json north_star's (tests/_parity.py)."""
+import numpy as np
+import pytest
+
+from paper_2501_03383_b200 import workloads as wl
+from tests import _parity as P
+
+pytestmark = pytest.mark.gpu
+
+C = 299792458.0
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _need_cuda():
+    import torch
+    from paper_2501_03383_b200 import build
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    build.build()
+
+
+def test_cfg0_tiny_helical_full(oracle_mod):
+    """BASELINE.json configs[0] in full: 256 e-, 128 steps, 8 x 64 bins, fp64 state."""
+    w = wl.make_workload("0")
+    steps = list(w.steps())
+    S, A, variant = P.run_gpu(w, steps, want_amplitude=True)
+    o = P.run_oracle(oracle_mod, w, steps)
+    l2, mr = P.assert_parity(S, o.spectrum(), what="cfg0")
+    Aref = o.amplitude()
+    assert np.abs(A - Aref).max() <= 2e-5 * np.abs(Aref).max()
+    print(f"cfg0 variant={variant} relL2={l2:.2e} maxrel={mr:.2e}")
+
+
+@pytest.mark.parametrize("cfg", ["1", "2", "3a", "3b", "3c", "3d", "4"])
+def test_reduced_particles_all_bins(oracle_mod, cfg):
+    """Every bin / tile path of configs 1-4 on a reduced workload (first 1000 particles --
+    a ragged tail for the 32-particle batches -- x 3 steps, incl. a late step index)."""
+    w = wl.make_workload(cfg)
+    n = 1000 if w.n_dir * w.n_omega <= 65536 else 300
+    steps = [(t if i < 2 else w.n_steps - 1, st) for i, (t, st) in enumerate(w.steps(n_steps=3, n_particles=n))]
+    S, variant = P.run_gpu(w, steps)
+    o = P.run_oracle(oracle_mod, w, steps)
+    l2, mr = P.assert_parity(S, o.spectrum(), what=f"cfg{cfg} reduced")
+    print(f"cfg{cfg} reduced variant={variant} relL2={l2:.2e} maxrel={mr:.2e}")
+
+
+def test_cfg1_many_particles_bin_subset(oracle_mod):
+    """Config 1 particle count (65 536, spans many chunks/blocks) x 4 steps; oracle on a
+    stratified bin subset plus the GPU arg-max bin (bins are independent sums)."""
+    w = wl.make_workload("1")
+    steps = list(w.steps(n_steps=4))
+    S, _ = P.run_gpu(w, steps)
+    bins = P.stratified_bins(w.n_dir, w.n_omega, 4, 8, extra=[int(np.argmax(S))])
+    o = P.run_oracle(oracle_mod, w, steps, bins=bins)
+    Sref = o.spectrum().ravel()[bins]
+    P.assert_parity(S.ravel()[bins], Sref, peak=S.max(), what="cfg1 subset")
+    assert S.ravel()[int(np.argmax(S))] == pytest.approx(o.spectrum().ravel()[int(np.argmax(S))], rel=1e-4)
+
+
+def test_closed_form_pins_on_gpu():
+    """The oracle's closed forms hold for the CUDA path too (Dirichlet kernel incl. complex
+    phase, Doppler shift): a direct GPU-vs-mathematics check, no oracle involved."""
+    dirs = np.array([[1.0, 0, 0], [0, 0, 2.0], [0.3, -0.5, 0.8], [-0.6, 0.64, 0.48]])
+    unit = dirs / np.linalg.norm(dirs, axis=1, keepdims=True)
+    omega = np.array([3.0e14, 1.0e15, 2.7e15, 8.1e15, 3.3e16])
+    dt, T, wgt, t0 = 2.0e-17, 31, 0.8, 3.7e-16
+    r0 = np.array([0.4e-6, 0.9e-6, -0.3e-6]); beta = np.array([0.31, -0.12, 0.22])
+    b = np.array([-1.0e12, 3.0e12, 2.0e12])
+    w = wl.Workload("pin", 1, T, dt, dirs, omega, np.float64, 0, "helix", t0=t0)
+    steps = [(t, [np.array([v]) for v in list(r0 + C * beta * t * dt) + list(beta) + list(b) + [wgt]])
+             for t in range(T)]
+    S, A, _ = P.run_gpu(w, steps, want_amplitude=True)
+    for i, n in enumerate(unit):
+        d = 1.0 - n @ beta
+        vec = (n - beta) * (n @ b) - b * d
+        for j, om in enumerate(omega):
+            x = om * d * dt
+            dk = np.sin(T * x / 2) / np.sin(x / 2)
+            assert S[i, j] == pytest.approx(wgt ** 2 * (vec @ vec) / d ** 4 * dt ** 2 * dk ** 2, rel=2e-5)
+            ph = np.exp(1j * om * (t0 - (n @ r0) / C)) * np.exp(1j * x * (T - 1) / 2.0)
+            a_ref = wgt * dt * vec / d ** 2 * ph * dk
+            assert np.abs(A[i, j] - a_ref).max() <= 2e-5 * np.abs(a_ref).max()
+
+
+def test_zero_for_unaccelerated_motion_and_linearity():
+    w = wl.make_workload("3c")
+    (t, st), = list(w.steps(n_steps=1, n_particles=777))
+    zero = st[:6] + [np.zeros_like(st[6])] * 3 + [st[9]]
+    S, _ = P.run_gpu(w, [(0, zero)])
+    assert np.all(S == 0.0)
+    S1, _ = P.run_gpu(w, [(0, st)])
+    S3, _ = P.run_gpu(w, [(0, st[:9] + [3.0 * st[9]])])
+    m = S1 > 1e-9 * S1.max()
+    assert np.allclose(S3[m], 9.0 * S1[m], rtol=1e-4)
+    # same particles split over two calls with the same step index
+    Ssplit, _ = P.run_gpu(w, [(0, [a[:300] for a in st]), (0, [a[300:] for a in st])])
+    assert P.rel_l2(Ssplit, S1) < 1e-6
+
+
+def test_api_semantics_reset_add_amplitude_host_path_deterministic(oracle_mod):
+    import torch
+    from paper_2501_03383_b200 import binding
+    w = wl.make_workload("3b")
+    steps = list(w.steps(n_steps=2, n_particles=2500))
+    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    # host-buffer entry point (library stages the copies)
+    S_host, _ = P.run_gpu(w, steps, host=True)
+    P.assert_parity(S_host, ref, what="host path")
+    # deterministic flag: parity and bit-reproducibility
+    Sd1, _ = P.run_gpu(w, steps, flags=binding.RAD_FLAG_DETERMINISTIC)
+    Sd2, _ = P.run_gpu(w, steps, flags=binding.RAD_FLAG_DETERMINISTIC)
+    P.assert_parity(Sd1, ref, what="deterministic")
+    assert np.array_equal(Sd1, Sd2)
+    # reset + add_amplitude: two detectors on particle halves, amplitudes summed (multi-GPU path)
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0) as a, \
+            binding.Detector(w.dirs, w.omega, w.dt, scale=1.0) as b:
+        for t, st in steps:
+            a.accumulate_step(t, P.to_device([x[:1200] for x in st]))
+            b.accumulate_step(t, P.to_device([x[1200:] for x in st]))
+        amp_a = torch.empty(w.n_dir, w.n_omega, 3, 2, dtype=torch.float64, device="cuda")
+        amp_b = torch.empty_like(amp_a)
+        a.amplitude(out=amp_a); b.amplitude(out=amp_b)
+        total = amp_a + amp_b
+        a.reset()
+        assert np.all(a.spectrum() == 0.0)
+        a.add_amplitude(total)
+        P.assert_parity(a.spectrum(), ref, what="add_amplitude")
+        out_dev = torch.empty(w.n_dir, w.n_omega, dtype=torch.float64, device="cuda")
+        a.spectrum(out=out_dev)
+        torch.cuda.synchronize()
+        assert np.array_equal(out_dev.cpu().numpy(), a.spectrum())
+        assert a.launch_count > 0
+
+
+def test_edge_cases(oracle_mod):
+    from paper_2501_03383_b200 import binding
+    # single direction, single frequency, single particle; default SI scale
+    w = wl.Workload("edge", 1, 1, 1e-17, np.array([[0.0, 1.0, 0.0]]), np.array([5e15]), np.float32, 0, "khi")
+    st = [np.array([v], dtype=np.float32) for v in (1e-6, 2e-6, 3e-6, 0.1, 0.2, 0.0, 1e12, -2e12, 5e11, 2.0)]
+    S, _ = P.run_gpu(w, [(5, st)], scale=0.0)
+    ref = P.run_oracle(oracle_mod, w, [(5, st)], scale=0.0).spectrum()
+    assert S[0, 0] == pytest.approx(ref[0, 0], rel=1e-5)
+    # empty input is a no-op; ragged sizes 1, 31, 33; awkward grid 5 x 37
+    w2 = wl.Workload("ragged", 33, 1, 1e-17, wl.dirs_fibonacci(5), wl.omega_log(37), np.float32,
+                     wl.BASE_SEED + 9, "khi")
+    (t, full), = list(w2.steps(n_steps=1))
+    with binding.Detector(w2.dirs, w2.omega, w2.dt, scale=1.0) as det:
+        det.accumulate_step(0, P.to_device([a[:0] for a in full]))
+        assert np.all(det.spectrum() == 0.0)
+    for n in (1, 31, 33):
+        sub = [a[:n] for a in full]
+        S, _ = P.run_gpu(w2, [(0, sub)])
+        P.assert_parity(S, P.run_oracle(oracle_mod, w2, [(0, sub)]).spectrum(), what=f"ragged n={n}")
+    # large |tau|: late time and far-away particles (integer phase path wraps exactly)
+    w3 = wl.Workload("far", 64, 1, 1e-17, wl.dirs_fibonacci(8), wl.omega_log(64), np.float64,
+                     wl.BASE_SEED + 10, "khi", t0=1e-10)
+    (t, st3), = list(w3.steps(n_steps=1))
+    st3 = [a.copy() for a in st3]
+    st3[0] += 0.5; st3[2] -= 2.0   # metres away from the origin (fp64 state)
+    S, _ = P.run_gpu(w3, [(12345, st3)])
+    P.assert_parity(S, P.run_oracle(oracle_mod, w3, [(12345, st3)]).spectrum(), what="far/late")
