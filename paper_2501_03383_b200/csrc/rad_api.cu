@@ -80,14 +80,14 @@ void choose_tile(Handle &h)
 int choose_chunk(const Handle &h, long long n)
 {
     const long long gx = (h.n_wtiles + kWarpsPerBlock - 1) / kWarpsPerBlock;
-    const long long want_blocks = 8LL * h.sm_count * 4;
+    const long long want_blocks = 8LL * h.sm_count * kMinBlocks;
     long long n_chunks = (want_blocks + gx - 1) / gx;
     long long chunk = (n + n_chunks - 1) / n_chunks;
     chunk = (chunk + kBatch - 1) / kBatch * kBatch;
     if (chunk < 256) chunk = 256;
     if (chunk > 4096) chunk = 4096;
     // small inputs: prefer filling the SMs over amortising the fold
-    while (chunk > kBatch && gx * ((n + chunk - 1) / chunk) < (long long)h.sm_count * 4) chunk /= 2;
+    while (chunk > kBatch && gx * ((n + chunk - 1) / chunk) < (long long)h.sm_count * kMinBlocks) chunk /= 2;
     chunk = (chunk + kBatch - 1) / kBatch * kBatch;
     return (int)chunk;
 }

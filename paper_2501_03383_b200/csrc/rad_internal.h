@@ -18,6 +18,14 @@ constexpr double kTwo32 = 4294967296.0;        // 2^32
 constexpr int kWarpsPerBlock = 4;              // one warp per SM sub-partition
 constexpr int kThreads = 32 * kWarpsPerBlock;
 constexpr int kBatch = 32;                     // particles staged per warp batch (one per lane)
+#ifndef RAD_STRIP
+#define RAD_STRIP 8
+#endif
+#ifndef RAD_MINB
+#define RAD_MINB 4
+#endif
+constexpr int kStrip = RAD_STRIP;              // frequency bins per thread (register strip)
+constexpr int kMinBlocks = RAD_MINB;           // resident blocks per SM the kernels are bounded for
 
 // Per direction (device table).  k = n * (f_unit 2^32 / c): the dot product k.r is the
 // light-travel delay n.r/c measured in units of 2^-32 "unit turns" (phase).
@@ -66,7 +74,7 @@ cudaError_t launch_reduce_partials(const Handle &h, const double *partial, int n
 struct Handle {
     int device = 0;
     int D = 0, W = 0, w_pad = 0;
-    int lw = 32, strip = 8;          // lanes along frequency, bins per lane
+    int lw = 32, strip = kStrip;          // lanes along frequency, bins per lane
     int n_ftiles = 0, n_wtiles = 0;
     double dt = 0, t0 = 0, scale = 0, f_unit = 0;
     bool state_f64 = false, deterministic = false, uniform = false;

@@ -206,10 +206,10 @@ template <typename ST>
 static cudaError_t dispatch_general(const Handle &h, const AccumParams &p, cudaStream_t s)
 {
     switch (h.lw) {
-        case 32: return launch_general<ST, 32, 8, 4>(p, s);
-        case 16: return launch_general<ST, 16, 8, 4>(p, s);
-        case 8: return launch_general<ST, 8, 8, 4>(p, s);
-        default: return launch_general<ST, 4, 8, 4>(p, s);
+        case 32: return launch_general<ST, 32, kStrip, kMinBlocks>(p, s);
+        case 16: return launch_general<ST, 16, kStrip, kMinBlocks>(p, s);
+        case 8: return launch_general<ST, 8, kStrip, kMinBlocks>(p, s);
+        default: return launch_general<ST, 4, kStrip, kMinBlocks>(p, s);
     }
 }
 
