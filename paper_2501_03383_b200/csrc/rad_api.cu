@@ -127,7 +127,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.dt = (float)h.dt;
     p.acc = h.acc_d;
     p.partial = nullptr;
-    p.f0_unit = h.f0_unit; p.df_unit = h.df_unit;
+    p.rot_G = h.rot_G; p.rot_Gf = h.rot_Gf; p.rot_gl = h.rot_gl;
     const int n_chunks = (int)((n + p.chunk - 1) / p.chunk);
     if (h.deterministic) {
         const size_t need = (size_t)n_chunks * h.D * h.w_pad * 4 * sizeof(double);
@@ -223,6 +223,20 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         r.pad[0] = r.pad[1] = r.pad[2] = 0.0f;
     }
     choose_tile(h);
+    // uniform grid?  w_j = w_0 + j dw to fp64 rounding -> rotation-recurrence kernel (a2')
+    h.uniform = false;
+    if (h.W >= 2 * h.strip && !(cfg->flags & RAD_FLAG_FORCE_GENERAL)) {
+        const double dw = (h.omega_h.back() - h.omega_h.front()) / (h.W - 1);
+        bool uni = true;
+        for (int j = 0; j < h.W && uni; ++j)
+            uni = std::fabs(h.omega_h[j] - (h.omega_h[0] + j * dw)) <= 4e-16 * h.omega_h.back() * (1 + j);
+        if (uni) {
+            const double step = dw / (2.0 * kPi) / h.f_unit * h.lw;  // rotator frequency, f_unit units
+            const double G = std::nearbyint(step);
+            h.uniform = true;
+            h.rot_G = (uint32_t)G; h.rot_Gf = (float)G; h.rot_gl = (float)(step - G);
+        }
+    }
     std::vector<uint32_t> F(h.w_pad, 0u);
     std::vector<float> Ff(h.w_pad, 0.0f), fl(h.w_pad, 0.0f);
     for (int j = 0; j < h.W; ++j) {

@@ -56,8 +56,9 @@ struct AccumParams {
     float dt;              // quadrature weight
     double *acc;           // [D][w_pad][4]: A1.re A1.im A2.re A2.im (transverse components)
     double *partial;       // deterministic mode: [n_chunks][D][w_pad][4], else NULL
-    // uniform-grid variant only
-    double f0_unit, df_unit;  // f_0 / f_unit and (f_1 - f_0)/f_unit
+    // uniform-grid variant only: LW*(f_1 - f_0)/f_unit = rot_G + rot_gl (integer + fraction)
+    uint32_t rot_G;
+    float rot_Gf, rot_gl;
 };
 
 struct Handle;
@@ -78,7 +79,8 @@ struct Handle {
     int n_ftiles = 0, n_wtiles = 0;
     double dt = 0, t0 = 0, scale = 0, f_unit = 0;
     bool state_f64 = false, deterministic = false, uniform = false;
-    double f0_unit = 0, df_unit = 0;
+    uint32_t rot_G = 0;              // uniform grid: rotator frequency LW*df in f_unit units
+    float rot_Gf = 0, rot_gl = 0;
     int sm_count = 148;
     std::vector<double> dirs_h;      // normalised [D][3]
     std::vector<double> omega_h;

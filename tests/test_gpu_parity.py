@@ -29,6 +29,25 @@ def test_cfg0_tiny_helical_full(oracle_mod):
     Aref = o.amplitude()
     assert np.abs(A - Aref).max() <= 2e-5 * np.abs(Aref).max()
     print(f"cfg0 variant={variant} relL2={l2:.2e} maxrel={mr:.2e}")
+    assert variant == "uniform"      # linear grid -> rotation-recurrence kernel (a2')
+    # the general kernel must give the same answer on the same grid
+    from paper_2501_03383_b200 import binding
+    Sg, vg = P.run_gpu(w, steps, flags=binding.RAD_FLAG_FORCE_GENERAL)
+    assert vg == "general"
+    P.assert_parity(Sg, o.spectrum(), what="cfg0 general kernel")
+
+
+@pytest.mark.parametrize("D,W,dtype", [(37, 300, np.float32), (5, 1024, np.float32), (64, 64, np.float64)])
+def test_uniform_grid_recurrence_kernel(oracle_mod, D, W, dtype):
+    """a2': linear frequency grids (any tile shape, ragged W) use the recurrence kernel and
+    match the oracle; high frequencies (up to 2e17 rad/s) stress the rotator phase."""
+    w = wl.Workload("lin", 1500, 3, 1e-17, wl.dirs_fibonacci(D), np.linspace(2e14, 2e17, W), dtype,
+                    wl.BASE_SEED + 20, "khi")
+    steps = [(t * 400, st) for t, st in w.steps(n_steps=3)]
+    S, variant = P.run_gpu(w, steps)
+    assert variant == "uniform"
+    l2, mr = P.assert_parity(S, P.run_oracle(oracle_mod, w, steps).spectrum(), what=f"uniform {D}x{W}")
+    print(f"uniform {D}x{W} relL2={l2:.2e} maxrel={mr:.2e}")
 
 
 @pytest.mark.parametrize("cfg", ["1", "2", "3a", "3b", "3c", "3d", "4"])
@@ -159,3 +178,48 @@ def test_edge_cases(oracle_mod):
     st3[0] += 0.5; st3[2] -= 2.0   # metres away from the origin (fp64 state)
     S, _ = P.run_gpu(w3, [(12345, st3)])
     P.assert_parity(S, P.run_oracle(oracle_mod, w3, [(12345, st3)]).spectrum(), what="far/late")
+
+
+# ------------------------------------------------------------------ full sizes, sampled bins
+def _full_size_sampled(oracle_mod, cfg, n_steps, n_dir=3, n_om=6):
+    """BASELINE.json's full particle count in the launch configuration bench.py times
+    (same handle set-up, same per-step call); the oracle computes a stratified sample of
+    bins plus the GPU arg-max bin one by one (bins are independent sums)."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    w = wl.make_workload(cfg)
+    bins = P.stratified_bins(w.n_dir, w.n_omega, n_dir, n_om)
+    o = oracle_mod.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=bins)
+    first = None
+    with binding.Detector(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, state_dtype=w.state_dtype) as det:
+        for t, st in w.steps(n_steps=n_steps):
+            det.accumulate_step(t, P.to_device(st))
+            o.accumulate_step(t, *st)
+            first = first or st
+        torch.cuda.synchronize()
+        S = det.spectrum()
+    jmax = int(np.argmax(S))
+    Sref = o.spectrum().ravel()[bins]
+    l2, mr = P.assert_parity(S.ravel()[bins], Sref, peak=S.max(), what=f"cfg{cfg} full-size sample")
+    if n_steps == 1:  # the arg-max bin itself, verified separately (cheap for one step)
+        om = oracle_mod.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=np.array([jmax]))
+        om.accumulate_step(0, *first)
+        assert S.ravel()[jmax] == pytest.approx(om.spectrum().ravel()[jmax], rel=1e-4)
+    print(f"cfg{cfg} full-size: {len(bins)} bins relL2={l2:.2e} maxrel={mr:.2e}")
+
+
+def test_cfg1_full_workload_all_1000_steps(oracle_mod):
+    _full_size_sampled(oracle_mod, "1", 1000, n_dir=3, n_om=5)
+
+
+@pytest.mark.parametrize("cfg", ["3a", "3b", "3c", "3d"])
+def test_cfg3_full_particles(oracle_mod, cfg):
+    _full_size_sampled(oracle_mod, cfg, 4, n_dir=3, n_om=6)
+
+
+def test_cfg2_full_particles(oracle_mod):
+    _full_size_sampled(oracle_mod, "2", 2, n_dir=3, n_om=6)
+
+
+def test_cfg4_full_particles(oracle_mod):
+    _full_size_sampled(oracle_mod, "4", 1, n_dir=3, n_om=6)
