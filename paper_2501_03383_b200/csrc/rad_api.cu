@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 
 #include "rad_internal.h"
@@ -120,6 +121,10 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     for (int i = 0; i < 10; ++i) p.st[i] = st[i];
     p.n_particles = n;
     p.chunk = choose_chunk(h, n);
+    if (const char *e = getenv("RAD_CHUNK")) {  // tuning/debug override (particles per block)
+        const int c = atoi(e);
+        if (c >= kBatch) p.chunk = c / kBatch * kBatch;
+    }
     p.n_dir = h.D; p.n_omega = h.W; p.w_pad = h.w_pad;
     p.n_ftiles = h.n_ftiles; p.n_wtiles = h.n_wtiles;
     p.dirs = h.dirs_d; p.F = h.F_d; p.Ff = h.Ff_d; p.fl = h.fl_d;
