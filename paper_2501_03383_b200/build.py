@@ -14,7 +14,7 @@ PKG = Path(__file__).resolve().parent
 ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "librad.so"
-SOURCES = ["rad_api.cu", "rad_kernels.cu", "rad_finalize.cu"]
+SOURCES = ["rad_api.cu", "rad_kernels.cu", "rad_stream.cu", "rad_finalize.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--use_fast_math", "-Xcompiler", "-fPIC,-fvisibility=hidden,-O2", "-shared",
               "-cudart", "static"]

@@ -1,6 +1,7 @@
 // rad_api.cu -- host runtime and the extern "C" boundary declared in include/rad.h.
 // a0 (set-up at rad_create): normalise n, transverse basis, frequency
 // tables (integer + fractional part in units of f_unit), tile-shape choice, zeroed A.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -133,7 +134,15 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.acc = h.acc_d;
     p.partial = nullptr;
     p.rot_G = h.rot_G; p.rot_Gf = h.rot_Gf; p.rot_gl = h.rot_gl;
-    const int n_chunks = (int)((n + p.chunk - 1) / p.chunk);
+    int n_chunks = (int)((n + p.chunk - 1) / p.chunk);
+    int stream_grid = 0;
+    if (h.stream_nb) {  // few bins: persistent particle-streaming kernel, one partial slot per block
+        const int tile = stream_tile_particles(h.state_f64);
+        const long long n_tiles = (n + tile - 1) / tile;
+        stream_grid = (int)std::min<long long>(n_tiles, (long long)stream_blocks_per_sm(h.stream_nb) * h.sm_count);
+        for (int j = 0; j < 16; ++j) { p.sF[j] = h.sF[j]; p.sFf[j] = h.sFf[j]; p.sfl[j] = h.sfl[j]; }
+        n_chunks = stream_grid;
+    }
     if (h.deterministic) {
         const size_t need = (size_t)n_chunks * h.D * h.w_pad * 4 * sizeof(double);
         if (need > h.partial_bytes) {
@@ -147,10 +156,17 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
             h.partial_bytes = need;
         }
         p.partial = h.partial_d;
+        if (h.stream_nb) RAD_CUDA(&h, cudaMemsetAsync(h.partial_d, 0, need, s));  // padded bins stay 0
     }
-    int nl = 0;
-    RAD_CUDA(&h, launch_accumulate(h, p, h.state_f64, s, &nl, &h.variant));
-    h.launches += nl;
+    if (h.stream_nb) {
+        RAD_CUDA(&h, launch_accumulate_stream(h, p, h.state_f64, stream_grid, s));
+        h.variant = "stream";
+        h.launches += 1;
+    } else {
+        int nl = 0;
+        RAD_CUDA(&h, launch_accumulate(h, p, h.state_f64, s, &nl, &h.variant));
+        h.launches += nl;
+    }
     if (h.deterministic) {
         RAD_CUDA(&h, launch_reduce_partials(h, h.partial_d, n_chunks, s));
         h.launches += 1;
@@ -228,6 +244,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         r.pad[0] = r.pad[1] = r.pad[2] = 0.0f;
     }
     choose_tile(h);
+    h.stream_nb = stream_shape(h.D, h.W, &h.stream_nd);
     // uniform grid?  w_j = w_0 + j dw to fp64 rounding -> rotation-recurrence kernel (a2')
     h.uniform = false;
     if (h.W >= 2 * h.strip && !(cfg->flags & RAD_FLAG_FORCE_GENERAL)) {
@@ -250,6 +267,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         F[j] = (uint32_t)Fi;
         Ff[j] = (float)Fi;
         fl[j] = (float)(fu - Fi);
+        if (j < 16) { h.sF[j] = F[j]; h.sFf[j] = Ff[j]; h.sfl[j] = fl[j]; }
     }
 
     cudaError_t e = cudaSetDevice(h.device);

@@ -56,6 +56,9 @@ struct AccumParams {
     float dt;              // quadrature weight
     double *acc;           // [D][w_pad][4]: A1.re A1.im A2.re A2.im (transverse components)
     double *partial;       // deterministic mode: [n_chunks][D][w_pad][4], else NULL
+    // streaming variant only: per-frequency constants in the parameter constant bank
+    uint32_t sF[16];
+    float sFf[16], sfl[16];
     // uniform-grid variant only: LW*(f_1 - f_0)/f_unit = rot_G + rot_gl (integer + fraction)
     uint32_t rot_G;
     float rot_Gf, rot_gl;
@@ -66,6 +69,11 @@ struct Handle;
 // kernels/launchers (rad_kernels.cu, rad_finalize.cu)
 cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_f64,
                               cudaStream_t s, int *n_launches, const char **variant);
+cudaError_t launch_accumulate_stream(const Handle &h, const AccumParams &p, bool state_f64, int grid,
+                                     cudaStream_t s);
+int stream_tile_particles(bool state_f64);
+int stream_blocks_per_sm(int nb);
+int stream_shape(int D, int W, int *nd);
 cudaError_t launch_spectrum(const Handle &h, double *out_dev, cudaStream_t s);
 cudaError_t launch_amplitude(const Handle &h, double *out_dev, cudaStream_t s);
 cudaError_t launch_add_amplitude(const Handle &h, const double *amp_dev, cudaStream_t s);
@@ -77,6 +85,8 @@ struct Handle {
     int D = 0, W = 0, w_pad = 0;
     int lw = 32, strip = kStrip;          // lanes along frequency, bins per lane
     int n_ftiles = 0, n_wtiles = 0;
+    int stream_nd = 1;
+    int stream_nb = 0;               // > 0: D*W <= 16 -> particle-streaming kernel with 8 or 16 bins/thread
     double dt = 0, t0 = 0, scale = 0, f_unit = 0;
     bool state_f64 = false, deterministic = false, uniform = false;
     uint32_t rot_G = 0;              // uniform grid: rotator frequency LW*df in f_unit units
@@ -84,6 +94,8 @@ struct Handle {
     int sm_count = 148;
     std::vector<double> dirs_h;      // normalised [D][3]
     std::vector<double> omega_h;
+    uint32_t sF[16] = {0};           // streaming shapes: first 16 frequency constants (host copy)
+    float sFf[16] = {0}, sfl[16] = {0};
     DirRec *dirs_d = nullptr;
     double *basis_d = nullptr;       // [D][6] fp64 e1, e2 (amplitude export/import)
     uint32_t *F_d = nullptr;

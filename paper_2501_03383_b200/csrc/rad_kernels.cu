@@ -16,93 +16,14 @@
 // for any |tau|); the other two are O(1/2 turn) and O(tau f_unit) and are added in fp32.
 #include <math_constants.h>
 
+#include "rad_device.cuh"
 #include "rad_internal.h"
 
 namespace rad {
 
 namespace {
 
-constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: fp64 round-to-integer constant
-constexpr float kTwoPi = 6.283185307179586f;
-constexpr float kUnitToRad = 1.4629180792671596e-09f;  // 2 pi / 2^32
-
-template <typename ST>
-__device__ __forceinline__ ST ld_state(const void *p, long long k)
-{
-    return __ldg(reinterpret_cast<const ST *>(p) + k);
-}
-
-// a1: stage one particle for one direction -> record {T, ql, a1, a2} + sf.
-struct Particle {
-    double rx, ry, rz, bx, by, bz;  // fp64 for the phase and the Doppler factor
-    float bfx, bfy, bfz, bdx, bdy, bdz, wdt;
-};
-
-__device__ __forceinline__ void stage_record(const Particle &p, const DirRec &dr, double ts32,
-                                             float4 &rec, float &sf, uint32_t *T_out = nullptr)
-{
-    // phase: s32 = (t - n.r/c) f_unit 2^32 in fp64, split into integer (mod 2^32) + residual
-    const double s32 = ts32 - fma(dr.kx, p.rx, fma(dr.ky, p.ry, dr.kz * p.rz));
-    const double m = s32 + kMagic;
-    const uint32_t T = (uint32_t)__double2loint(m);
-    const double res = s32 - (m - kMagic);
-    // Doppler factor d = 1 - n.beta in fp64 (no cancellation error for beta -> 1)
-    const double d64 = 1.0 - fma(dr.nx, p.bx, fma(dr.ny, p.by, dr.nz * p.bz));
-    const float d = (float)d64;
-    // amplitude: n x ((n-beta) x bd) = (n-beta)(n.bd) - bd (1-n.beta); it is _|_ n, so its
-    // components on the transverse basis are a_i = -(e_i.beta)(n.bd) - (e_i.bd) d
-    const float g = fmaf(dr.nfx, p.bdx, fmaf(dr.nfy, p.bdy, dr.nfz * p.bdz));
-    const float e1b = fmaf(dr.e1x, p.bfx, fmaf(dr.e1y, p.bfy, dr.e1z * p.bfz));
-    const float e2b = fmaf(dr.e2x, p.bfx, fmaf(dr.e2y, p.bfy, dr.e2z * p.bfz));
-    const float e1d = fmaf(dr.e1x, p.bdx, fmaf(dr.e1y, p.bdy, dr.e1z * p.bdz));
-    const float e2d = fmaf(dr.e2x, p.bdx, fmaf(dr.e2y, p.bdy, dr.e2z * p.bdz));
-    const float inv = 1.0f / d;
-    const float pre = -p.wdt * inv * inv;  // -w dt / d^2
-    rec.x = __uint_as_float(T);
-    rec.y = (float)res * kUnitToRad;
-    rec.z = pre * fmaf(e1b, g, e1d * d);
-    rec.w = pre * fmaf(e2b, g, e2d * d);
-    sf = (float)s32 * kUnitToRad;
-    if (T_out) *T_out = T;
-}
-
-// exp(i 2 pi f tau) for one frequency f = (F + phi) f_unit from a staged record (integer phase)
-__device__ __forceinline__ void phase_sincos(uint32_t F, float Ff, float fl, uint32_t T, float ql,
-                                             float sf, float &sn, float &cs)
-{
-    const uint32_t u = F * T;
-#ifdef RAD_CENTER
-    const float v = __uint_as_float(0x3f800000u | (u >> 9)) - 1.5f;  // frac - 1/2 in turns (exact)
-#else
-    const float v = __uint_as_float(0x3f800000u | (u >> 9));  // 1 + frac, in turns
-#endif
-    const float q = fmaf(fl, sf, Ff * ql);
-    __sincosf(fmaf(v, kTwoPi, q), &sn, &cs);
-}
-
-template <typename ST>
-__device__ __forceinline__ Particle load_particle(const AccumParams &P, long long k, bool valid)
-{
-    Particle p;
-    if (valid) {
-        const ST rx = ld_state<ST>(P.st[0], k), ry = ld_state<ST>(P.st[1], k),
-                 rz = ld_state<ST>(P.st[2], k);
-        const ST bx = ld_state<ST>(P.st[3], k), by = ld_state<ST>(P.st[4], k),
-                 bz = ld_state<ST>(P.st[5], k);
-        const ST dx = ld_state<ST>(P.st[6], k), dy = ld_state<ST>(P.st[7], k),
-                 dz = ld_state<ST>(P.st[8], k);
-        const ST w = ld_state<ST>(P.st[9], k);
-        p.rx = rx; p.ry = ry; p.rz = rz;
-        p.bx = bx; p.by = by; p.bz = bz;
-        p.bfx = (float)bx; p.bfy = (float)by; p.bfz = (float)bz;
-        p.bdx = (float)dx; p.bdy = (float)dy; p.bdz = (float)dz;
-        p.wdt = (float)w * P.dt;
-    } else {  // padding lane: zero amplitude, harmless phase
-        p.rx = p.ry = p.rz = p.bx = p.by = p.bz = 0.0;
-        p.bfx = p.bfy = p.bfz = p.bdx = p.bdy = p.bdz = p.wdt = 0.0f;
-    }
-    return p;
-}
+using namespace dev;
 
 // a3: fold one thread's fp32 partials into the fp64 accumulator (or the deterministic
 // per-chunk workspace).

@@ -223,3 +223,49 @@ def test_cfg2_full_particles(oracle_mod):
 
 def test_cfg4_full_particles(oracle_mod):
     _full_size_sampled(oracle_mod, "4", 1, n_dir=3, n_om=6)
+
+
+# --------------------------------------------------------------- particle-streaming kernel
+@pytest.mark.parametrize("D,W,dtype,n", [(1, 8, np.float32, 5000), (1, 8, np.float32, 4096), (2, 8, np.float32, 3001),
+                                         (2, 3, np.float32, 1025), (1, 1, np.float32, 100), (1, 13, np.float32, 1537),
+                                         (1, 8, np.float64, 2077), (2, 7, np.float64, 513)])
+def test_stream_kernel_few_bins(oracle_mod, D, W, dtype, n):
+    """<= 2 directions x <= 8 frequencies (or 1 x <= 16) -> particle-owner streaming kernel (bulk-copy staged tiles, ragged tail via
+    plain loads, warp-shuffle reduction); parity incl. the deterministic mode."""
+    from paper_2501_03383_b200 import binding
+    w = wl.Workload("stream", n, 2, 1e-17, wl.dirs_fibonacci(max(D, 2))[:D], wl.omega_log(max(W, 2))[:W], dtype,
+                    wl.BASE_SEED + 30, "khi")
+    steps = [(t * 700, st) for t, st in w.steps(n_steps=2)]
+    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    S, variant = P.run_gpu(w, steps)
+    assert variant == "stream"
+    P.assert_parity(S, ref, what=f"stream {D}x{W}")
+    Sd, _ = P.run_gpu(w, steps, flags=binding.RAD_FLAG_DETERMINISTIC)
+    Sd2, _ = P.run_gpu(w, steps, flags=binding.RAD_FLAG_DETERMINISTIC)
+    P.assert_parity(Sd, ref, what=f"stream deterministic {D}x{W}")
+    assert np.array_equal(Sd, Sd2)
+
+
+def test_stream_kernel_unaligned_arrays_use_plain_loads(oracle_mod):
+    """State arrays that are not 16-byte aligned (views at an odd offset) must not take the
+    bulk-copy path; result still matches."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    w = wl.Workload("stream_unaligned", 4099, 1, 1e-17, wl.dirs_fibonacci(2)[:1], wl.omega_log(8), np.float32,
+                    wl.BASE_SEED + 31, "khi")
+    (t, st), = list(w.steps(n_steps=1))
+    ref = P.run_oracle(oracle_mod, w, [(3, st)]).spectrum()
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0) as det:
+        dev = []
+        for a in st:
+            buf = torch.empty(a.shape[0] + 1, dtype=torch.float32, device="cuda")
+            buf[1:] = torch.from_numpy(a).cuda()
+            dev.append(buf[1:])                      # 4-byte offset: not 16-B aligned
+        assert dev[0].data_ptr() % 16 != 0
+        det.accumulate_step(3, dev)
+        S = det.spectrum()
+    P.assert_parity(S, ref, what="stream unaligned")
+
+
+def test_cfg4b_full_particles(oracle_mod):
+    _full_size_sampled(oracle_mod, "4b", 1, n_dir=1, n_om=8)
