@@ -11,6 +11,23 @@ constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: fp64 round-to-inte
 constexpr float kTwoPi = 6.283185307179586f;
 constexpr float kUnitToRad = 1.4629180792671596e-09f;  // 2 pi / 2^32
 
+// state element -> fp64.  fp32 -> fp64 by integer ops (exponent re-bias) instead of F2F.F64.F32:
+// the conversion unit shares the XU pipe with MUFU.SIN/COS, the bound of the whole path, while
+// the integer pipe idles.  Exact for normal numbers; 0 maps to 2^-127 (5.9e-39, harmless: the
+// value only enters sums with terms >= 1e-30 larger); denormals/Inf/NaN are not meaningful
+// particle state.
+__device__ __forceinline__ double to_f64(double x) { return x; }
+__device__ __forceinline__ double to_f64(float x)
+{
+#ifdef RAD_F2D_XU
+    return (double)x;
+#else
+    const uint32_t u = __float_as_uint(x);
+    const uint32_t hi = (u & 0x80000000u) | (((u & 0x7fffffffu) >> 3) + 0x38000000u);
+    return __hiloint2double((int)hi, (int)(u << 29));
+#endif
+}
+
 template <typename ST>
 __device__ __forceinline__ ST ld_state(const void *p, long long k)
 {
@@ -77,8 +94,8 @@ __device__ __forceinline__ Particle load_particle(const AccumParams &P, long lon
         const ST dx = ld_state<ST>(P.st[6], k), dy = ld_state<ST>(P.st[7], k),
                  dz = ld_state<ST>(P.st[8], k);
         const ST w = ld_state<ST>(P.st[9], k);
-        p.rx = rx; p.ry = ry; p.rz = rz;
-        p.bx = bx; p.by = by; p.bz = bz;
+        p.rx = to_f64(rx); p.ry = to_f64(ry); p.rz = to_f64(rz);
+        p.bx = to_f64(bx); p.by = to_f64(by); p.bz = to_f64(bz);
         p.bfx = (float)bx; p.bfy = (float)by; p.bfz = (float)bz;
         p.bdx = (float)dx; p.bdy = (float)dy; p.bdz = (float)dz;
         p.wdt = (float)w * P.dt;

@@ -23,9 +23,22 @@ namespace {
 
 using namespace dev;
 
+#ifndef RAD_S_STAGES
+#define RAD_S_STAGES 2
+#endif
+#ifndef RAD_S_TILEBYTES
+#define RAD_S_TILEBYTES 4096
+#endif
+#ifndef RAD_S_UNROLL
+#define RAD_S_UNROLL 4
+#endif
+#ifndef RAD_S_MINB
+#define RAD_S_MINB 2
+#endif
 constexpr int kSThreads = 256;
-constexpr int kSStages = 3;
-constexpr int kSTileBytes = 2048;  // per array per stage -> 512 fp32 / 256 fp64 particles
+constexpr int kSStages = RAD_S_STAGES;
+constexpr int kSUnroll = RAD_S_UNROLL;
+constexpr int kSTileBytes = RAD_S_TILEBYTES;  // per array per stage -> 1024 fp32 / 512 fp64 particles
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -68,8 +81,8 @@ __device__ __forceinline__ Particle make_particle(ST rx, ST ry, ST rz, ST bx, ST
                                                   ST dy, ST dz, ST w, float dt)
 {
     Particle p;
-    p.rx = rx; p.ry = ry; p.rz = rz;
-    p.bx = bx; p.by = by; p.bz = bz;
+    p.rx = to_f64(rx); p.ry = to_f64(ry); p.rz = to_f64(rz);
+    p.bx = to_f64(bx); p.by = to_f64(by); p.bz = to_f64(bz);
     p.bfx = (float)bx; p.bfy = (float)by; p.bfz = (float)bz;
     p.bdx = (float)dx; p.bdy = (float)dy; p.bdz = (float)dz;
     p.wdt = (float)w * dt;
@@ -80,7 +93,7 @@ __device__ __forceinline__ Particle make_particle(ST rx, ST ry, ST rz, ST bx, ST
 // zero-frequency bins that are discarded).  Per-bin frequency constants come straight from the
 // kernel-parameter constant bank (P.sF/sFf/sfl), not from registers.
 template <typename ST, int NB, int ND>
-__global__ void __launch_bounds__(kSThreads, NB <= 8 ? 3 : 1) rad_accum_stream(const AccumParams P, const int use_bulk)
+__global__ void __launch_bounds__(kSThreads, NB <= 8 ? RAD_S_MINB : 1) rad_accum_stream(const AccumParams P, const int use_bulk)
 {
     constexpr int TILE = kSTileBytes / (int)sizeof(ST);  // particles per tile
     constexpr int PPT = TILE / kSThreads;                 // particles per thread per tile
@@ -136,7 +149,7 @@ __global__ void __launch_bounds__(kSThreads, NB <= 8 ? 3 : 1) rad_accum_stream(c
             phase_bits ^= 1u << stage;
         }
         const ST *sm = reinterpret_cast<const ST *>(s_raw + (size_t)stage * 10 * kSTileBytes);
-#pragma unroll 1
+#pragma unroll kSUnroll
         for (int pp = 0; pp < PPT; ++pp) {
             const int kl = tid + pp * kSThreads;
             const long long k = t * TILE + kl;
@@ -225,7 +238,7 @@ cudaError_t dispatch_stream(const Handle &h, const AccumParams &p, int grid, cud
 }  // namespace
 
 int stream_tile_particles(bool state_f64) { return kSTileBytes / (state_f64 ? 8 : 4); }
-int stream_blocks_per_sm(int nb) { return nb <= 8 ? 3 : 1; }
+int stream_blocks_per_sm(int nb) { return nb <= 8 ? RAD_S_MINB : 1; }
 
 // Shapes served: ND in {1, 2} directions x WB = NB/ND frequencies, NB in {8, 16}.
 // Returns NB (and *nd), or 0 if this detector shape is not a streaming shape.
