@@ -255,24 +255,34 @@ def run_ours(args):
     achieved = updates_per_step / (kernel_ms * 1e-3) / 1e9
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
-    peak = n_sm * MUFU_LANES_PER_SM / MUFU_PER_UPDATE * sm_max * 1e6 / 1e9
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    hbm_achieved = bytes_per_step / (kernel_ms * 1e-3) / 1e9
     traffic = None
     try:
         traffic = json.loads((ROOT / "profiles" / "traffic.json").read_text()).get(w.name, {}).get("bytes")
     except Exception:
         pass
-    roofline = {
-        "bound": "alu", "pipe": "MUFU (sin+cos per update)", "achieved": achieved, "peak": peak,
-        "unit": UNIT, "frac": achieved / peak, "traffic": traffic,
-        "algorithmic_bytes": int(bytes_per_step),
-        "kernel": f"rad_accum_{det.kernel_variant}", "kernel_ms": kernel_ms,
-        "peak_how": f"{n_sm} SMs x {MUFU_LANES_PER_SM} MUFU/clk/SM / {MUFU_PER_UPDATE} MUFU per update x "
-                    f"{sm_max:.0f} MHz (max SM clock, {peaks_src}); DESIGN.md 'Roofline'",
-        "hbm_gbs_achieved": bytes_per_step / (kernel_ms * 1e-3) / 1e9,
-        "hbm_gbs_peak": float(peaks.get("hbm_gbs", 6650.0)),
-    }
+    variant = det.kernel_variant
+    if variant == "stream":      # few bins per particle: the 40 B/particle stream from HBM binds
+        roofline = {"bound": "hbm", "achieved": hbm_achieved, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": hbm_achieved / hbm_peak, "traffic": traffic,
+                    "peak_how": f"MEASURED_PEAKS.json hbm_gbs ({peaks_src})"}
+    else:
+        if variant == "uniform":  # rotation recurrence: 4 FP32 rotate + 4 FMA accumulate per update
+            per_clk_sm, pipe = 128.0 / 8.0, "FP32 (8 FMA-pipe instr per update)"
+        else:                     # general grid: sin + cos per update on the 16-lane MUFU
+            per_clk_sm, pipe = MUFU_LANES_PER_SM / MUFU_PER_UPDATE, "MUFU (sin+cos per update)"
+        peak = n_sm * per_clk_sm * sm_max * 1e6 / 1e9
+        roofline = {"bound": "alu", "pipe": pipe, "achieved": achieved, "peak": peak, "unit": UNIT,
+                    "frac": achieved / peak, "traffic": traffic,
+                    "peak_how": f"{n_sm} SMs x {per_clk_sm:g} updates/clk/SM x {sm_max:.0f} MHz (max SM clock, "
+                                f"{peaks_src}); DESIGN.md section 5"}
+    roofline.update({"kernel": f"rad_accum_{variant}", "kernel_ms": kernel_ms,
+                     "algorithmic_bytes": int(bytes_per_step), "updates_per_launch": int(updates_per_step),
+                     "gupdates_per_s": achieved, "hbm_gbs_achieved": hbm_achieved, "hbm_gbs_peak": hbm_peak})
     if clocks.get("sm_mhz"):
-        roofline["frac_at_sampled_clock"] = achieved / (peak * clocks["sm_mhz"] / sm_max)
+        if roofline["bound"] == "alu":
+            roofline["frac_at_sampled_clock"] = roofline["frac"] * sm_max / clocks["sm_mhz"]
 
     # end to end through the public API with HOST buffers: H2D of the step's state and D2H of
     # the step's spectrum inside the timed region, every step
