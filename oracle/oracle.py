@@ -44,6 +44,13 @@ def _load():
              ctypes.c_double, ctypes.c_double, ctypes.c_longlong, ctypes.c_longlong, ctypes.c_int]
             + [ctypes.c_void_p] * 10
             + [ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p])
+        lib.oracle_accumulate_step_regions.restype = ctypes.c_int
+        lib.oracle_accumulate_step_regions.argtypes = (
+            [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p,
+             ctypes.c_double, ctypes.c_double, ctypes.c_longlong, ctypes.c_longlong,
+             ctypes.c_void_p, ctypes.c_int]
+            + [ctypes.c_void_p] * 10
+            + [ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p])
         lib.oracle_spectrum.restype = ctypes.c_int
         lib.oracle_spectrum.argtypes = [ctypes.c_longlong, ctypes.c_void_p, ctypes.c_double,
                                         ctypes.c_void_p]
@@ -102,6 +109,66 @@ class Oracle:
     def spectrum(self):
         S = np.empty((self.D, self.W), dtype=np.float64)
         rc = _load().oracle_spectrum(self.D * self.W, self.A.ctypes.data, self.scale, S.ctypes.data)
+        if rc != 0:
+            raise ValueError("oracle_spectrum: bad argument")
+        return S
+
+
+class RegionOracle:
+    """Per-region (sub-volume) detectors: A[r] is the oracle sum over the particles of region r
+    only.  Particles are sorted by region; ``offsets`` [R+1] (non-decreasing) are passed with
+    every step.  Same (optional) bin subset in every region."""
+
+    def __init__(self, n_regions, dirs, omega, dt, t0=0.0, scale=0.0, bins=None):
+        self.dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
+        self.omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
+        self.dt, self.t0, self.scale = float(dt), float(t0), float(scale)
+        self.R, self.D, self.W = int(n_regions), self.dirs.shape[0], self.omega.shape[0]
+        self.bins = None if bins is None else np.ascontiguousarray(bins, dtype=np.int64)
+        self.A = np.zeros((self.R, self.D, self.W, 3, 2), dtype=np.float64)
+
+    def reset(self):
+        self.A[...] = 0.0
+
+    def accumulate_step(self, step_index, offsets, rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w):
+        offsets = np.ascontiguousarray(offsets, dtype=np.int64)
+        if offsets.shape != (self.R + 1,):
+            raise ValueError("offsets must have n_regions + 1 entries")
+        arrs = [rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w]
+        dt0 = np.asarray(arrs[0]).dtype
+        if dt0 not in (np.dtype(np.float32), np.dtype(np.float64)):
+            raise TypeError("state must be float32 or float64")
+        arrs = [np.ascontiguousarray(a, dtype=dt0) for a in arrs]
+        n = arrs[0].shape[0]
+        if any(a.shape != (n,) for a in arrs) or offsets[-1] > n:
+            raise ValueError("state arrays must be 1-D, of equal length >= offsets[-1]")
+        nb = 0 if self.bins is None else self.bins.shape[0]
+        bp = None if self.bins is None else self.bins.ctypes.data
+        rc = _load().oracle_accumulate_step_regions(
+            self.D, self.dirs.ctypes.data, self.W, self.omega.ctypes.data, self.dt, self.t0,
+            int(step_index), self.R, offsets.ctypes.data, int(dt0 == np.dtype(np.float32)),
+            *[a.ctypes.data for a in arrs], nb, bp, self.A.ctypes.data)
+        if rc != 0:
+            raise ValueError("oracle_accumulate_step_regions: bad argument")
+
+    def amplitude(self):
+        """Complex amplitude [R, D, W, 3] (complex128)."""
+        return self.A[..., 0] + 1j * self.A[..., 1]
+
+    def spectrum(self):
+        """[R, D, W]: every region's own |A_r|^2."""
+        S = np.empty((self.R, self.D, self.W), dtype=np.float64)
+        rc = _load().oracle_spectrum(self.R * self.D * self.W, self.A.ctypes.data, self.scale,
+                                     S.ctypes.data)
+        if rc != 0:
+            raise ValueError("oracle_spectrum: bad argument")
+        return S
+
+    def spectrum_total(self):
+        """[D, W]: |sum_r A_r|^2 -- amplitudes, not intensities, add up."""
+        tot = np.ascontiguousarray(self.A.sum(axis=0))
+        S = np.empty((self.D, self.W), dtype=np.float64)
+        rc = _load().oracle_spectrum(self.D * self.W, tot.ctypes.data, self.scale, S.ctypes.data)
         if rc != 0:
             raise ValueError("oracle_spectrum: bad argument")
         return S

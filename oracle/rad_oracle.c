@@ -35,6 +35,13 @@
  * interference, linearity/superposition, cyclotron (Schott) harmonics, SI constant,
  * mpmath/numpy brute force.  The spectra of the five BASELINE.json configs themselves
  * have no published values: "parity unpinned" except through those pins.
+ *
+ * Per-region detectors ("which type of local
+ * particle dynamics ... gave rise to an observed radiation spectrum", line 196 the 3e4
+ * particles of one sample, line 285 "a selected example sub-volume"):
+ * oracle_accumulate_step_regions() is the same sum restricted to the particles of each
+ * region, A_r = sum over k in region r; pins: sum_r A_r = A of all particles, an empty
+ * region is exactly zero, regions are independent, masked numpy brute force.
  */
 #include <math.h>
 #include <stddef.h>
@@ -131,6 +138,40 @@ int oracle_accumulate_step(int n_dir, const double *dirs, int n_omega, const dou
         for (int c = 0; c < 6; ++c) dst[c] += acc[c];
     }
 #undef LOAD
+    return 0;
+}
+
+/*
+ * Per-region detectors: particles are sorted by region, region r owns the particles
+ * [offsets[r], offsets[r+1]) (offsets non-decreasing, n_regions+1 entries), and
+ *   A_r[n][j][c] += the sum above over the particles of region r only.
+ * A is [n_regions][n_dir][n_omega][3][2]; bin_idx (optional) selects the same (n, j) bins in
+ * every region.  Written as the definition: one plain oracle_accumulate_step per region
+ * on that region's slice of the state arrays.
+ */
+int oracle_accumulate_step_regions(int n_dir, const double *dirs, int n_omega, const double *omega,
+                                   double dt, double t0, long long step_index, long long n_regions,
+                                   const long long *offsets, int is_f32, const void *rx,
+                                   const void *ry, const void *rz, const void *bx, const void *by,
+                                   const void *bz, const void *bdx, const void *bdy,
+                                   const void *bdz, const void *w, long long n_bins,
+                                   const long long *bin_idx, double *A)
+{
+    if (n_regions <= 0 || !offsets || offsets[0] < 0) return 1;
+    for (long long r = 0; r < n_regions; ++r)
+        if (offsets[r + 1] < offsets[r]) return 1;
+    const size_t es = is_f32 ? sizeof(float) : sizeof(double);
+#define AT(p, k) ((const void *)((const char *)(p) + (size_t)(k) * es))
+    for (long long r = 0; r < n_regions; ++r) {
+        const long long k0 = offsets[r], n_r = offsets[r + 1] - offsets[r];
+        double *A_r = A + (size_t)r * n_dir * n_omega * 6;
+        const int rc = oracle_accumulate_step(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_r,
+                                              is_f32, AT(rx, k0), AT(ry, k0), AT(rz, k0), AT(bx, k0),
+                                              AT(by, k0), AT(bz, k0), AT(bdx, k0), AT(bdy, k0),
+                                              AT(bdz, k0), AT(w, k0), n_bins, bin_idx, A_r);
+        if (rc != 0) return rc;
+    }
+#undef AT
     return 0;
 }
 

@@ -109,11 +109,25 @@ class KHISource:
     """
 
     def __init__(self, n: int, seed: int, dt: float, L=10e-6, B0=50.0, stream=0.2,
-                 sigma=0.01, shear=0.5e-6):
+                 sigma=0.01, shear=0.5e-6, regions=None):
         self.n, self.dt, self.L, self.B0, self.shear = n, dt, L, B0, shear
         self.r = np.stack([L * uniform01(seed, s, n) for s in (0, 1, 2)], axis=0)
         self.b = np.stack([sigma * normal01(seed, 10 + s, n) for s in (0, 1, 2)], axis=0)
         self.b[0] += np.where(self.r[1] < 0.5 * L, stream, -stream)
+        self.region_offsets = None
+        if regions is not None:
+            # sub-volumes: an (Rx, Ry) grid of boxes in the x-y plane; particles are stored
+            # sorted by the box their INITIAL position lies in (region id = ix*Ry + iy), as a
+            # PIC code stores them cell by cell.  Membership is kept for the run: over the few
+            # hundred steps of 1e-17 s used here a particle moves < 1 nm.
+            rx_n, ry_n = regions
+            ix = np.minimum((self.r[0] / L * rx_n).astype(np.int64), rx_n - 1)
+            iy = np.minimum((self.r[1] / L * ry_n).astype(np.int64), ry_n - 1)
+            rid = ix * ry_n + iy
+            order = np.argsort(rid, kind="stable")
+            self.r, self.b = self.r[:, order], self.b[:, order]
+            counts = np.bincount(rid, minlength=rx_n * ry_n)
+            self.region_offsets = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
         g = 1.0 / np.sqrt(1.0 - np.sum(self.b * self.b, axis=0))
         self.qm = (-E_CHARGE / M_ELECTRON) / g      # q/(gamma m); gamma is conserved (E=0)
         self.w = np.ones(n)
@@ -164,6 +178,18 @@ class Workload:
     def updates_per_step(self) -> int:
         return self.n_particles * self.n_dir * self.n_omega
 
+    @property
+    def n_regions(self) -> int:
+        rg = self.extra.get("regions")
+        return 1 if rg is None else int(rg[0] * rg[1])
+
+    def region_offsets(self, n_particles: Optional[int] = None) -> np.ndarray:
+        """[n_regions+1] int64 offsets of the region-sorted particle arrays steps() yields."""
+        N = self.n_particles if n_particles is None else n_particles
+        if self.kind != "khi" or self.extra.get("regions") is None:
+            return np.array([0, N], dtype=np.int64)
+        return KHISource(N, self.seed, self.dt, **self.extra).region_offsets
+
     def steps(self, n_steps: Optional[int] = None, n_particles: Optional[int] = None
               ) -> Iterator[tuple]:
         """Yield (step_index, [10 arrays of state_dtype]); optionally only the first
@@ -187,7 +213,8 @@ SWEEP_SHAPES = ((16, 4096), (64, 1024), (256, 256), (1024, 64))
 
 
 def make_workload(cfg: str) -> Workload:
-    """cfg in {"0","1","2","3a","3b","3c","3d","4","4b"} (BASELINE.json configs, 0-based)."""
+    """cfg in {"0","1","2","3a","3b","3c","3d","4","4b"} (BASELINE.json configs, 0-based),
+    or "5r": the per-region (sub-volume) detector workload of SURVEY.md section 8(f) NEXT-2."""
     if cfg == "0":
         wc = 1e14
         return Workload("cfg0_tiny_helical", 256, 128, 1.0 / (20.0 * wc),
@@ -209,7 +236,13 @@ def make_workload(cfg: str) -> Workload:
     if cfg == "4b":
         return Workload("cfg4b_streaming_1x8", 16777216, 4, 1e-17, dirs_fibonacci(1),
                         omega_log(8), np.float32, BASE_SEED + 4, "khi")
+    if cfg == "5r":
+        # smallest KHI run = 192 x 256 x 12 cells x 9 particles per cell on 16
+        # GPUs -> 331 776 particles per GPU; line 196: one ML sample = the ~3e4 particles of a
+        # sub-volume -> 12 sub-volumes; line 184: "spectrum observed in one direction".
+        return Workload("cfg5r_regions_12x1x512", 331776, 200, 1e-17, np.array([[1.0, 0.0, 0.0]]),
+                        omega_log(512), np.float32, BASE_SEED + 5, "khi", extra={"regions": (2, 6)})
     raise KeyError(cfg)
 
 
-ALL_CONFIGS = ("0", "1", "2", "3a", "3b", "3c", "3d", "4", "4b")
+ALL_CONFIGS = ("0", "1", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r")

@@ -313,3 +313,92 @@ def test_p10_frequency_integral_matches_angular_power(oracle_mod):
     # observer-time signal at either edge; equal by periodicity): add it beyond the grid
     integral = np.sum(S) * dw + 2.0 * jump2 / (om[-1] + 0.5 * dw)
     assert integral == pytest.approx(np.pi * power, rel=2e-4)
+
+
+# ------------------------------------------------- P11 per-region detectors (NEXT-2)
+def _region_case(rng, T=4, sizes=(5, 0, 9, 1, 7)):
+    off = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+    return off, _random_steps(rng, int(off[-1]), T)
+
+
+def test_p11_regions_sum_to_the_global_detector_and_are_independent(oracle_mod):
+    """A_r = the sum over the particles of region r: (i) sum_r A_r = A of all particles,
+    (ii) an empty region is exactly zero, (iii) region r equals a plain detector fed only
+    region r's particles, (iv) changing the particles of one region leaves the others alone,
+    (v) the total spectrum is |sum_r A_r|^2, not sum_r |A_r|^2."""
+    rng = np.random.default_rng(11)
+    off, steps = _region_case(rng)
+    R = len(off) - 1
+    ro = oracle_mod.RegionOracle(R, DIRS, OMEGA, DT, t0=2e-17, scale=1.0)
+    for t, st in steps:
+        ro.accumulate_step(t, off, *st)
+    glob = _run(oracle_mod, DIRS, OMEGA, DT, steps, t0=2e-17)
+    A = ro.amplitude()
+    scale = np.abs(glob.amplitude()).max()
+    assert np.allclose(A.sum(0), glob.amplitude(), rtol=0, atol=1e-13 * scale)
+    assert np.all(ro.A[1] == 0.0)
+    for r in range(R):
+        sub = [(t, [a[off[r]:off[r + 1]] for a in st]) for t, st in steps]
+        assert np.array_equal(A[r], _run(oracle_mod, DIRS, OMEGA, DT, sub, t0=2e-17).amplitude())
+    assert np.allclose(ro.spectrum_total(), glob.spectrum(), rtol=1e-11)
+    assert not np.allclose(ro.spectrum().sum(0), glob.spectrum(), rtol=1e-3)
+    # (iv)
+    steps2 = [(t, [a.copy() for a in st]) for t, st in steps]
+    for t, st in steps2:
+        st[6][off[2]:off[3]] *= -3.0
+    ro2 = oracle_mod.RegionOracle(R, DIRS, OMEGA, DT, t0=2e-17, scale=1.0)
+    for t, st in steps2:
+        ro2.accumulate_step(t, off, *st)
+    for r in (0, 1, 3, 4):
+        assert np.array_equal(ro2.A[r], ro.A[r])
+    assert not np.allclose(ro2.A[2], ro.A[2])
+
+
+def test_p11_regions_bruteforce_masked_numpy(oracle_mod):
+    """Independent formulation: one pass over ALL particles with a region-membership mask
+    (no slicing), numpy complex128; offsets[0] > 0 and a tail beyond offsets[-1] are skipped."""
+    rng = np.random.default_rng(111)
+    T, N = 3, 20
+    steps = _random_steps(rng, N, T)
+    off = np.array([2, 6, 6, 13, 17], dtype=np.int64)          # particles 0,1 and 17..19 in no region
+    R = len(off) - 1
+    rid = np.full(N, -1)
+    for r in range(R):
+        rid[off[r]:off[r + 1]] = r
+    ro = oracle_mod.RegionOracle(R, DIRS, OMEGA, DT, scale=1.0)
+    ref = np.zeros((R, len(DIRS), len(OMEGA), 3), dtype=np.complex128)
+    for t, st in steps:
+        ro.accumulate_step(t, off, *st)
+        r_, be, bd, w = np.stack(st[0:3], 1), np.stack(st[3:6], 1), np.stack(st[6:9], 1), st[9]
+        for i, n in enumerate(UNIT):
+            vec = np.cross(n, np.cross(n - be, bd))                       # [N,3]
+            a = w[:, None] * vec / (1.0 - be @ n)[:, None] ** 2
+            ph = np.exp(1j * OMEGA[None, :] * (t * DT - (r_ @ n) / C)[:, None])   # [N,W]
+            for r in range(R):
+                m = (rid == r).astype(float)
+                ref[r, i] += np.einsum("k,kc,kw->wc", m, a, ph) * DT
+    assert np.allclose(ro.amplitude(), ref, rtol=0, atol=1e-12 * np.abs(ref).max())
+    assert np.allclose(ro.spectrum(), (np.abs(ref) ** 2).sum(-1), rtol=1e-11, atol=0)
+
+
+def test_p11_regions_bin_subset_and_f32(oracle_mod):
+    rng = np.random.default_rng(112)
+    off, steps = _region_case(rng, T=2)
+    steps32 = [(t, [a.astype(np.float32) for a in st]) for t, st in steps]
+    R = len(off) - 1
+    full = oracle_mod.RegionOracle(R, DIRS, OMEGA, DT, scale=1.0)
+    bins = np.array([1, len(OMEGA) + 2, 3 * len(OMEGA) - 1], dtype=np.int64)
+    sub = oracle_mod.RegionOracle(R, DIRS, OMEGA, DT, scale=1.0, bins=bins)
+    for t, st in steps32:
+        full.accumulate_step(t, off, *st)
+        sub.accumulate_step(t, off, *st)
+    Sf, Ss = full.spectrum().reshape(R, -1), sub.spectrum().reshape(R, -1)
+    assert np.array_equal(Sf[:, bins], Ss[:, bins])
+    mask = np.ones(Sf.shape[1], bool); mask[bins] = False
+    assert np.all(Ss[:, mask] == 0.0)
+    # fp32 state is promoted value for value
+    steps64 = [(t, [a.astype(np.float64) for a in st]) for t, st in steps32]
+    f64 = oracle_mod.RegionOracle(R, DIRS, OMEGA, DT, scale=1.0)
+    for t, st in steps64:
+        f64.accumulate_step(t, off, *st)
+    assert np.array_equal(f64.A, full.A)

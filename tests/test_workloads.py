@@ -35,7 +35,8 @@ def test_config_shapes(cfg):
     sizes = {"0": (256, 128, 8, 64), "1": (65536, 1000, 128, 512), "2": (1048576, 2000, 256, 1024),
              "3a": (262144, 200, 16, 4096), "3b": (262144, 200, 64, 1024),
              "3c": (262144, 200, 256, 256), "3d": (262144, 200, 1024, 64),
-             "4": (16777216, 4, 16, 128), "4b": (16777216, 4, 1, 8)}[cfg]
+             "4": (16777216, 4, 16, 128), "4b": (16777216, 4, 1, 8),
+             "5r": (331776, 200, 1, 512)}[cfg]
     assert (w.n_particles, w.n_steps, w.n_dir, w.n_omega) == sizes
     assert w.state_dtype == (np.float64 if cfg == "0" else np.float32)
 
@@ -93,3 +94,25 @@ def test_cfg0_oracle_regression_fixture(oracle_mod):
     for t, st in w.steps():
         o.accumulate_step(t, *st)
     assert np.allclose(o.spectrum(), gold, rtol=1e-12, atol=0)
+
+
+def test_region_workload_is_sorted_by_sub_volume():
+    """cfg 5r: particles come sorted by the (2 x 6) x-y box of their initial position and the
+    offsets partition them; the unsorted generator yields the same particle set."""
+    w = wl.make_workload("5r")
+    assert w.n_regions == 12
+    n = 6000
+    off = w.region_offsets(n)
+    assert off.shape == (13,) and off[0] == 0 and off[-1] == n and np.all(np.diff(off) > 0)
+    (_, st), = list(w.steps(n_steps=1, n_particles=n))
+    L = 10e-6
+    rid = np.minimum((st[0].astype(np.float64) / L * 2).astype(int), 1) * 6 + \
+        np.minimum((st[1].astype(np.float64) / L * 6).astype(int), 5)
+    assert np.all(np.diff(rid) >= 0)
+    for r in range(12):
+        assert np.all(rid[off[r]:off[r + 1]] == r)
+    plain = wl.Workload("p", n, 1, w.dt, w.dirs, w.omega, np.float32, w.seed, "khi")
+    (_, st0), = list(plain.steps())
+    assert np.array_equal(np.sort(st0[0]), np.sort(st[0]))
+    assert wl.make_workload("1").n_regions == 1
+    assert np.array_equal(wl.make_workload("1").region_offsets(10), [0, 10])
