@@ -118,9 +118,15 @@ def time_oracle(w, state, n_bins_target=None, budget_s=15.0):
 
     def run(nb):
         bins = np.unique(np.linspace(0, total - 1, nb).round().astype(np.int64))
-        o = oracle.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=bins)
-        t0 = time.perf_counter()
-        o.accumulate_step(0, *state)
+        if w.n_regions > 1:       # per-region detectors: every particle feeds its own region's bins
+            o = oracle.RegionOracle(w.n_regions, w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=bins)
+            off = w.region_offsets(n)
+            t0 = time.perf_counter()
+            o.accumulate_step(0, off, *state)
+        else:
+            o = oracle.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=bins)
+            t0 = time.perf_counter()
+            o.accumulate_step(0, *state)
         dt = time.perf_counter() - t0
         return bins.shape[0] * n / dt, dt, bins.shape[0]
 
@@ -198,16 +204,25 @@ def run_ours(args):
     dev_states = [[a.cuda(non_blocking=True) for a in st] for st in host_states]
     torch.cuda.synchronize()
 
+    R = w.n_regions
+    off = w.region_offsets(n) if R > 1 else None
     det = binding.Detector(w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0, state_dtype=w.state_dtype,
-                           device=local)
-    spec_dev = torch.empty(w.n_dir, w.n_omega, dtype=torch.float64, device="cuda")
+                           device=local, n_regions=R if R > 1 else 0)
+    spec_dev = torch.empty(R * w.n_dir, w.n_omega, dtype=torch.float64, device="cuda")
     if world > 1:
         det_glob = binding.Detector(w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0,
-                                    state_dtype=w.state_dtype, device=local)
-        amp_buf = torch.empty(w.n_dir, w.n_omega, 3, 2, dtype=torch.float64, device="cuda")
+                                    state_dtype=w.state_dtype, device=local, n_regions=R if R > 1 else 0)
+        amp_buf = torch.empty(R * w.n_dir, w.n_omega, 3, 2, dtype=torch.float64, device="cuda")
+
+    def accumulate(i, host=False):
+        st = (host_states if host else dev_states)[i % ring]
+        if R > 1:
+            (det.accumulate_step_regions_host if host else det.accumulate_step_regions)(i, off, st)
+        else:
+            (det.accumulate_step_host if host else det.accumulate_step)(i, st)
 
     def step(i):
-        det.accumulate_step(i, dev_states[i % ring])
+        accumulate(i)
         if world > 1:   # the one exchange of the path: sum complex amplitudes, then |A|^2
             multi.global_spectrum(det, det_glob, amp_buf, out=spec_dev)
         else:
@@ -248,7 +263,7 @@ def run_ours(args):
     k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     k0.record()
     for i in range(W, W + K):
-        det.accumulate_step(i, dev_states[i % ring])
+        accumulate(i)
     k1.record()
     torch.cuda.synchronize()
     kernel_ms = k0.elapsed_time(k1) / K
@@ -289,15 +304,15 @@ def run_ours(args):
     e2e = None
     if not args.no_e2e:
         det.reset()
-        spec_host = np.empty((w.n_dir, w.n_omega), dtype=np.float64)
+        spec_host = np.empty((R * w.n_dir, w.n_omega), dtype=np.float64)
         ke = max(1, min(K, 50))
         for i in range(min(W, 3)):
-            det.accumulate_step_host(i, host_states[i % ring])
+            accumulate(i, host=True)
         barrier()
         a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a0.record()
         for i in range(W, W + ke):
-            det.accumulate_step_host(i, host_states[i % ring])
+            accumulate(i, host=True)
             if world > 1:
                 multi.global_spectrum(det, det_glob, amp_buf, out=spec_dev)
                 spec_host[...] = spec_dev.cpu().numpy()
@@ -326,7 +341,8 @@ def run_ours(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32 phase/amplitude, f64 set-up and accumulators", "data": "synthetic",
-            "config": {"workload": w.name, "n_particles_per_gpu": n, "n_dir": w.n_dir, "n_omega": w.n_omega,
+            "config": {"workload": w.name, "n_particles_per_gpu": n, "n_regions": R, "n_dir": w.n_dir,
+                       "n_omega": w.n_omega,
                        "state_dtype": np.dtype(w.state_dtype).name, "parallelism": f"particle-shard x{world}",
                        "l2": f"ring of {ring} distinct step inputs ({ring * bytes_per_step / 2**20:.0f} MiB) + "
                              f"L2 flush before the timed region"},

@@ -13,6 +13,15 @@
  *   S(n, w_j) = scale * |A(n, w_j)|^2              (d^2 I / dOmega dw)
  *
  * on a grid of n_dir observation directions n and n_omega angular frequencies w_j.
+ *
+ * Per-region (sub-volume) detectors (rad_config.n_regions > 1): the ML application of the
+ * paper learns from pairs (particles of a sub-volume, radiation of that sub-volume) --
+ * PAPER.md line 184 "which type of local particle dynamics ... gave rise to an observed
+ * radiation spectrum observed in one direction", line 196 (the 3e4 particles of one sample),
+ * line 285 "a selected example sub-volume".  The handle then holds one amplitude per region,
+ *   A_r(n, w_j) = the same sum over the particles of region r only,
+ * fed by rad_accumulate_step_regions(); sum_r A_r is the detector of all particles
+ * (rad_spectrum_total).
  * Units are SI: r [m], beta = v/c [1], betadot [1/s], omega [rad/s], dt [s];
  * c = 299 792 458 m/s.  Readings of the paper where it is silent: DESIGN.md.
  *
@@ -75,6 +84,8 @@ typedef struct {
     double scale;          /* S = scale*|A|^2; 0 -> SI e^2/(16 pi^3 eps0 c) J s            */
     int32_t state_dtype;   /* rad_dtype of the 10 particle arrays                          */
     uint32_t flags;        /* RAD_FLAG_*                                                   */
+    int32_t n_regions;     /* 0 or 1: one detector; R > 1: R per-region detectors          */
+    int32_t reserved;      /* must be 0                                                    */
 } rad_config;
 
 /* Create a detector: copies dirs/omega, builds the device tables, zeroes A.
@@ -103,10 +114,44 @@ RAD_API rad_status rad_accumulate_step_host(rad_handle *h, int64_t step_index, i
                                             const void *bdx, const void *bdy, const void *bdz,
                                             const void *w, void *cuda_stream);
 
+/* Per-region form (handles created with n_regions = R > 1; also valid with R = 1).
+ * The particle arrays are sorted by region: region r owns the particles
+ * [region_offsets[r], region_offsets[r+1]); region_offsets is HOST memory, n_regions + 1
+ * non-decreasing entries, region_offsets[0] >= 0; it is copied before the call returns.
+ * Particles before region_offsets[0] or from region_offsets[n_regions] on belong to no
+ * region and are not read.  Empty regions are allowed.  A_r += contributions of region r's
+ * particles at time t0 + step_index*dt, for every r, in ONE kernel launch.
+ * n_regions must equal the handle's.  rad_accumulate_step() on a handle with R > 1 fails
+ * with RAD_ERR_INVALID_ARG (it would not say which region the particles belong to). */
+RAD_API rad_status rad_accumulate_step_regions(rad_handle *h, int64_t step_index, int32_t n_regions,
+                                               const int64_t *region_offsets,
+                                               const void *rx, const void *ry, const void *rz,
+                                               const void *bx, const void *by, const void *bz,
+                                               const void *bdx, const void *bdy, const void *bdz,
+                                               const void *w, void *cuda_stream);
+
+/* Same with the state in HOST memory (see rad_accumulate_step_host); the arrays are read
+ * from element region_offsets[0] to region_offsets[n_regions] - 1. */
+RAD_API rad_status rad_accumulate_step_regions_host(rad_handle *h, int64_t step_index, int32_t n_regions,
+                                                    const int64_t *region_offsets,
+                                                    const void *rx, const void *ry, const void *rz,
+                                                    const void *bx, const void *by, const void *bz,
+                                                    const void *bdx, const void *bdy, const void *bdz,
+                                                    const void *w, void *cuda_stream);
+
+/* In rad_spectrum, rad_amplitude and rad_add_amplitude a handle with R = n_regions > 1 adds a
+ * leading region dimension: spectrum out[R][n_dir][n_omega], amplitude
+ * out/amp[R][n_dir][n_omega][3][2]. */
+
 /* out[n_dir][n_omega] (row-major, fp64) = scale * sum_c |A_c|^2.  Non-destructive.
  * out_on_device != 0: `out` is DEVICE memory, call is asynchronous; else HOST and the
  * call returns after the data has arrived. */
 RAD_API rad_status rad_spectrum(rad_handle *h, double *out, int out_on_device, void *cuda_stream);
+
+/* out[n_dir][n_omega] = scale * sum_c |sum_r A_r,c|^2: the detector of all particles of all
+ * regions (amplitudes, not intensities, add up: PAPER.md line 80).  Equals rad_spectrum for
+ * R = 1.  Same HOST/DEVICE convention as rad_spectrum. */
+RAD_API rad_status rad_spectrum_total(rad_handle *h, double *out, int out_on_device, void *cuda_stream);
 
 /* out[n_dir][n_omega][3][2] fp64: (re, im) of the x, y, z components of A
  * ("complex amplitude and phase for each wavelength and direction"). */

@@ -21,8 +21,9 @@ RAD_F32, RAD_F64 = 0, 1
 RAD_FLAG_DETERMINISTIC, RAD_FLAG_FORCE_GENERAL = 1, 2
 
 ABI_SYMBOLS = (
-    "rad_create", "rad_accumulate_step", "rad_accumulate_step_host", "rad_spectrum",
-    "rad_amplitude", "rad_add_amplitude", "rad_reset", "rad_destroy", "rad_launch_count",
+    "rad_create", "rad_accumulate_step", "rad_accumulate_step_host",
+    "rad_accumulate_step_regions", "rad_accumulate_step_regions_host", "rad_spectrum",
+    "rad_spectrum_total", "rad_amplitude", "rad_add_amplitude", "rad_reset", "rad_destroy", "rad_launch_count",
     "rad_kernel_variant", "rad_status_string", "rad_last_error", "rad_version",
 )
 
@@ -34,6 +35,7 @@ class rad_config(ctypes.Structure):
         ("dirs", ctypes.c_void_p), ("omega", ctypes.c_void_p),
         ("dt", ctypes.c_double), ("t0", ctypes.c_double), ("scale", ctypes.c_double),
         ("state_dtype", ctypes.c_int32), ("flags", ctypes.c_uint32),
+        ("n_regions", ctypes.c_int32), ("reserved", ctypes.c_int32),
     ]
 
 
@@ -64,7 +66,11 @@ def load(path: Optional[Path] = None) -> ctypes.CDLL:
         f = getattr(lib, name)
         f.restype = ctypes.c_int
         f.argtypes = [vp, i64, i64] + [vp] * 10 + [vp]
-    for name in ("rad_spectrum", "rad_amplitude"):
+    for name in ("rad_accumulate_step_regions", "rad_accumulate_step_regions_host"):
+        f = getattr(lib, name)
+        f.restype = ctypes.c_int
+        f.argtypes = [vp, i64, ctypes.c_int32, vp] + [vp] * 10 + [vp]
+    for name in ("rad_spectrum", "rad_spectrum_total", "rad_amplitude"):
         f = getattr(lib, name)
         f.restype = ctypes.c_int
         f.argtypes = [vp, vp, ctypes.c_int, vp]
@@ -104,12 +110,13 @@ def _check(status: int, handle) -> None:
 
 # ------------------------------------------------------------------ ABI-named functions
 def rad_create(dirs, omega, dt: float, t0: float = 0.0, scale: float = 0.0,
-               state_dtype: int = RAD_F32, flags: int = 0, device: int = 0) -> int:
+               state_dtype: int = RAD_F32, flags: int = 0, device: int = 0, n_regions: int = 0) -> int:
     """-> opaque handle (int).  dirs [D,3], omega [W]: HOST fp64 (copied by the library)."""
     dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
     omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
     cfg = rad_config(ctypes.sizeof(rad_config), device, dirs.shape[0], omega.shape[0],
-                     dirs.ctypes.data, omega.ctypes.data, dt, t0, scale, state_dtype, flags)
+                     dirs.ctypes.data, omega.ctypes.data, dt, t0, scale, state_dtype, flags,
+                     n_regions, 0)
     h = ctypes.c_void_p()
     _check(load().rad_create(ctypes.byref(cfg), ctypes.byref(h)), None)
     return h.value
@@ -127,8 +134,28 @@ def rad_accumulate_step_host(handle: int, step_index: int, n_particles: int,
     _check(load().rad_accumulate_step_host(handle, step_index, n_particles, *state_ptrs, stream), handle)
 
 
+def rad_accumulate_step_regions(handle: int, step_index: int, region_offsets: np.ndarray,
+                                state_ptrs: Sequence[int], stream: int = 0) -> None:
+    """region_offsets: HOST int64 [R+1]; state_ptrs: 10 DEVICE pointers."""
+    off = np.ascontiguousarray(region_offsets, dtype=np.int64)
+    _check(load().rad_accumulate_step_regions(handle, step_index, off.shape[0] - 1, off.ctypes.data,
+                                              *state_ptrs, stream), handle)
+
+
+def rad_accumulate_step_regions_host(handle: int, step_index: int, region_offsets: np.ndarray,
+                                     state_ptrs: Sequence[int], stream: int = 0) -> None:
+    """region_offsets: HOST int64 [R+1]; state_ptrs: 10 HOST pointers."""
+    off = np.ascontiguousarray(region_offsets, dtype=np.int64)
+    _check(load().rad_accumulate_step_regions_host(handle, step_index, off.shape[0] - 1, off.ctypes.data,
+                                                   *state_ptrs, stream), handle)
+
+
 def rad_spectrum(handle: int, out_ptr: int, out_on_device: bool, stream: int = 0) -> None:
     _check(load().rad_spectrum(handle, out_ptr, int(out_on_device), stream), handle)
+
+
+def rad_spectrum_total(handle: int, out_ptr: int, out_on_device: bool, stream: int = 0) -> None:
+    _check(load().rad_spectrum_total(handle, out_ptr, int(out_on_device), stream), handle)
 
 
 def rad_amplitude(handle: int, out_ptr: int, out_on_device: bool, stream: int = 0) -> None:
@@ -160,13 +187,18 @@ class Detector:
     """Owns one rad_handle.  State may be torch CUDA tensors (device path) or numpy /
     pinned torch CPU tensors (host path, copies inside the library)."""
 
-    def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, state_dtype=np.float32, flags=0, device=0):
+    def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, state_dtype=np.float32, flags=0, device=0,
+                 n_regions=0):
         self.D = int(np.asarray(dirs).reshape(-1, 3).shape[0])
         self.W = int(np.asarray(omega).reshape(-1).shape[0])
+        self.R = max(1, int(n_regions))
         self.np_dtype = np.dtype(state_dtype)
         code = {np.dtype(np.float32): RAD_F32, np.dtype(np.float64): RAD_F64}[self.np_dtype]
         self.device = device
-        self.handle = rad_create(dirs, omega, dt, t0, scale, code, flags, device)
+        self.handle = rad_create(dirs, omega, dt, t0, scale, code, flags, device, n_regions)
+
+    def _shape(self, *tail):
+        return ((self.R,) if self.R > 1 else ()) + (self.D, self.W) + tail
 
     # -- helpers
     @staticmethod
@@ -204,21 +236,43 @@ class Detector:
         n, ptrs = self._ptrs(state, want_cuda=False)
         rad_accumulate_step_host(self.handle, step_index, n, ptrs, self._stream())
 
+    def accumulate_step_regions(self, step_index: int, region_offsets, state) -> None:
+        """Per-region detectors: state sorted by region, region r = [offsets[r], offsets[r+1])."""
+        n, ptrs = self._ptrs(state, want_cuda=True)
+        if int(region_offsets[-1]) > n:
+            raise ValueError("region_offsets[-1] exceeds the state length")
+        rad_accumulate_step_regions(self.handle, step_index, region_offsets, ptrs, self._stream())
+
+    def accumulate_step_regions_host(self, step_index: int, region_offsets, state) -> None:
+        n, ptrs = self._ptrs(state, want_cuda=False)
+        if int(region_offsets[-1]) > n:
+            raise ValueError("region_offsets[-1] exceeds the state length")
+        rad_accumulate_step_regions_host(self.handle, step_index, region_offsets, ptrs, self._stream())
+
     def spectrum(self, out=None):
-        """out: optional torch CUDA fp64 tensor [D, W] (asynchronous); default -> numpy."""
+        """out: optional torch CUDA fp64 tensor [(R,) D, W] (asynchronous); default -> numpy."""
         if out is not None:
             rad_spectrum(self.handle, out.data_ptr(), True, self._stream())
             return out
-        res = np.empty((self.D, self.W), dtype=np.float64)
+        res = np.empty(self._shape(), dtype=np.float64)
         rad_spectrum(self.handle, res.ctypes.data, False, self._stream())
         return res
 
+    def spectrum_total(self, out=None):
+        """[D, W]: scale * |sum over regions of A_r|^2."""
+        if out is not None:
+            rad_spectrum_total(self.handle, out.data_ptr(), True, self._stream())
+            return out
+        res = np.empty((self.D, self.W), dtype=np.float64)
+        rad_spectrum_total(self.handle, res.ctypes.data, False, self._stream())
+        return res
+
     def amplitude(self, out=None):
-        """Complex amplitude; default -> numpy complex128 [D, W, 3]."""
+        """Complex amplitude; default -> numpy complex128 [(R,) D, W, 3]."""
         if out is not None:
             rad_amplitude(self.handle, out.data_ptr(), True, self._stream())
             return out
-        res = np.empty((self.D, self.W, 3, 2), dtype=np.float64)
+        res = np.empty(self._shape(3, 2), dtype=np.float64)
         rad_amplitude(self.handle, res.ctypes.data, False, self._stream())
         return res[..., 0] + 1j * res[..., 1]
 

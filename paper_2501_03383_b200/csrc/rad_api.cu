@@ -50,7 +50,10 @@ void free_all(Handle &h)
 {
     cudaFree(h.dirs_d); cudaFree(h.basis_d); cudaFree(h.F_d); cudaFree(h.Ff_d); cudaFree(h.fl_d);
     cudaFree(h.acc_d); cudaFree(h.partial_d); cudaFree(h.stage_d[0]); cudaFree(h.stage_d[1]);
-    cudaFree(h.out_d);
+    cudaFree(h.out_d); cudaFree(h.chunks_d); cudaFree(h.reg_cstart_d);
+    if (h.chunks_h) cudaFreeHost(h.chunks_h);
+    if (h.reg_cstart_h) cudaFreeHost(h.reg_cstart_h);
+    if (h.reg_uploaded) cudaEventDestroy(h.reg_uploaded);
     for (int i = 0; i < 2; ++i) {
         if (h.copied[i]) cudaEventDestroy(h.copied[i]);
         if (h.consumed[i]) cudaEventDestroy(h.consumed[i]);
@@ -81,17 +84,89 @@ void choose_tile(Handle &h)
 // (rounding), and the fold (a3) stays ~1 % of the sweep.
 int choose_chunk(const Handle &h, long long n)
 {
-    const long long gx = (h.n_wtiles + kWarpsPerBlock - 1) / kWarpsPerBlock;
-    const long long want_blocks = 8LL * h.sm_count * kMinBlocks;
-    long long n_chunks = (want_blocks + gx - 1) / gx;
-    long long chunk = (n + n_chunks - 1) / n_chunks;
-    chunk = (chunk + kBatch - 1) / kBatch * kBatch;
-    if (chunk < 256) chunk = 256;
-    if (chunk > 4096) chunk = 4096;
-    // small inputs: prefer filling the SMs over amortising the fold
-    while (chunk > kBatch && gx * ((n + chunk - 1) / chunk) < (long long)h.sm_count * kMinBlocks) chunk /= 2;
-    chunk = (chunk + kBatch - 1) / kBatch * kBatch;
-    return (int)chunk;
+    // a warp task = (warp tile, chunk); a block runs 4 tasks; cap blocks are resident at once
+    const long long cap = (long long)h.sm_count * kMinBlocks;
+    auto blocks_at = [&](long long chunk) {
+        return (h.n_wtiles * ((n + chunk - 1) / chunk) + kWarpsPerBlock - 1) / kWarpsPerBlock;
+    };
+    if (blocks_at(256) >= 4 * cap) {  // large input: ~8 waves keep the tail of the grid small
+        const long long want_tasks = 8 * cap * kWarpsPerBlock;
+        const long long n_chunks = (want_tasks + h.n_wtiles - 1) / h.n_wtiles;
+        long long chunk = (n + n_chunks - 1) / n_chunks;
+        chunk = (chunk + kBatch - 1) / kBatch * kBatch;
+        return (int)std::min<long long>(std::max<long long>(chunk, 256), 4096);
+    }
+    // small input (a few waves at most): fit the grid to whole waves.  For w = 1..4 waves take the
+    // smallest chunk whose grid fits into w waves; cost ~ w * (chunk + per-chunk overhead of
+    // ~32 particle-equivalents for constants, fold and launch ramp); keep the cheapest.
+    long long best = 4096, best_cost = -1;
+    for (int w = 1; w <= 4; ++w) {
+        long long lo = kBatch, hi = 4096;  // smallest multiple of 32 with blocks_at(chunk) <= w*cap
+        if (blocks_at(hi) > w * cap) continue;
+        while (lo < hi) {
+            const long long mid = (lo + hi) / 2 / kBatch * kBatch;
+            if (blocks_at(mid) <= w * cap) hi = mid; else lo = mid + kBatch;
+        }
+        const long long cost = w * (lo + 32);
+        if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = lo; }
+    }
+    return (int)best;
+}
+
+// Per-region calls: (re)build the chunk table for these offsets (shifted so that the first
+// region starts at particle `base` of the device arrays) and upload it on stream s.  Chunks
+// never straddle a region; a region of n_r particles is cut into ceil(n_r / chunk) chunks
+// of equal length (rounded up to whole 32-particle batches).
+rad_status build_chunk_table(Handle &h, const int64_t *off, long long base, int chunk, cudaStream_t s)
+{
+    bool same = h.reg_chunk == chunk && (int)h.reg_offsets.size() == h.R + 1;
+    for (int r = 0; same && r <= h.R; ++r) same = h.reg_offsets[r] == off[r] - base;
+    if (same) return RAD_OK;
+    size_t need = 0;
+    for (int r = 0; r < h.R; ++r) need += (size_t)((off[r + 1] - off[r] + chunk - 1) / chunk);
+    if (need > (size_t)INT32_MAX) return fail(&h, RAD_ERR_INVALID_ARG, "too many particle chunks");
+    if (h.reg_uploaded) RAD_CUDA(&h, cudaEventSynchronize(h.reg_uploaded));  // pinned copy is free again
+    else RAD_CUDA(&h, cudaEventCreateWithFlags(&h.reg_uploaded, cudaEventDisableTiming));
+    if (need > h.reg_cap || !h.reg_cstart_h) {
+        RAD_CUDA(&h, cudaDeviceSynchronize());
+        cudaFree(h.chunks_d); h.chunks_d = nullptr;
+        if (h.chunks_h) cudaFreeHost(h.chunks_h);
+        h.chunks_h = nullptr; h.reg_cap = 0;
+        const size_t cap = std::max<size_t>(need + need / 4, 64);
+        bool ok = cudaMallocHost(&h.chunks_h, cap * sizeof(ChunkRec)) == cudaSuccess &&
+                  cudaMalloc(&h.chunks_d, cap * sizeof(ChunkRec)) == cudaSuccess;
+        if (ok && !h.reg_cstart_h)
+            ok = cudaMallocHost(&h.reg_cstart_h, (h.R + 1) * sizeof(int)) == cudaSuccess &&
+                 cudaMalloc(&h.reg_cstart_d, (h.R + 1) * sizeof(int)) == cudaSuccess;
+        if (!ok) {
+            cudaGetLastError();
+            return fail(&h, RAD_ERR_ALLOC, "allocation of the region chunk table failed");
+        }
+        h.reg_cap = cap;
+    }
+    int n = 0;
+    for (int r = 0; r < h.R; ++r) {
+        h.reg_cstart_h[r] = n;
+        const long long n_r = off[r + 1] - off[r], k0 = off[r] - base;
+        if (n_r == 0) continue;
+        const long long pieces = (n_r + chunk - 1) / chunk;
+        long long len = (n_r + pieces - 1) / pieces;
+        len = (len + kBatch - 1) / kBatch * kBatch;
+        for (long long k = 0; k < n_r; k += len)
+            h.chunks_h[n++] = ChunkRec{k0 + k, (int)std::min(len, n_r - k), r};
+    }
+    h.reg_cstart_h[h.R] = n;
+    h.reg_n_chunks = n;
+    h.reg_chunk = chunk;
+    h.reg_offsets.resize(h.R + 1);
+    for (int r = 0; r <= h.R; ++r) h.reg_offsets[r] = off[r] - base;
+    if (n > 0)
+        RAD_CUDA(&h, cudaMemcpyAsync(h.chunks_d, h.chunks_h, (size_t)n * sizeof(ChunkRec),
+                                     cudaMemcpyHostToDevice, s));
+    RAD_CUDA(&h, cudaMemcpyAsync(h.reg_cstart_d, h.reg_cstart_h, (h.R + 1) * sizeof(int),
+                                 cudaMemcpyHostToDevice, s));
+    RAD_CUDA(&h, cudaEventRecord(h.reg_uploaded, s));
+    return RAD_OK;
 }
 
 rad_status ensure_out(Handle &h, size_t bytes)
@@ -116,12 +191,17 @@ rad_status check_handle(rad_handle *hh)
     return RAD_OK;
 }
 
-rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *const st[10], cudaStream_t s)
+// st: DEVICE arrays.  region_off == NULL: particles [0, n) of the one detector; else n_regions+1
+// HOST offsets into arrays whose element 0 is particle `region_base` of the caller's numbering
+// and n = particles spanned by the regions.
+rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *const st[10], cudaStream_t s,
+                             const int64_t *region_off = nullptr, long long region_base = 0)
 {
     AccumParams p{};
     for (int i = 0; i < 10; ++i) p.st[i] = st[i];
     p.n_particles = n;
-    p.chunk = choose_chunk(h, n);
+    // per-region calls: every region rounds its own chunk count up -> leave room for that
+    p.chunk = choose_chunk(h, region_off ? n + (long long)h.R * 64 : n);
     if (const char *e = getenv("RAD_CHUNK")) {  // tuning/debug override (particles per block)
         const int c = atoi(e);
         if (c >= kBatch) p.chunk = c / kBatch * kBatch;
@@ -135,6 +215,14 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.partial = nullptr;
     p.rot_G = h.rot_G; p.rot_Gf = h.rot_Gf; p.rot_gl = h.rot_gl;
     int n_chunks = (int)((n + p.chunk - 1) / p.chunk);
+    if (region_off) {
+        rad_status st_ = build_chunk_table(h, region_off, region_base, p.chunk, s);
+        if (st_ != RAD_OK) return st_;
+        n_chunks = h.reg_n_chunks;
+        p.chunks = h.chunks_d;
+        if (n_chunks == 0) return RAD_OK;
+    }
+    p.n_chunks = n_chunks;
     int stream_grid = 0;
     if (h.stream_nb) {  // few bins: persistent particle-streaming kernel, one partial slot per block
         const int tile = stream_tile_particles(h.state_f64);
@@ -168,7 +256,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
         h.launches += nl;
     }
     if (h.deterministic) {
-        RAD_CUDA(&h, launch_reduce_partials(h, h.partial_d, n_chunks, s));
+        RAD_CUDA(&h, launch_reduce_partials(h, h.partial_d, n_chunks, region_off ? h.reg_cstart_d : nullptr, s));
         h.launches += 1;
     }
     return RAD_OK;
@@ -193,6 +281,8 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         return fail(nullptr, RAD_ERR_INVALID_ARG, "state_dtype must be RAD_F32 or RAD_F64");
     if (cfg->flags & ~(RAD_FLAG_DETERMINISTIC | RAD_FLAG_FORCE_GENERAL))
         return fail(nullptr, RAD_ERR_INVALID_ARG, "unknown flag bits");
+    if (cfg->n_regions < 0 || cfg->reserved != 0)
+        return fail(nullptr, RAD_ERR_INVALID_ARG, "n_regions must be >= 0 and reserved == 0");
     for (int j = 0; j < cfg->n_omega; ++j) {
         const double w = cfg->omega[j];
         if (!std::isfinite(w) || !(w > 0.0) || (j > 0 && !(w > cfg->omega[j - 1])))
@@ -202,6 +292,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     if (!hh) return fail(nullptr, RAD_ERR_ALLOC, "out of host memory");
     Handle &h = hh->h;
     h.device = cfg->device; h.D = cfg->n_dir; h.W = cfg->n_omega;
+    h.R = cfg->n_regions > 1 ? cfg->n_regions : 1;
     h.dt = cfg->dt; h.t0 = cfg->t0;
     h.scale = cfg->scale == 0.0 ? default_scale() : cfg->scale;
     h.state_f64 = cfg->state_dtype == RAD_F64;
@@ -244,7 +335,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         r.pad[0] = r.pad[1] = r.pad[2] = 0.0f;
     }
     choose_tile(h);
-    h.stream_nb = stream_shape(h.D, h.W, &h.stream_nd);
+    h.stream_nb = h.R > 1 ? 0 : stream_shape(h.D, h.W, &h.stream_nd);  // per-region: bin-owner kernels only
     // uniform grid?  w_j = w_0 + j dw to fp64 rounding -> rotation-recurrence kernel (a2')
     h.uniform = false;
     if (h.W >= 2 * h.strip && !(cfg->flags & RAD_FLAG_FORCE_GENERAL)) {
@@ -276,7 +367,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     e = cudaGetDeviceProperties(&prop, h.device);
     if (e != cudaSuccess) { delete hh; return cuda_fail(nullptr, e, "cudaGetDeviceProperties"); }
     h.sm_count = prop.multiProcessorCount;
-    const size_t acc_bytes = (size_t)h.D * h.w_pad * 4 * sizeof(double);
+    const size_t acc_bytes = (size_t)h.R * h.D * h.w_pad * 4 * sizeof(double);
     bool ok = cudaMalloc(&h.dirs_d, sizeof(DirRec) * h.D) == cudaSuccess &&
               cudaMalloc(&h.basis_d, sizeof(double) * 6 * h.D) == cudaSuccess &&
               cudaMalloc(&h.F_d, sizeof(uint32_t) * h.w_pad) == cudaSuccess &&
@@ -313,6 +404,7 @@ rad_status rad_accumulate_step(rad_handle *hh, int64_t step_index, int64_t n_par
     rad_status st = check_handle(hh);
     if (st != RAD_OK) return st;
     Handle &h = hh->h;
+    if (h.R > 1) return fail(&h, RAD_ERR_INVALID_ARG, "per-region handle: use rad_accumulate_step_regions");
     if (n_particles < 0) return fail(&h, RAD_ERR_INVALID_ARG, "n_particles < 0");
     if (n_particles == 0) return RAD_OK;
     const void *arr[10] = {rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w};
@@ -321,20 +413,48 @@ rad_status rad_accumulate_step(rad_handle *hh, int64_t step_index, int64_t n_par
     return accumulate_device(h, step_index, n_particles, arr, (cudaStream_t)cuda_stream);
 }
 
-rad_status rad_accumulate_step_host(rad_handle *hh, int64_t step_index, int64_t n_particles,
-                                    const void *rx, const void *ry, const void *rz, const void *bx,
-                                    const void *by, const void *bz, const void *bdx, const void *bdy,
-                                    const void *bdz, const void *w, void *cuda_stream)
+static rad_status check_regions(Handle &h, int32_t n_regions, const int64_t *off)
+{
+    if (n_regions != h.R) return fail(&h, RAD_ERR_INVALID_ARG, "n_regions differs from the handle's");
+    if (!off) return fail(&h, RAD_ERR_INVALID_ARG, "region_offsets is NULL");
+    if (off[0] < 0) return fail(&h, RAD_ERR_INVALID_ARG, "region_offsets[0] < 0");
+    for (int r = 0; r < n_regions; ++r)
+        if (off[r + 1] < off[r]) return fail(&h, RAD_ERR_INVALID_ARG, "region_offsets must be non-decreasing");
+    return RAD_OK;
+}
+
+rad_status rad_accumulate_step_regions(rad_handle *hh, int64_t step_index, int32_t n_regions,
+                                       const int64_t *region_offsets, const void *rx, const void *ry,
+                                       const void *rz, const void *bx, const void *by, const void *bz,
+                                       const void *bdx, const void *bdy, const void *bdz, const void *w,
+                                       void *cuda_stream)
 {
     rad_status st = check_handle(hh);
     if (st != RAD_OK) return st;
     Handle &h = hh->h;
-    if (n_particles < 0) return fail(&h, RAD_ERR_INVALID_ARG, "n_particles < 0");
-    if (n_particles == 0) return RAD_OK;
+    st = check_regions(h, n_regions, region_offsets);
+    if (st != RAD_OK) return st;
+    const long long n = region_offsets[n_regions] - region_offsets[0];
+    if (n == 0) return RAD_OK;
     const void *arr[10] = {rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w};
     for (const void *p : arr)
         if (!p) return fail(&h, RAD_ERR_INVALID_ARG, "NULL state array");
-    cudaStream_t s = (cudaStream_t)cuda_stream;
+    if (h.R == 1) {  // one region = the plain call on the sub-range [offsets[0], offsets[1])
+        const size_t esz = h.state_f64 ? 8 : 4;
+        const void *sub[10];
+        for (int i = 0; i < 10; ++i) sub[i] = (const char *)arr[i] + (size_t)region_offsets[0] * esz;
+        return accumulate_device(h, step_index, n, sub, (cudaStream_t)cuda_stream);
+    }
+    // the kernels index the caller's arrays directly: offsets stay absolute (base 0)
+    return accumulate_device(h, step_index, region_offsets[n_regions], arr, (cudaStream_t)cuda_stream,
+                             region_offsets, 0);
+}
+
+// HOST state: elements [first, first + n_particles) of the 10 arrays go through the handle's
+// double-buffered device staging; region_off (optional) are the caller's absolute offsets.
+static rad_status accumulate_host(Handle &h, int64_t step_index, long long first, int64_t n_particles,
+                                  const void *const arr[10], const int64_t *region_off, cudaStream_t s)
+{
     const size_t esz = h.state_f64 ? 8 : 4;
     const size_t stride = ((size_t)n_particles * esz + 255) / 256 * 256;
     const int b = h.stage_next;
@@ -355,17 +475,55 @@ rad_status rad_accumulate_step_host(rad_handle *hh, int64_t step_index, int64_t 
     const void *dev[10];
     for (int i = 0; i < 10; ++i) {
         char *dst = (char *)h.stage_d[b] + stride * i;
-        RAD_CUDA(&h, cudaMemcpyAsync(dst, arr[i], (size_t)n_particles * esz, cudaMemcpyHostToDevice,
-                                     h.copy_stream));
+        RAD_CUDA(&h, cudaMemcpyAsync(dst, (const char *)arr[i] + (size_t)first * esz,
+                                     (size_t)n_particles * esz, cudaMemcpyHostToDevice, h.copy_stream));
         dev[i] = dst;
     }
     RAD_CUDA(&h, cudaEventRecord(h.copied[b], h.copy_stream));
     RAD_CUDA(&h, cudaStreamWaitEvent(s, h.copied[b], 0));
-    st = accumulate_device(h, step_index, n_particles, dev, s);
+    rad_status st = accumulate_device(h, step_index, n_particles, dev, s, region_off, first);
     if (st != RAD_OK) return st;
     RAD_CUDA(&h, cudaEventRecord(h.consumed[b], s));
     h.consumed_valid[b] = true;
     return RAD_OK;
+}
+
+rad_status rad_accumulate_step_host(rad_handle *hh, int64_t step_index, int64_t n_particles,
+                                    const void *rx, const void *ry, const void *rz, const void *bx,
+                                    const void *by, const void *bz, const void *bdx, const void *bdy,
+                                    const void *bdz, const void *w, void *cuda_stream)
+{
+    rad_status st = check_handle(hh);
+    if (st != RAD_OK) return st;
+    Handle &h = hh->h;
+    if (h.R > 1) return fail(&h, RAD_ERR_INVALID_ARG, "per-region handle: use rad_accumulate_step_regions_host");
+    if (n_particles < 0) return fail(&h, RAD_ERR_INVALID_ARG, "n_particles < 0");
+    if (n_particles == 0) return RAD_OK;
+    const void *arr[10] = {rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w};
+    for (const void *p : arr)
+        if (!p) return fail(&h, RAD_ERR_INVALID_ARG, "NULL state array");
+    return accumulate_host(h, step_index, 0, n_particles, arr, nullptr, (cudaStream_t)cuda_stream);
+}
+
+rad_status rad_accumulate_step_regions_host(rad_handle *hh, int64_t step_index, int32_t n_regions,
+                                            const int64_t *region_offsets, const void *rx,
+                                            const void *ry, const void *rz, const void *bx,
+                                            const void *by, const void *bz, const void *bdx,
+                                            const void *bdy, const void *bdz, const void *w,
+                                            void *cuda_stream)
+{
+    rad_status st = check_handle(hh);
+    if (st != RAD_OK) return st;
+    Handle &h = hh->h;
+    st = check_regions(h, n_regions, region_offsets);
+    if (st != RAD_OK) return st;
+    const long long n = region_offsets[n_regions] - region_offsets[0];
+    if (n == 0) return RAD_OK;
+    const void *arr[10] = {rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w};
+    for (const void *p : arr)
+        if (!p) return fail(&h, RAD_ERR_INVALID_ARG, "NULL state array");
+    return accumulate_host(h, step_index, region_offsets[0], n, arr, h.R == 1 ? nullptr : region_offsets,
+                           (cudaStream_t)cuda_stream);
 }
 
 static rad_status deliver(Handle &h, double *out, int out_on_device, size_t bytes, cudaStream_t s,
@@ -390,15 +548,23 @@ rad_status rad_spectrum(rad_handle *hh, double *out, int out_on_device, void *cu
 {
     rad_status st = check_handle(hh);
     if (st != RAD_OK) return st;
-    return deliver(hh->h, out, out_on_device, (size_t)hh->h.D * hh->h.W * sizeof(double),
+    return deliver(hh->h, out, out_on_device, (size_t)hh->h.R * hh->h.D * hh->h.W * sizeof(double),
                    (cudaStream_t)cuda_stream, launch_spectrum);
+}
+
+rad_status rad_spectrum_total(rad_handle *hh, double *out, int out_on_device, void *cuda_stream)
+{
+    rad_status st = check_handle(hh);
+    if (st != RAD_OK) return st;
+    return deliver(hh->h, out, out_on_device, (size_t)hh->h.D * hh->h.W * sizeof(double),
+                   (cudaStream_t)cuda_stream, launch_spectrum_total);
 }
 
 rad_status rad_amplitude(rad_handle *hh, double *out, int out_on_device, void *cuda_stream)
 {
     rad_status st = check_handle(hh);
     if (st != RAD_OK) return st;
-    return deliver(hh->h, out, out_on_device, (size_t)hh->h.D * hh->h.W * 6 * sizeof(double),
+    return deliver(hh->h, out, out_on_device, (size_t)hh->h.R * hh->h.D * hh->h.W * 6 * sizeof(double),
                    (cudaStream_t)cuda_stream, launch_amplitude);
 }
 
@@ -417,7 +583,7 @@ rad_status rad_reset(rad_handle *hh, void *cuda_stream)
     rad_status st = check_handle(hh);
     if (st != RAD_OK) return st;
     Handle &h = hh->h;
-    RAD_CUDA(&h, cudaMemsetAsync(h.acc_d, 0, (size_t)h.D * h.w_pad * 4 * sizeof(double),
+    RAD_CUDA(&h, cudaMemsetAsync(h.acc_d, 0, (size_t)h.R * h.D * h.w_pad * 4 * sizeof(double),
                                  (cudaStream_t)cuda_stream));
     return RAD_OK;
 }
@@ -452,6 +618,6 @@ const char *rad_status_string(rad_status s)
 
 const char *rad_last_error(const rad_handle *hh) { return hh ? hh->h.err.c_str() : g_create_error.c_str(); }
 
-const char *rad_version(void) { return "rad-b200 0.1 (sm_100a)"; }
+const char *rad_version(void) { return "rad-b200 0.2 (sm_100a)"; }
 
 }  // extern "C"

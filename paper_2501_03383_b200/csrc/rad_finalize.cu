@@ -1,6 +1,8 @@
 // rad_finalize.cu -- a4: |A|^2 and normalisation, amplitude export /
 // import in Cartesian components, and the deterministic reduction of per-chunk partials.
 // All fp64, one thread per (direction, frequency) bin; bandwidth-trivial (<= a few MB).
+// Per-region handles: "row" = region * D + direction runs over R*D rows; the basis of a row is
+// that of direction row mod D.
 #include "rad_internal.h"
 
 namespace rad {
@@ -23,14 +25,14 @@ __global__ void rad_spectrum_kernel(const double *__restrict__ acc, double *__re
 // A_xyz = A1 e1 + A2 e2  ->  out[n][j][3][2]
 __global__ void rad_amplitude_kernel(const double *__restrict__ acc, const DirRec *__restrict__ dirs,
                                      const double *__restrict__ basis, double *__restrict__ out,
-                                     int D, int W, int w_pad)
+                                     int rows, int D, int W, int w_pad)
 {
     const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= (long long)D * W) return;
+    if (b >= (long long)rows * W) return;
     const int d = (int)(b / W), j = (int)(b - (long long)d * W);
     const double2 *a = reinterpret_cast<const double2 *>(acc + ((size_t)d * w_pad + j) * 4);
     const double2 a1 = a[0], a2 = a[1];
-    const double *e = basis + (size_t)d * 6;  // fp64 e1, e2
+    const double *e = basis + (size_t)(d % D) * 6;  // fp64 e1, e2
     double *o = out + (size_t)b * 6;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
@@ -41,12 +43,12 @@ __global__ void rad_amplitude_kernel(const double *__restrict__ acc, const DirRe
 
 // A1 += e1 . amp, A2 += e2 . amp
 __global__ void rad_add_amplitude_kernel(double *__restrict__ acc, const double *__restrict__ basis,
-                                         const double *__restrict__ amp, int D, int W, int w_pad)
+                                         const double *__restrict__ amp, int rows, int D, int W, int w_pad)
 {
     const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= (long long)D * W) return;
+    if (b >= (long long)rows * W) return;
     const int d = (int)(b / W), j = (int)(b - (long long)d * W);
-    const double *e = basis + (size_t)d * 6;
+    const double *e = basis + (size_t)(d % D) * 6;
     const double *in = amp + (size_t)b * 6;
     double r1 = 0, i1 = 0, r2 = 0, i2 = 0;
 #pragma unroll
@@ -60,15 +62,36 @@ __global__ void rad_add_amplitude_kernel(double *__restrict__ acc, const double 
     a[0] += r1; a[1] += i1; a[2] += r2; a[3] += i2;
 }
 
-// deterministic mode: acc[e] += sum over chunks (fixed order) of partial[chunk][e]
+// deterministic mode: acc[region][e] += sum over the region's chunks (fixed order) of
+// partial[chunk][e]; cstart[r] = first chunk of region r (NULL: one region, all chunks)
 __global__ void rad_reduce_partials_kernel(double *__restrict__ acc, const double *__restrict__ partial,
-                                           long long n_elem, int n_chunks)
+                                           long long n_elem, int n_chunks, int R,
+                                           const int *__restrict__ cstart)
 {
-    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= n_elem) return;
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_elem * R) return;
+    const int r = (int)(t / n_elem);
+    const long long e = t - (long long)r * n_elem;
+    const int c0 = cstart ? cstart[r] : 0, c1 = cstart ? cstart[r + 1] : n_chunks;
     double s = 0.0;
-    for (int c = 0; c < n_chunks; ++c) s += partial[(size_t)c * n_elem + e];
-    acc[e] += s;
+    for (int c = c0; c < c1; ++c) s += partial[(size_t)c * n_elem + e];
+    acc[t] += s;
+}
+
+// S_total[n][j] = scale * |sum_r A_r|^2 (amplitudes of the regions add up, then the modulus)
+__global__ void rad_spectrum_total_kernel(const double *__restrict__ acc, double *__restrict__ out,
+                                          int R, int D, int W, int w_pad, double scale)
+{
+    const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= (long long)D * W) return;
+    const int d = (int)(b / W), j = (int)(b - (long long)d * W);
+    double s0 = 0, s1 = 0, s2 = 0, s3 = 0;
+    for (int r = 0; r < R; ++r) {
+        const double2 *a = reinterpret_cast<const double2 *>(acc + (((size_t)r * D + d) * w_pad + j) * 4);
+        const double2 a1 = a[0], a2 = a[1];
+        s0 += a1.x; s1 += a1.y; s2 += a2.x; s3 += a2.y;
+    }
+    out[b] = scale * (s0 * s0 + s1 * s1 + s2 * s2 + s3 * s3);
 }
 
 inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) / t); }
@@ -77,31 +100,42 @@ inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) /
 
 cudaError_t launch_spectrum(const Handle &h, double *out_dev, cudaStream_t s)
 {
-    const long long n = (long long)h.D * h.W;
-    rad_spectrum_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, out_dev, h.D, h.W, h.w_pad, h.scale);
+    const long long n = (long long)h.R * h.D * h.W;
+    rad_spectrum_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, out_dev, h.R * h.D, h.W, h.w_pad, h.scale);
     return cudaGetLastError();
 }
 
 cudaError_t launch_amplitude(const Handle &h, double *out_dev, cudaStream_t s)
 {
-    const long long n = (long long)h.D * h.W;
+    const long long n = (long long)h.R * h.D * h.W;
     rad_amplitude_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, h.dirs_d, h.basis_d, out_dev,
-                                                            h.D, h.W, h.w_pad);
+                                                            h.R * h.D, h.D, h.W, h.w_pad);
     return cudaGetLastError();
 }
 
 cudaError_t launch_add_amplitude(const Handle &h, const double *amp_dev, cudaStream_t s)
 {
-    const long long n = (long long)h.D * h.W;
-    rad_add_amplitude_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, h.basis_d, amp_dev, h.D,
-                                                                h.W, h.w_pad);
+    const long long n = (long long)h.R * h.D * h.W;
+    rad_add_amplitude_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, h.basis_d, amp_dev, h.R * h.D,
+                                                                h.D, h.W, h.w_pad);
     return cudaGetLastError();
 }
 
-cudaError_t launch_reduce_partials(const Handle &h, const double *partial, int n_chunks, cudaStream_t s)
+cudaError_t launch_reduce_partials(const Handle &h, const double *partial, int n_chunks,
+                                   const int *region_chunk_start, cudaStream_t s)
 {
     const long long n = (long long)h.D * h.w_pad * 4;
-    rad_reduce_partials_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, partial, n, n_chunks);
+    const int R = region_chunk_start ? h.R : 1;
+    rad_reduce_partials_kernel<<<blocks_for(n * R, 256), 256, 0, s>>>(h.acc_d, partial, n, n_chunks, R,
+                                                                     region_chunk_start);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_spectrum_total(const Handle &h, double *out_dev, cudaStream_t s)
+{
+    const long long n = (long long)h.D * h.W;
+    rad_spectrum_total_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, out_dev, h.R, h.D, h.W, h.w_pad,
+                                                                 h.scale);
     return cudaGetLastError();
 }
 

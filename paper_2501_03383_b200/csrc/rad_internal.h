@@ -39,11 +39,21 @@ struct DirRec {
 };
 static_assert(sizeof(DirRec) == 96, "DirRec layout");
 
+// One unit of particle work of a per-region call: particles [k0, k0+len) of one region.
+struct ChunkRec {
+    long long k0;
+    int len;
+    int region;
+};
+static_assert(sizeof(ChunkRec) == 16, "ChunkRec layout");
+
 // Everything the accumulate kernels need, passed by value.
 struct AccumParams {
     const void *st[10];    // rx ry rz bx by bz bdx bdy bdz w (DEVICE, float or double)
     long long n_particles;
-    int chunk;             // particles per block (multiple of kBatch)
+    int chunk;             // particles per chunk (multiple of kBatch); chunk c = [c*chunk, ...)
+    int n_chunks;          // a warp task = (warp tile, chunk); n_tasks = n_wtiles * n_chunks
+    const ChunkRec *chunks; // per-region calls: [n_chunks] chunk table (DEVICE), else NULL
     int n_dir, n_omega;    // D, W
     int w_pad;             // W padded to the frequency tile
     int n_ftiles;          // frequency tiles per direction group
@@ -78,11 +88,13 @@ cudaError_t launch_spectrum(const Handle &h, double *out_dev, cudaStream_t s);
 cudaError_t launch_amplitude(const Handle &h, double *out_dev, cudaStream_t s);
 cudaError_t launch_add_amplitude(const Handle &h, const double *amp_dev, cudaStream_t s);
 cudaError_t launch_reduce_partials(const Handle &h, const double *partial, int n_chunks,
-                                   cudaStream_t s);
+                                   const int *region_chunk_start, cudaStream_t s);
+cudaError_t launch_spectrum_total(const Handle &h, double *out_dev, cudaStream_t s);
 
 struct Handle {
     int device = 0;
     int D = 0, W = 0, w_pad = 0;
+    int R = 1;                            // per-region detectors: acc is [R][D][w_pad][4]
     int lw = 32, strip = kStrip;          // lanes along frequency, bins per lane
     int n_ftiles = 0, n_wtiles = 0;
     int stream_nd = 1;
@@ -110,6 +122,14 @@ struct Handle {
     cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr};
     bool consumed_valid[2] = {false, false};
     int stage_next = 0;
+    // per-region calls: chunk table (pinned host copy + device copy), rebuilt when the
+    // caller's offsets or the chunk size change
+    std::vector<long long> reg_offsets;   // offsets of the table currently on the device
+    int reg_chunk = 0, reg_n_chunks = 0;
+    ChunkRec *chunks_h = nullptr, *chunks_d = nullptr;   // [reg_cap]
+    int *reg_cstart_h = nullptr, *reg_cstart_d = nullptr; // [R+1] first chunk of each region
+    size_t reg_cap = 0;
+    cudaEvent_t reg_uploaded = nullptr;
     double *out_d = nullptr;         // scratch for HOST-destination results
     size_t out_bytes = 0;
     int64_t launches = 0;
