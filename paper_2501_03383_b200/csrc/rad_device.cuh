@@ -82,6 +82,35 @@ __device__ __forceinline__ void phase_sincos(uint32_t F, float Ff, float fl, uin
     __sincosf(fmaf(v, kTwoPi, q), &sn, &cs);
 }
 
+// The same exp(i 2 pi f tau) WITHOUT the XU pipe: the reduced phase goes through FMA-pipe
+// polynomials.  t = frac + q/(2 pi) turns; r = t - rint(2t)/2 in [-1/4, 1/4]; sin(2 pi r) and
+// cos(2 pi r) by near-minimax odd/even polynomials (fp32 abs. error 1.9e-7 / 2.9e-7, below
+// MUFU.SIN/COS's ~4e-7); the half-turn parity flips both signs.  27 FMA/ALU-pipe instructions
+// instead of 10 + 2 MUFU: used for a fraction of the bins to take load off the XU pipe, the
+// bound of the general kernel (DESIGN.md section 5.1 "hybrid").
+__device__ __forceinline__ void phase_sincos_poly(uint32_t F, float Ff, float fl, uint32_t T, float ql,
+                                                  float sf, float &sn, float &cs)
+{
+    constexpr float kMagicF = 12582912.0f;  // 1.5 * 2^23
+    const uint32_t u = F * T;
+    const float v = __uint_as_float(0x3f800000u | (u >> 9));  // 1 + frac, in turns
+    const float q = fmaf(fl, sf, Ff * ql);                    // radians
+    const float t = fmaf(q, 0.15915494309189535f, v);         // turns, in [0.5, 2.5]
+    const float kf = fmaf(t, 2.0f, kMagicF);                  // low mantissa bits = rint(2t)
+    const float r = fmaf(kf - kMagicF, -0.5f, t);             // [-1/4, 1/4] turns
+    const uint32_t sign = __float_as_uint(kf) << 31;          // odd half-turn: z -> -z
+    const float r2 = r * r;
+    float ps = fmaf(3.976161437e+01f, r2, -7.658139608e+01f);
+    ps = fmaf(ps, r2, 8.160248510e+01f);
+    ps = fmaf(ps, r2, -4.134168072e+01f);
+    ps = fmaf(ps, r2, 6.283185280e+00f);
+    float pc = fmaf(5.702861988e+01f, r2, -8.533239558e+01f);
+    pc = fmaf(pc, r2, 6.493784751e+01f);
+    pc = fmaf(pc, r2, -1.973920580e+01f);
+    sn = __uint_as_float(__float_as_uint(ps * r) ^ sign);
+    cs = __uint_as_float(__float_as_uint(fmaf(pc, r2, 1.0f)) ^ sign);
+}
+
 template <typename ST>
 __device__ __forceinline__ Particle load_particle(const AccumParams &P, long long k, bool valid)
 {

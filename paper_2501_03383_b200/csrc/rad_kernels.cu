@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
         {  // a1: stage
             const long long k = kb + lane;
             const Particle p = load_particle<ST>(P, k, k < k1);
-#pragma unroll
+#pragma unroll(DPW > 2 ? 1 : DPW)  // 4 or 8 directions per warp: keep the staging code out of the register budget
             for (int dd = 0; dd < DPW; ++dd) {
                 const int dir = min(dg * DPW + dd, P.n_dir - 1);
                 float4 r4;
@@ -181,20 +181,29 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 }
             }
         } else {
-#pragma unroll 2
-            for (int kk = 0; kk < kBatch; ++kk) {  // a2: sweep
+            // a2: sweep.  Hybrid: of every two particles, kPolyEven / kPolyOdd of the S bins take
+            // the FMA-pipe polynomial sincos instead of MUFU.SIN/COS (balances XU against issue).
+            auto sweep_one = [&](const int kk, const int n_poly) {
                 const float4 r4 = rec[kk * DPW + ld];
                 const float sf = sfs[kk * DPW + ld];
                 const uint32_t T = __float_as_uint(r4.x);
 #pragma unroll
                 for (int i = 0; i < S; ++i) {
                     float sn, cs;
-                    phase_sincos(F[i % NC], Ff[i % NC], fl[i % NC], T, r4.y, sf, sn, cs);
+                    if (i >= S - n_poly)
+                        phase_sincos_poly(F[i % NC], Ff[i % NC], fl[i % NC], T, r4.y, sf, sn, cs);
+                    else
+                        phase_sincos(F[i % NC], Ff[i % NC], fl[i % NC], T, r4.y, sf, sn, cs);
                     acc[i][0] = fmaf(r4.z, cs, acc[i][0]);
                     acc[i][1] = fmaf(r4.z, sn, acc[i][1]);
                     acc[i][2] = fmaf(r4.w, cs, acc[i][2]);
                     acc[i][3] = fmaf(r4.w, sn, acc[i][3]);
                 }
+            };
+#pragma unroll 1
+            for (int kk = 0; kk < kBatch; kk += 2) {
+                sweep_one(kk, LW >= kPolyMinLW ? kPolyEven : 0);
+                sweep_one(kk + 1, LW >= kPolyMinLW ? kPolyOdd : 0);
             }
         }
         __syncwarp();
