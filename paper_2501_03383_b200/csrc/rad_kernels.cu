@@ -212,147 +212,12 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
 }
 
 // ------------------------------------------------------------------------------------------
-// a2, packed: the same arithmetic as rad_accum<..., UNI=false> with Blackwell's two-wide fp32
-// instructions (fma/mul/add.rn.f32x2 -> FFMA2/FMUL2/FADD2): the two bins (i, i+1) of a thread
-// share every non-transcendental instruction, so an update costs ~9 issue slots instead of
-// 12.6 while the XU pipe still does its 2 MUFU per update.  Fewer issue slots leave the MUFU
-// queue better fed, and the spare slot pays for centring the reduced phase on 0 (v - 1.5),
-// which halves the fp32 rounding of the MUFU argument.
-typedef unsigned long long u64;
-__device__ __forceinline__ u64 pack2(float lo, float hi)
-{
-    u64 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void unpack2(u64 v, float &lo, float &hi)
-{
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ u64 fma2(u64 a, u64 b, u64 c)
-{
-    u64 d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-__device__ __forceinline__ u64 mul2(u64 a, u64 b)
-{
-    u64 d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ u64 add2(u64 a, u64 b)
-{
-    u64 d;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-
-template <typename ST, int LW, int S, int MINB>
-__global__ void __launch_bounds__(kThreads, MINB) rad_accum_x2(const AccumParams P)
-{
-    static_assert(S % 2 == 0, "bins are processed in pairs");
-    constexpr int DPW = 32 / LW;
-    constexpr int H = S / 2;
-    __shared__ float4 s_rec[kWarpsPerBlock][kBatch * DPW];
-    __shared__ float s_sf[kWarpsPerBlock][kBatch * DPW];
-
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    int wt, ci, region;
-    long long k0, k1;
-    if (!decode_task(P, warp, wt, ci, k0, k1, region)) return;
-    const int dg = wt / P.n_ftiles, ft = wt - dg * P.n_ftiles;
-    const int ld = lane / LW, lf = lane - ld * LW;
-    const int jbase = ft * (LW * S) + lf;
-
-    uint32_t F[S];
-    u64 Ff2[H], fl2[H], a1re[H], a1im[H], a2re[H], a2im[H];
-#pragma unroll
-    for (int i = 0; i < S; ++i) F[i] = __ldg(P.F + jbase + i * LW);
-#pragma unroll
-    for (int h = 0; h < H; ++h) {
-        const int j0 = jbase + 2 * h * LW, j1 = j0 + LW;
-        Ff2[h] = pack2(__ldg(P.Ff + j0), __ldg(P.Ff + j1));
-        fl2[h] = pack2(__ldg(P.fl + j0), __ldg(P.fl + j1));
-        a1re[h] = a1im[h] = a2re[h] = a2im[h] = pack2(0.0f, 0.0f);
-    }
-    const u64 twopi2 = pack2(kTwoPi, kTwoPi), mhalf2 = pack2(-1.5f, -1.5f);
-
-    float4 *rec = s_rec[warp];
-    float *sfs = s_sf[warp];
-
-    for (long long kb = k0; kb < k1; kb += kBatch) {
-        {  // a1: stage
-            const long long k = kb + lane;
-            const Particle p = load_particle<ST>(P, k, k < k1);
-#pragma unroll
-            for (int dd = 0; dd < DPW; ++dd) {
-                const int dir = min(dg * DPW + dd, P.n_dir - 1);
-                float4 r4;
-                float sf;
-                stage_record(p, P.dirs[dir], P.ts32, r4, sf);
-                rec[lane * DPW + dd] = r4;
-                sfs[lane * DPW + dd] = sf;
-            }
-        }
-        __syncwarp();
-#pragma unroll 2
-        for (int kk = 0; kk < kBatch; ++kk) {  // a2: sweep, two bins per instruction
-            const float4 r4 = rec[kk * DPW + ld];
-            const float sf = sfs[kk * DPW + ld];
-            const uint32_t T = __float_as_uint(r4.x);
-            const u64 ql2 = pack2(r4.y, r4.y), sf2 = pack2(sf, sf);
-            const u64 a1 = pack2(r4.z, r4.z), a2 = pack2(r4.w, r4.w);
-#pragma unroll
-            for (int h = 0; h < H; ++h) {
-                const uint32_t u0 = F[2 * h] * T, u1 = F[2 * h + 1] * T;
-                const float v0 = __uint_as_float(0x3f800000u | (u0 >> 9));
-                const float v1 = __uint_as_float(0x3f800000u | (u1 >> 9));
-                const u64 v2 = add2(pack2(v0, v1), mhalf2);  // frac - 1/2 turns, exact
-                const u64 q2 = fma2(fl2[h], sf2, mul2(Ff2[h], ql2));
-                const u64 x2 = fma2(v2, twopi2, q2);
-                float x0, x1, s0, c0, s1, c1;
-                unpack2(x2, x0, x1);
-                __sincosf(x0, &s0, &c0);
-                __sincosf(x1, &s1, &c1);
-                const u64 c2 = pack2(c0, c1), s2 = pack2(s0, s1);
-                a1re[h] = fma2(a1, c2, a1re[h]);
-                a1im[h] = fma2(a1, s2, a1im[h]);
-                a2re[h] = fma2(a2, c2, a2re[h]);
-                a2im[h] = fma2(a2, s2, a2im[h]);
-            }
-        }
-        __syncwarp();
-    }
-    float acc[S][4];
-#pragma unroll
-    for (int h = 0; h < H; ++h) {
-        unpack2(a1re[h], acc[2 * h][0], acc[2 * h + 1][0]);
-        unpack2(a1im[h], acc[2 * h][1], acc[2 * h + 1][1]);
-        unpack2(a2re[h], acc[2 * h][2], acc[2 * h + 1][2]);
-        unpack2(a2im[h], acc[2 * h][3], acc[2 * h + 1][3]);
-    }
-    // the phase was centred by half a turn: exp(i(theta - pi)) = -exp(i theta)
-#pragma unroll
-    for (int i = 0; i < S; ++i) {
-        acc[i][0] = -acc[i][0]; acc[i][1] = -acc[i][1]; acc[i][2] = -acc[i][2]; acc[i][3] = -acc[i][3];
-    }
-    fold<S, LW>(P, acc, dg * DPW + ld, jbase, ci, region);
-}
-
-// ------------------------------------------------------------------------------------------
 // Launch logic.
 template <typename ST, int LW, int S, int MINB, bool UNI>
 static cudaError_t launch_one(const AccumParams &p, cudaStream_t s)
 {
     const long long n_tasks = (long long)p.n_wtiles * p.n_chunks;
     const unsigned grid = (unsigned)((n_tasks + kWarpsPerBlock - 1) / kWarpsPerBlock);
-#ifdef RAD_PACKED  // measured r1: 1943 vs 1981 G updates/s for the scalar kernel on cfg 1 -> off
-    if (!UNI) {
-        rad_accum_x2<ST, LW, S, MINB><<<grid, kThreads, 0, s>>>(p);
-        return cudaGetLastError();
-    }
-#endif
     rad_accum<ST, LW, S, MINB, UNI><<<grid, kThreads, 0, s>>>(p);
     return cudaGetLastError();
 }
