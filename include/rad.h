@@ -103,6 +103,24 @@ RAD_API rad_status rad_accumulate_step(rad_handle *h, int64_t step_index, int64_
                                        const void *bdx, const void *bdy, const void *bdz,
                                        const void *w, void *cuda_stream);
 
+/* n_steps consecutive PIC steps in ONE launch: exactly the result (up to rounding order) of
+ *   for s in 0 .. n_steps-1: rad_accumulate_step(h, first_step_index + s, n_particles,
+ *                                                 rx + s*step_stride, ..., w + s*step_stride)
+ * i.e. each of the 10 DEVICE arrays holds the state of step s at elements
+ * [s*step_stride, s*step_stride + n_particles) (step_stride >= n_particles, in elements).
+ * For trajectories that are resident (replay, or a simulation that buffers a few steps):
+ * the grid covers (step, particle chunk) pairs, so launch latency, ramp and tail of the grid
+ * are paid once per call instead of once per step -- this is what makes small steps (a few
+ * 1e5 updates) run at the rate of large ones.  Not available on per-region handles
+ * (RAD_ERR_UNSUPPORTED).  Few-bin (streaming-kernel) detectors and RAD_FLAG_DETERMINISTIC
+ * handles run it as n_steps launches. */
+RAD_API rad_status rad_accumulate_steps(rad_handle *h, int64_t first_step_index, int32_t n_steps,
+                                        int64_t n_particles, int64_t step_stride,
+                                        const void *rx, const void *ry, const void *rz,
+                                        const void *bx, const void *by, const void *bz,
+                                        const void *bdx, const void *bdy, const void *bdz,
+                                        const void *w, void *cuda_stream);
+
 /* Same, state in HOST memory (pinned memory makes the copies asynchronous).  The
  * library stages the arrays through its own double-buffered device buffer: the
  * host->device copy of one call overlaps the kernels of the previous call.  The host

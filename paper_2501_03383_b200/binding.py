@@ -21,7 +21,7 @@ RAD_F32, RAD_F64 = 0, 1
 RAD_FLAG_DETERMINISTIC, RAD_FLAG_FORCE_GENERAL = 1, 2
 
 ABI_SYMBOLS = (
-    "rad_create", "rad_accumulate_step", "rad_accumulate_step_host",
+    "rad_create", "rad_accumulate_step", "rad_accumulate_steps", "rad_accumulate_step_host",
     "rad_accumulate_step_regions", "rad_accumulate_step_regions_host", "rad_spectrum",
     "rad_spectrum_total", "rad_amplitude", "rad_add_amplitude", "rad_reset", "rad_destroy", "rad_launch_count",
     "rad_kernel_variant", "rad_status_string", "rad_last_error", "rad_version",
@@ -66,6 +66,8 @@ def load(path: Optional[Path] = None) -> ctypes.CDLL:
         f = getattr(lib, name)
         f.restype = ctypes.c_int
         f.argtypes = [vp, i64, i64] + [vp] * 10 + [vp]
+    lib.rad_accumulate_steps.restype = ctypes.c_int
+    lib.rad_accumulate_steps.argtypes = [vp, i64, ctypes.c_int32, i64, i64] + [vp] * 10 + [vp]
     for name in ("rad_accumulate_step_regions", "rad_accumulate_step_regions_host"):
         f = getattr(lib, name)
         f.restype = ctypes.c_int
@@ -126,6 +128,13 @@ def rad_accumulate_step(handle: int, step_index: int, n_particles: int, state_pt
                         stream: int = 0) -> None:
     """state_ptrs: 10 DEVICE pointers (rx ry rz bx by bz bdx bdy bdz w)."""
     _check(load().rad_accumulate_step(handle, step_index, n_particles, *state_ptrs, stream), handle)
+
+
+def rad_accumulate_steps(handle: int, first_step_index: int, n_steps: int, n_particles: int,
+                         step_stride: int, state_ptrs: Sequence[int], stream: int = 0) -> None:
+    """state_ptrs: 10 DEVICE pointers to [n_steps][step_stride] arrays (first n_particles of each row)."""
+    _check(load().rad_accumulate_steps(handle, first_step_index, n_steps, n_particles, step_stride,
+                                       *state_ptrs, stream), handle)
 
 
 def rad_accumulate_step_host(handle: int, step_index: int, n_particles: int,
@@ -231,6 +240,19 @@ class Detector:
     def accumulate_step(self, step_index: int, state) -> None:
         n, ptrs = self._ptrs(state, want_cuda=True)
         rad_accumulate_step(self.handle, step_index, n, ptrs, self._stream())
+
+    def accumulate_steps(self, first_step_index: int, state) -> None:
+        """state: 10 torch CUDA tensors [n_steps, n_particles] (contiguous): all steps in one launch."""
+        import torch
+        if len(state) != 10:
+            raise ValueError("state must be 10 arrays: rx ry rz bx by bz bdx bdy bdz w")
+        shp = tuple(state[0].shape)
+        for a in state:
+            if not (isinstance(a, torch.Tensor) and a.is_cuda and a.dim() == 2 and a.is_contiguous()
+                    and tuple(a.shape) == shp and a.element_size() == self.np_dtype.itemsize):
+                raise ValueError("state tensors must be contiguous CUDA [n_steps, n_particles] of state_dtype")
+        rad_accumulate_steps(self.handle, first_step_index, shp[0], shp[1], shp[1],
+                             [a.data_ptr() for a in state], self._stream())
 
     def accumulate_step_host(self, step_index: int, state) -> None:
         n, ptrs = self._ptrs(state, want_cuda=False)

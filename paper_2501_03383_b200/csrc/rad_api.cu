@@ -113,18 +113,10 @@ int choose_chunk(const Handle &h, long long n)
     return (int)best;
 }
 
-// Per-region calls: (re)build the chunk table for these offsets (shifted so that the first
-// region starts at particle `base` of the device arrays) and upload it on stream s.  Chunks
-// never straddle a region; a region of n_r particles is cut into ceil(n_r / chunk) chunks
-// of equal length (rounded up to whole 32-particle batches).
-rad_status build_chunk_table(Handle &h, const int64_t *off, long long base, int chunk, cudaStream_t s)
+// Pinned + device storage for `need` chunk records (and the R+1 region chunk starts); waits
+// until the previous upload has left the pinned copy.
+rad_status ensure_chunk_capacity(Handle &h, size_t need)
 {
-    bool same = h.reg_chunk == chunk && (int)h.reg_offsets.size() == h.R + 1;
-    for (int r = 0; same && r <= h.R; ++r) same = h.reg_offsets[r] == off[r] - base;
-    if (same) return RAD_OK;
-    size_t need = 0;
-    for (int r = 0; r < h.R; ++r) need += (size_t)((off[r + 1] - off[r] + chunk - 1) / chunk);
-    if (need > (size_t)INT32_MAX) return fail(&h, RAD_ERR_INVALID_ARG, "too many particle chunks");
     if (h.reg_uploaded) RAD_CUDA(&h, cudaEventSynchronize(h.reg_uploaded));  // pinned copy is free again
     else RAD_CUDA(&h, cudaEventCreateWithFlags(&h.reg_uploaded, cudaEventDisableTiming));
     if (need > h.reg_cap || !h.reg_cstart_h) {
@@ -140,10 +132,27 @@ rad_status build_chunk_table(Handle &h, const int64_t *off, long long base, int 
                  cudaMalloc(&h.reg_cstart_d, (h.R + 1) * sizeof(int)) == cudaSuccess;
         if (!ok) {
             cudaGetLastError();
-            return fail(&h, RAD_ERR_ALLOC, "allocation of the region chunk table failed");
+            return fail(&h, RAD_ERR_ALLOC, "allocation of the chunk table failed");
         }
         h.reg_cap = cap;
     }
+    return RAD_OK;
+}
+
+// Per-region calls: (re)build the chunk table for these offsets (shifted so that the first
+// region starts at particle `base` of the device arrays) and upload it on stream s.  Chunks
+// never straddle a region; a region of n_r particles is cut into ceil(n_r / chunk) chunks
+// of equal length (rounded up to whole 32-particle batches).
+rad_status build_chunk_table(Handle &h, const int64_t *off, long long base, int chunk, cudaStream_t s)
+{
+    bool same = h.reg_chunk == chunk && (int)h.reg_offsets.size() == h.R + 1;
+    for (int r = 0; same && r <= h.R; ++r) same = h.reg_offsets[r] == off[r] - base;
+    if (same) return RAD_OK;
+    size_t need = 0;
+    for (int r = 0; r < h.R; ++r) need += (size_t)((off[r + 1] - off[r] + chunk - 1) / chunk);
+    if (need > (size_t)INT32_MAX) return fail(&h, RAD_ERR_INVALID_ARG, "too many particle chunks");
+    rad_status st_cap = ensure_chunk_capacity(h, need);
+    if (st_cap != RAD_OK) return st_cap;
     int n = 0;
     for (int r = 0; r < h.R; ++r) {
         h.reg_cstart_h[r] = n;
@@ -153,7 +162,7 @@ rad_status build_chunk_table(Handle &h, const int64_t *off, long long base, int 
         long long len = (n_r + pieces - 1) / pieces;
         len = (len + kBatch - 1) / kBatch * kBatch;
         for (long long k = 0; k < n_r; k += len)
-            h.chunks_h[n++] = ChunkRec{k0 + k, (int)std::min(len, n_r - k), r};
+            h.chunks_h[n++] = ChunkRec{k0 + k, (int)std::min(len, n_r - k), r, 0, 0};
     }
     h.reg_cstart_h[h.R] = n;
     h.reg_n_chunks = n;
@@ -194,14 +203,45 @@ rad_status check_handle(rad_handle *hh)
 // st: DEVICE arrays.  region_off == NULL: particles [0, n) of the one detector; else n_regions+1
 // HOST offsets into arrays whose element 0 is particle `region_base` of the caller's numbering
 // and n = particles spanned by the regions.
-rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *const st[10], cudaStream_t s,
-                             const int64_t *region_off = nullptr, long long region_base = 0)
+// Multi-step calls: chunk table over (step, particle chunk), all folding into region 0.
+rad_status build_step_table(Handle &h, int n_steps, long long n, long long stride, int chunk, cudaStream_t s)
 {
+    const size_t per_step = (size_t)((n + chunk - 1) / chunk);
+    const size_t need = per_step * (size_t)n_steps;
+    if (need > (size_t)INT32_MAX) return fail(&h, RAD_ERR_INVALID_ARG, "too many particle chunks");
+    rad_status st_cap = ensure_chunk_capacity(h, need);
+    if (st_cap != RAD_OK) return st_cap;
+    h.reg_chunk = 0; h.reg_offsets.clear();  // the cached per-region table (same buffers) is gone
+    int m = 0;
+    for (int t = 0; t < n_steps; ++t)
+        for (long long k = 0; k < n; k += chunk)
+            h.chunks_h[m++] = ChunkRec{(long long)t * stride + k, (int)std::min<long long>(chunk, n - k), 0, t, 0};
+    h.reg_n_chunks = m;
+    RAD_CUDA(&h, cudaMemcpyAsync(h.chunks_d, h.chunks_h, (size_t)m * sizeof(ChunkRec), cudaMemcpyHostToDevice, s));
+    RAD_CUDA(&h, cudaEventRecord(h.reg_uploaded, s));
+    return RAD_OK;
+}
+
+rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *const st[10], cudaStream_t s,
+                             const int64_t *region_off = nullptr, long long region_base = 0,
+                             int n_steps = 1, long long step_stride = 0)
+{
+    if (n_steps > 1 && (h.stream_nb || h.deterministic)) {
+        // few-bin streaming kernel / deterministic workspace: one launch per step
+        const size_t esz = h.state_f64 ? 8 : 4;
+        for (int t = 0; t < n_steps; ++t) {
+            const void *sub[10];
+            for (int i = 0; i < 10; ++i) sub[i] = (const char *)st[i] + (size_t)t * step_stride * esz;
+            rad_status st_ = accumulate_device(h, step + t, n, sub, s);
+            if (st_ != RAD_OK) return st_;
+        }
+        return RAD_OK;
+    }
     AccumParams p{};
     for (int i = 0; i < 10; ++i) p.st[i] = st[i];
     p.n_particles = n;
     // per-region calls: every region rounds its own chunk count up -> leave room for that
-    p.chunk = choose_chunk(h, region_off ? n + (long long)h.R * 64 : n);
+    p.chunk = choose_chunk(h, region_off ? n + (long long)h.R * 64 : n * n_steps);
     if (const char *e = getenv("RAD_CHUNK")) {  // tuning/debug override (particles per block)
         const int c = atoi(e);
         if (c >= kBatch) p.chunk = c / kBatch * kBatch;
@@ -210,6 +250,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.n_ftiles = h.n_ftiles; p.n_wtiles = h.n_wtiles;
     p.dirs = h.dirs_d; p.F = h.F_d; p.Ff = h.Ff_d; p.fl = h.fl_d;
     p.ts32 = (h.t0 + (double)step * h.dt) * h.f_unit * kTwo32;
+    p.dts32 = h.dt * h.f_unit * kTwo32;
     p.dt = (float)h.dt;
     p.acc = h.acc_d;
     p.partial = nullptr;
@@ -221,6 +262,11 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
         n_chunks = h.reg_n_chunks;
         p.chunks = h.chunks_d;
         if (n_chunks == 0) return RAD_OK;
+    } else if (n_steps > 1) {
+        rad_status st_ = build_step_table(h, n_steps, n, step_stride, p.chunk, s);
+        if (st_ != RAD_OK) return st_;
+        n_chunks = h.reg_n_chunks;
+        p.chunks = h.chunks_d;
     }
     p.n_chunks = n_chunks;
     int stream_grid = 0;
@@ -411,6 +457,27 @@ rad_status rad_accumulate_step(rad_handle *hh, int64_t step_index, int64_t n_par
     for (const void *p : arr)
         if (!p) return fail(&h, RAD_ERR_INVALID_ARG, "NULL state array");
     return accumulate_device(h, step_index, n_particles, arr, (cudaStream_t)cuda_stream);
+}
+
+rad_status rad_accumulate_steps(rad_handle *hh, int64_t first_step_index, int32_t n_steps,
+                                int64_t n_particles, int64_t step_stride, const void *rx, const void *ry,
+                                const void *rz, const void *bx, const void *by, const void *bz,
+                                const void *bdx, const void *bdy, const void *bdz, const void *w,
+                                void *cuda_stream)
+{
+    rad_status st = check_handle(hh);
+    if (st != RAD_OK) return st;
+    Handle &h = hh->h;
+    if (h.R > 1) return fail(&h, RAD_ERR_UNSUPPORTED, "rad_accumulate_steps on a per-region handle");
+    if (n_particles < 0 || n_steps < 0) return fail(&h, RAD_ERR_INVALID_ARG, "n_particles / n_steps < 0");
+    if (n_steps > 1 && step_stride < n_particles)
+        return fail(&h, RAD_ERR_INVALID_ARG, "step_stride < n_particles");
+    if (n_particles == 0 || n_steps == 0) return RAD_OK;
+    const void *arr[10] = {rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w};
+    for (const void *p : arr)
+        if (!p) return fail(&h, RAD_ERR_INVALID_ARG, "NULL state array");
+    return accumulate_device(h, first_step_index, n_particles, arr, (cudaStream_t)cuda_stream, nullptr, 0,
+                             n_steps, step_stride);
 }
 
 static rad_status check_regions(Handle &h, int32_t n_regions, const int64_t *off)

@@ -55,13 +55,16 @@ struct DirRec {
 };
 static_assert(sizeof(DirRec) == 96, "DirRec layout");
 
-// One unit of particle work of a per-region call: particles [k0, k0+len) of one region.
+// One unit of particle work of a per-region or multi-step call: particles [k0, k0+len) of one
+// region, at time step (first step of the call) + step.
 struct ChunkRec {
     long long k0;
     int len;
     int region;
+    int step;
+    int pad;
 };
-static_assert(sizeof(ChunkRec) == 16, "ChunkRec layout");
+static_assert(sizeof(ChunkRec) == 24, "ChunkRec layout");
 
 // Everything the accumulate kernels need, passed by value.
 struct AccumParams {
@@ -69,7 +72,7 @@ struct AccumParams {
     long long n_particles;
     int chunk;             // particles per chunk (multiple of kBatch); chunk c = [c*chunk, ...)
     int n_chunks;          // a warp task = (warp tile, chunk); n_tasks = n_wtiles * n_chunks
-    const ChunkRec *chunks; // per-region calls: [n_chunks] chunk table (DEVICE), else NULL
+    const ChunkRec *chunks; // per-region / multi-step calls: [n_chunks] chunk table (DEVICE), else NULL
     int n_dir, n_omega;    // D, W
     int w_pad;             // W padded to the frequency tile
     int n_ftiles;          // frequency tiles per direction group
@@ -79,6 +82,7 @@ struct AccumParams {
     const float *Ff;       // [w_pad] (float)F_j
     const float *fl;       // [w_pad] f_j / f_unit - F_j  in [-0.5, 0.5]
     double ts32;           // (t0 + step dt) f_unit 2^32
+    double dts32;          // dt f_unit 2^32: multi-step calls, chunk time = ts32 + chunk.step * dts32
     float dt;              // quadrature weight
     double *acc;           // [D][w_pad][4]: A1.re A1.im A2.re A2.im (transverse components)
     double *partial;       // deterministic mode: [n_chunks][D][w_pad][4], else NULL

@@ -62,7 +62,7 @@ __device__ __forceinline__ void fold(const AccumParams &P, const float (&acc)[S]
 
 // warp task -> (warp tile, chunk index, particle range, region); false: no task for this warp
 __device__ __forceinline__ bool decode_task(const AccumParams &P, int warp, int &wt, int &ci,
-                                            long long &k0, long long &k1, int &region)
+                                            long long &k0, long long &k1, int &region, double &ts32)
 {
     const long long task = (long long)blockIdx.x * kWarpsPerBlock + warp;
     if (task >= (long long)P.n_wtiles * P.n_chunks) return false;
@@ -71,7 +71,9 @@ __device__ __forceinline__ bool decode_task(const AccumParams &P, int warp, int 
     if (P.chunks) {
         const ChunkRec c = P.chunks[ci];
         k0 = c.k0; k1 = c.k0 + c.len; region = c.region;
+        ts32 = fma((double)c.step, P.dts32, P.ts32);
     } else {
+        ts32 = P.ts32;
         k0 = (long long)ci * P.chunk;
         k1 = min(P.n_particles, k0 + (long long)P.chunk);
         region = 0;
@@ -103,7 +105,8 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int wt, ci, region;
     long long k0, k1;
-    if (!decode_task(P, warp, wt, ci, k0, k1, region)) return;  // whole warp leaves; no block barrier below
+    double ts32;
+    if (!decode_task(P, warp, wt, ci, k0, k1, region, ts32)) return;  // whole warp leaves; no block barrier below
     const int dg = wt / P.n_ftiles, ft = wt - dg * P.n_ftiles;
     const int ld = lane / LW, lf = lane - ld * LW;
     const int jbase = ft * (LW * S) + lf;
@@ -134,7 +137,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 float4 r4;
                 float sf;
                 uint32_t T;
-                stage_record(p, P.dirs[dir], P.ts32, r4, sf, &T);
+                stage_record(p, P.dirs[dir], ts32, r4, sf, &T);
                 rec[lane * DPW + dd] = r4;
                 sfs[lane * DPW + dd] = sf;
                 if (UNI) {
