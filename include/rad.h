@@ -161,9 +161,16 @@ RAD_API rad_status rad_accumulate_step_regions_host(rad_handle *h, int64_t step_
  * leading region dimension: spectrum out[R][n_dir][n_omega], amplitude
  * out/amp[R][n_dir][n_omega][3][2]. */
 
+/* Where a result goes (the `out_on_device` argument of rad_spectrum / rad_spectrum_total /
+ * rad_amplitude). */
+#define RAD_OUT_HOST 0       /* HOST memory; the call returns after the data has arrived          */
+#define RAD_OUT_DEVICE 1     /* DEVICE memory; asynchronous on cuda_stream                          */
+#define RAD_OUT_HOST_ASYNC 2 /* HOST memory (pinned, else the copy blocks); asynchronous: the data
+                                is there once cuda_stream has passed this call (event / sync by
+                                the caller) -- lets the next step's work be queued meanwhile      */
+
 /* out[n_dir][n_omega] (row-major, fp64) = scale * sum_c |A_c|^2.  Non-destructive.
- * out_on_device != 0: `out` is DEVICE memory, call is asynchronous; else HOST and the
- * call returns after the data has arrived. */
+ * out_on_device: RAD_OUT_HOST, RAD_OUT_DEVICE or RAD_OUT_HOST_ASYNC. */
 RAD_API rad_status rad_spectrum(rad_handle *h, double *out, int out_on_device, void *cuda_stream);
 
 /* out[n_dir][n_omega] = scale * sum_c |sum_r A_r,c|^2: the detector of all particles of all

@@ -19,6 +19,7 @@ LIB_PATH = _PKG / "librad.so"
 RAD_OK, RAD_ERR_INVALID_ARG, RAD_ERR_ALLOC, RAD_ERR_CUDA, RAD_ERR_STATE, RAD_ERR_UNSUPPORTED = range(6)
 RAD_F32, RAD_F64 = 0, 1
 RAD_FLAG_DETERMINISTIC, RAD_FLAG_FORCE_GENERAL = 1, 2
+RAD_OUT_HOST, RAD_OUT_DEVICE, RAD_OUT_HOST_ASYNC = 0, 1, 2
 
 ABI_SYMBOLS = (
     "rad_create", "rad_accumulate_step", "rad_accumulate_steps", "rad_accumulate_step_host",
@@ -159,7 +160,8 @@ def rad_accumulate_step_regions_host(handle: int, step_index: int, region_offset
                                                    *state_ptrs, stream), handle)
 
 
-def rad_spectrum(handle: int, out_ptr: int, out_on_device: bool, stream: int = 0) -> None:
+def rad_spectrum(handle: int, out_ptr: int, out_on_device: int, stream: int = 0) -> None:
+    """out_on_device: RAD_OUT_HOST (False), RAD_OUT_DEVICE (True) or RAD_OUT_HOST_ASYNC."""
     _check(load().rad_spectrum(handle, out_ptr, int(out_on_device), stream), handle)
 
 
@@ -272,9 +274,11 @@ class Detector:
         rad_accumulate_step_regions_host(self.handle, step_index, region_offsets, ptrs, self._stream())
 
     def spectrum(self, out=None):
-        """out: optional torch CUDA fp64 tensor [(R,) D, W] (asynchronous); default -> numpy."""
+        """out: optional torch fp64 tensor [(R,) D, W]: CUDA (asynchronous) or pinned CPU
+        (RAD_OUT_HOST_ASYNC: valid once the current stream has passed the call); default -> numpy."""
         if out is not None:
-            rad_spectrum(self.handle, out.data_ptr(), True, self._stream())
+            mode = RAD_OUT_DEVICE if out.is_cuda else RAD_OUT_HOST_ASYNC
+            rad_spectrum(self.handle, out.data_ptr(), mode, self._stream())
             return out
         res = np.empty(self._shape(), dtype=np.float64)
         rad_spectrum(self.handle, res.ctypes.data, False, self._stream())

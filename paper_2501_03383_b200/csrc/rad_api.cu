@@ -597,7 +597,9 @@ static rad_status deliver(Handle &h, double *out, int out_on_device, size_t byte
                           cudaError_t (*launch)(const Handle &, double *, cudaStream_t))
 {
     if (!out) return fail(&h, RAD_ERR_INVALID_ARG, "out is NULL");
-    if (out_on_device) {
+    if (out_on_device < RAD_OUT_HOST || out_on_device > RAD_OUT_HOST_ASYNC)
+        return fail(&h, RAD_ERR_INVALID_ARG, "out_on_device must be RAD_OUT_HOST, RAD_OUT_DEVICE or RAD_OUT_HOST_ASYNC");
+    if (out_on_device == RAD_OUT_DEVICE) {
         RAD_CUDA(&h, launch(h, out, s));
         h.launches += 1;
         return RAD_OK;
@@ -607,7 +609,7 @@ static rad_status deliver(Handle &h, double *out, int out_on_device, size_t byte
     RAD_CUDA(&h, launch(h, h.out_d, s));
     h.launches += 1;
     RAD_CUDA(&h, cudaMemcpyAsync(out, h.out_d, bytes, cudaMemcpyDeviceToHost, s));
-    RAD_CUDA(&h, cudaStreamSynchronize(s));
+    if (out_on_device != RAD_OUT_HOST_ASYNC) RAD_CUDA(&h, cudaStreamSynchronize(s));
     return RAD_OK;
 }
 

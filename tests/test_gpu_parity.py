@@ -336,3 +336,20 @@ def test_accumulate_steps_argument_errors():
     with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, n_regions=3) as det:
         with pytest.raises(binding.RadError, match="UNSUPPORTED"):
             det.accumulate_steps(0, z)
+
+
+def test_spectrum_to_pinned_host_async():
+    """RAD_OUT_HOST_ASYNC: the result is in pinned host memory once the stream has passed the call;
+    invalid destinations are rejected."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    w = wl.make_workload("3c")
+    (t, st), = list(w.steps(n_steps=1, n_particles=500))
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0) as det:
+        det.accumulate_step(t, P.to_device(st))
+        pinned = torch.zeros(w.n_dir, w.n_omega, dtype=torch.float64).pin_memory()
+        det.spectrum(out=pinned)
+        torch.cuda.current_stream().synchronize()
+        assert np.array_equal(pinned.numpy(), det.spectrum())
+        with pytest.raises(binding.RadError, match="INVALID_ARG"):
+            binding.rad_spectrum(det.handle, pinned.data_ptr(), 3, 0)
