@@ -214,13 +214,10 @@ template <typename ST, int NB, int ND>
 cudaError_t launch_stream_t(const AccumParams &p, int grid, cudaStream_t s)
 {
     const size_t smem = (size_t)kSStages * 10 * kSTileBytes;
-    static bool configured = false;  // per template instance
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(rad_accum_stream<ST, NB, ND>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    // per device and per template instance; the call is a cheap host-side set, so no caching
+    cudaError_t e = cudaFuncSetAttribute(rad_accum_stream<ST, NB, ND>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
     int use_bulk = getenv("RAD_STREAM_PLAIN") ? 0 : 1;  // debug: force the plain-load path
     for (int a = 0; a < 10; ++a)
         if (reinterpret_cast<uintptr_t>(p.st[a]) & 15) use_bulk = 0;
