@@ -166,8 +166,9 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": el / max(args.steps, 1) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": {"workload": w.name, "n_particles": n, "n_dir": w.n_dir,
-                                        "n_omega": w.n_omega, "state_dtype": np.dtype(w.state_dtype).name},
+        "data": "synthetic", "config": {"workload": w.name, "n_particles": n, "n_regions": w.n_regions,
+                                        "n_dir": w.n_dir, "n_omega": w.n_omega,
+                                        "state_dtype": np.dtype(w.state_dtype).name},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
