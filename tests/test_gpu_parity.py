@@ -353,3 +353,33 @@ def test_spectrum_to_pinned_host_async():
         assert np.array_equal(pinned.numpy(), det.spectrum())
         with pytest.raises(binding.RadError, match="INVALID_ARG"):
             binding.rad_spectrum(det.handle, pinned.data_ptr(), 3, 0)
+
+
+def test_multi_gpu_plumbing_on_one_device(oracle_mod):
+    """multi.global_spectrum (export A, all-reduce, import into a second handle, |A|^2) is the
+    path bench.py --gpus N takes; with no process group the all-reduce is the identity, so the
+    result must equal the local spectrum, and two 'ranks' emulated by two handles on particle
+    shards must sum to the oracle of all particles."""
+    import torch
+    from paper_2501_03383_b200 import binding, multi
+    w = wl.make_workload("3b")
+    steps = list(w.steps(n_steps=2, n_particles=1500))
+    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    dets = [binding.Detector(w.dirs, w.omega, w.dt, scale=1.0) for _ in range(3)]
+    try:
+        amp = [torch.empty(w.n_dir, w.n_omega, 3, 2, dtype=torch.float64, device="cuda") for _ in range(2)]
+        for r in range(2):
+            b, e = multi.shard_range(1500, r, 2)
+            for t, st in steps:
+                dets[r].accumulate_step(t, P.to_device([a[b:e] for a in st]))
+            dets[r].amplitude(out=amp[r])
+        out = torch.empty(w.n_dir, w.n_omega, dtype=torch.float64, device="cuda")
+        multi.global_spectrum(dets[0], dets[2], amp[0], out=out)      # world size 1: identity
+        torch.cuda.synchronize()
+        assert np.array_equal(out.cpu().numpy(), dets[0].spectrum())
+        dets[2].reset()
+        dets[2].add_amplitude(amp[0] + amp[1])                       # what the all-reduce delivers
+        P.assert_parity(dets[2].spectrum(), ref, what="two shards summed")
+    finally:
+        for d in dets:
+            d.close()
