@@ -376,10 +376,38 @@ def test_multi_gpu_plumbing_on_one_device(oracle_mod):
         out = torch.empty(w.n_dir, w.n_omega, dtype=torch.float64, device="cuda")
         multi.global_spectrum(dets[0], dets[2], amp[0], out=out)      # world size 1: identity
         torch.cuda.synchronize()
-        assert np.array_equal(out.cpu().numpy(), dets[0].spectrum())
+        assert np.allclose(out.cpu().numpy(), dets[0].spectrum(), rtol=1e-12, atol=0)   # xyz round trip
         dets[2].reset()
         dets[2].add_amplitude(amp[0] + amp[1])                       # what the all-reduce delivers
         P.assert_parity(dets[2].spectrum(), ref, what="two shards summed")
     finally:
         for d in dets:
             d.close()
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_relativistic_beam_small_doppler_factor(oracle_mod, dtype):
+    """Degenerate regime of the formula: beta -> 1 along the line of sight, 1 - beta.n down to
+    ~1e-4 (gamma ~ 70), amplitudes spanning (1 - beta.n)^-2 ~ 1e8.  The Doppler factor is formed
+    in fp64 on the GPU, so parity must hold for fp32 and fp64 state alike."""
+    rng = np.random.default_rng(77)
+    n = 2000
+    gamma = 10.0 ** rng.uniform(0.5, 1.85, n)
+    beta = np.sqrt(1.0 - 1.0 / gamma ** 2)
+    th, ph = rng.normal(0, 2.0 / gamma), rng.uniform(0, 2 * np.pi, n)       # cone ~ 1/gamma around +x
+    bx, by, bz = beta * np.cos(th), beta * np.sin(th) * np.cos(ph), beta * np.sin(th) * np.sin(ph)
+    r = rng.uniform(0, 5e-6, (3, n))
+    bd = rng.normal(0, 1e13, (3, n))
+    st = [np.ascontiguousarray(a, dtype=dtype) for a in (r[0], r[1], r[2], bx, by, bz, bd[0], bd[1], bd[2],
+                                                         rng.uniform(0.5, 2.0, n))]
+    assert np.all(st[3].astype(np.float64) ** 2 + st[4].astype(np.float64) ** 2 + st[5].astype(np.float64) ** 2 < 1)
+    dirs = np.array([[1.0, 0.0, 0.0], [0.9999, 0.01, 0.0], [0.99, 0.1, 0.05], [0.0, 1.0, 0.0], [-1.0, 0.0, 0.0]])
+    w = wl.Workload("beam", n, 1, 1e-18, dirs, wl.omega_log(96, 1e15, 1e19), dtype, 0, "khi")
+    steps = [(3, st), (4, st)]
+    S, variant = P.run_gpu(w, steps)
+    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    dmin = (1 - (dirs[0] / np.linalg.norm(dirs[0])) @ np.stack([st[3], st[4], st[5]]).astype(np.float64)).min()
+    l2, mr = P.assert_parity(S, ref, what=f"relativistic beam {np.dtype(dtype).name}")
+    for d in range(len(dirs)):      # every direction on its own scale (forward/backward differ by ~1e14)
+        P.assert_parity(S[d], ref[d], what=f"beam dir {d}")
+    print(f"beam {np.dtype(dtype).name}: min(1-beta.n)={dmin:.2e} relL2={l2:.2e} maxrel={mr:.2e}")
