@@ -303,15 +303,15 @@ def run_ours(args):
     # rad_accumulate_steps: T resident steps in one launch (ramp/tail/launch latency paid once)
     multi_step = None
     T = int(min(16, ring, (2 << 30) // max(bytes_per_step, 1)))
-    if R == 1 and T >= 2 and world == 1:
+    if T >= 2 and world == 1:
         stacked = [torch.stack([dev_states[i][c] for i in range(T)]).contiguous() for c in range(10)]
-        det.accumulate_steps(0, stacked)
+        det.accumulate_steps(0, stacked, region_offsets=off)
         torch.cuda.synchronize()
         m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         reps = max(1, min(10, K // T))
         m0.record()
         for r_ in range(reps):
-            det.accumulate_steps(r_ * T, stacked)
+            det.accumulate_steps(r_ * T, stacked, region_offsets=off)
         m1.record()
         torch.cuda.synchronize()
         ms_ms = m0.elapsed_time(m1) / reps

@@ -111,8 +111,8 @@ RAD_API rad_status rad_accumulate_step(rad_handle *h, int64_t step_index, int64_
  * For trajectories that are resident (replay, or a simulation that buffers a few steps):
  * the grid covers (step, particle chunk) pairs, so launch latency, ramp and tail of the grid
  * are paid once per call instead of once per step -- this is what makes small steps (a few
- * 1e5 updates) run at the rate of large ones.  Not available on per-region handles
- * (RAD_ERR_UNSUPPORTED).  Few-bin (streaming-kernel) detectors and RAD_FLAG_DETERMINISTIC
+ * 1e5 updates) run at the rate of large ones.  Per-region handles: rad_accumulate_steps_regions
+ * (this call returns RAD_ERR_UNSUPPORTED there).  Few-bin (streaming-kernel) detectors and RAD_FLAG_DETERMINISTIC
  * handles run it as n_steps launches. */
 RAD_API rad_status rad_accumulate_steps(rad_handle *h, int64_t first_step_index, int32_t n_steps,
                                         int64_t n_particles, int64_t step_stride,
@@ -120,6 +120,17 @@ RAD_API rad_status rad_accumulate_steps(rad_handle *h, int64_t first_step_index,
                                         const void *bx, const void *by, const void *bz,
                                         const void *bdx, const void *bdy, const void *bdz,
                                         const void *w, void *cuda_stream);
+
+/* The multi-step form of rad_accumulate_step_regions: n_steps consecutive steps, step s of every
+ * array at elements [s*step_stride, ...), the same region_offsets (relative to the start of each
+ * step's row) for all steps; step_stride >= region_offsets[n_regions]. */
+RAD_API rad_status rad_accumulate_steps_regions(rad_handle *h, int64_t first_step_index, int32_t n_steps,
+                                                int64_t step_stride, int32_t n_regions,
+                                                const int64_t *region_offsets,
+                                                const void *rx, const void *ry, const void *rz,
+                                                const void *bx, const void *by, const void *bz,
+                                                const void *bdx, const void *bdy, const void *bdz,
+                                                const void *w, void *cuda_stream);
 
 /* Same, state in HOST memory (pinned memory makes the copies asynchronous).  The
  * library stages the arrays through its own double-buffered device buffer: the

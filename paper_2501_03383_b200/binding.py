@@ -22,7 +22,8 @@ RAD_FLAG_DETERMINISTIC, RAD_FLAG_FORCE_GENERAL = 1, 2
 RAD_OUT_HOST, RAD_OUT_DEVICE, RAD_OUT_HOST_ASYNC = 0, 1, 2
 
 ABI_SYMBOLS = (
-    "rad_create", "rad_accumulate_step", "rad_accumulate_steps", "rad_accumulate_step_host",
+    "rad_create", "rad_accumulate_step", "rad_accumulate_steps", "rad_accumulate_steps_regions",
+    "rad_accumulate_step_host",
     "rad_accumulate_step_regions", "rad_accumulate_step_regions_host", "rad_spectrum",
     "rad_spectrum_total", "rad_amplitude", "rad_add_amplitude", "rad_reset", "rad_destroy", "rad_launch_count",
     "rad_kernel_variant", "rad_status_string", "rad_last_error", "rad_version",
@@ -69,6 +70,8 @@ def load(path: Optional[Path] = None) -> ctypes.CDLL:
         f.argtypes = [vp, i64, i64] + [vp] * 10 + [vp]
     lib.rad_accumulate_steps.restype = ctypes.c_int
     lib.rad_accumulate_steps.argtypes = [vp, i64, ctypes.c_int32, i64, i64] + [vp] * 10 + [vp]
+    lib.rad_accumulate_steps_regions.restype = ctypes.c_int
+    lib.rad_accumulate_steps_regions.argtypes = [vp, i64, ctypes.c_int32, i64, ctypes.c_int32, vp] + [vp] * 10 + [vp]
     for name in ("rad_accumulate_step_regions", "rad_accumulate_step_regions_host"):
         f = getattr(lib, name)
         f.restype = ctypes.c_int
@@ -136,6 +139,14 @@ def rad_accumulate_steps(handle: int, first_step_index: int, n_steps: int, n_par
     """state_ptrs: 10 DEVICE pointers to [n_steps][step_stride] arrays (first n_particles of each row)."""
     _check(load().rad_accumulate_steps(handle, first_step_index, n_steps, n_particles, step_stride,
                                        *state_ptrs, stream), handle)
+
+
+def rad_accumulate_steps_regions(handle: int, first_step_index: int, n_steps: int, step_stride: int,
+                                 region_offsets: np.ndarray, state_ptrs: Sequence[int], stream: int = 0) -> None:
+    """region_offsets: HOST int64 [R+1], the same for every step; state_ptrs: 10 DEVICE pointers."""
+    off = np.ascontiguousarray(region_offsets, dtype=np.int64)
+    _check(load().rad_accumulate_steps_regions(handle, first_step_index, n_steps, step_stride,
+                                               off.shape[0] - 1, off.ctypes.data, *state_ptrs, stream), handle)
 
 
 def rad_accumulate_step_host(handle: int, step_index: int, n_particles: int,
@@ -243,8 +254,9 @@ class Detector:
         n, ptrs = self._ptrs(state, want_cuda=True)
         rad_accumulate_step(self.handle, step_index, n, ptrs, self._stream())
 
-    def accumulate_steps(self, first_step_index: int, state) -> None:
-        """state: 10 torch CUDA tensors [n_steps, n_particles] (contiguous): all steps in one launch."""
+    def accumulate_steps(self, first_step_index: int, state, region_offsets=None) -> None:
+        """state: 10 torch CUDA tensors [n_steps, n_particles] (contiguous): all steps in one launch.
+        region_offsets (per-region handles): HOST int64 [R+1], the same for every step."""
         import torch
         if len(state) != 10:
             raise ValueError("state must be 10 arrays: rx ry rz bx by bz bdx bdy bdz w")
@@ -253,8 +265,14 @@ class Detector:
             if not (isinstance(a, torch.Tensor) and a.is_cuda and a.dim() == 2 and a.is_contiguous()
                     and tuple(a.shape) == shp and a.element_size() == self.np_dtype.itemsize):
                 raise ValueError("state tensors must be contiguous CUDA [n_steps, n_particles] of state_dtype")
-        rad_accumulate_steps(self.handle, first_step_index, shp[0], shp[1], shp[1],
-                             [a.data_ptr() for a in state], self._stream())
+        ptrs = [a.data_ptr() for a in state]
+        if region_offsets is not None:
+            if int(region_offsets[-1]) > shp[1]:
+                raise ValueError("region_offsets[-1] exceeds the row length")
+            rad_accumulate_steps_regions(self.handle, first_step_index, shp[0], shp[1], region_offsets, ptrs,
+                                         self._stream())
+        else:
+            rad_accumulate_steps(self.handle, first_step_index, shp[0], shp[1], shp[1], ptrs, self._stream())
 
     def accumulate_step_host(self, step_index: int, state) -> None:
         n, ptrs = self._ptrs(state, want_cuda=False)

@@ -143,30 +143,36 @@ rad_status ensure_chunk_capacity(Handle &h, size_t need)
 // region starts at particle `base` of the device arrays) and upload it on stream s.  Chunks
 // never straddle a region; a region of n_r particles is cut into ceil(n_r / chunk) chunks
 // of equal length (rounded up to whole 32-particle batches).
-rad_status build_chunk_table(Handle &h, const int64_t *off, long long base, int chunk, cudaStream_t s)
+rad_status build_chunk_table(Handle &h, const int64_t *off, long long base, int chunk, cudaStream_t s,
+                             int n_steps = 1, long long stride = 0)
 {
-    bool same = h.reg_chunk == chunk && (int)h.reg_offsets.size() == h.R + 1;
+    bool same = h.reg_chunk == chunk && (int)h.reg_offsets.size() == h.R + 1 && h.reg_steps == n_steps &&
+                h.reg_stride == stride;
     for (int r = 0; same && r <= h.R; ++r) same = h.reg_offsets[r] == off[r] - base;
     if (same) return RAD_OK;
     size_t need = 0;
     for (int r = 0; r < h.R; ++r) need += (size_t)((off[r + 1] - off[r] + chunk - 1) / chunk);
+    need *= (size_t)n_steps;
     if (need > (size_t)INT32_MAX) return fail(&h, RAD_ERR_INVALID_ARG, "too many particle chunks");
     rad_status st_cap = ensure_chunk_capacity(h, need);
     if (st_cap != RAD_OK) return st_cap;
     int n = 0;
-    for (int r = 0; r < h.R; ++r) {
-        h.reg_cstart_h[r] = n;
-        const long long n_r = off[r + 1] - off[r], k0 = off[r] - base;
-        if (n_r == 0) continue;
-        const long long pieces = (n_r + chunk - 1) / chunk;
-        long long len = (n_r + pieces - 1) / pieces;
-        len = (len + kBatch - 1) / kBatch * kBatch;
-        for (long long k = 0; k < n_r; k += len)
-            h.chunks_h[n++] = ChunkRec{k0 + k, (int)std::min(len, n_r - k), r, 0, 0};
-    }
-    h.reg_cstart_h[h.R] = n;
+    for (int t = 0; t < n_steps; ++t)      // step-major (the region chunk starts serve single-step calls only)
+        for (int r = 0; r < h.R; ++r) {
+            if (t == 0) h.reg_cstart_h[r] = n;
+            const long long n_r = off[r + 1] - off[r], k0 = off[r] - base + (long long)t * stride;
+            if (n_r == 0) continue;
+            const long long pieces = (n_r + chunk - 1) / chunk;
+            long long len = (n_r + pieces - 1) / pieces;
+            len = (len + kBatch - 1) / kBatch * kBatch;
+            for (long long k = 0; k < n_r; k += len)
+                h.chunks_h[n++] = ChunkRec{k0 + k, (int)std::min(len, n_r - k), r, t, 0};
+        }
+    h.reg_cstart_h[h.R] = n_steps == 1 ? n : 0;
     h.reg_n_chunks = n;
     h.reg_chunk = chunk;
+    h.reg_steps = n_steps;
+    h.reg_stride = stride;
     h.reg_offsets.resize(h.R + 1);
     for (int r = 0; r <= h.R; ++r) h.reg_offsets[r] = off[r] - base;
     if (n > 0)
@@ -232,7 +238,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
         for (int t = 0; t < n_steps; ++t) {
             const void *sub[10];
             for (int i = 0; i < 10; ++i) sub[i] = (const char *)st[i] + (size_t)t * step_stride * esz;
-            rad_status st_ = accumulate_device(h, step + t, n, sub, s);
+            rad_status st_ = accumulate_device(h, step + t, n, sub, s, region_off, region_base);
             if (st_ != RAD_OK) return st_;
         }
         return RAD_OK;
@@ -241,7 +247,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     for (int i = 0; i < 10; ++i) p.st[i] = st[i];
     p.n_particles = n;
     // per-region calls: every region rounds its own chunk count up -> leave room for that
-    p.chunk = choose_chunk(h, region_off ? n + (long long)h.R * 64 : n * n_steps);
+    p.chunk = choose_chunk(h, (region_off ? n + (long long)h.R * 64 : n) * n_steps);
     if (const char *e = getenv("RAD_CHUNK")) {  // tuning/debug override (particles per block)
         const int c = atoi(e);
         if (c >= kBatch) p.chunk = c / kBatch * kBatch;
@@ -257,7 +263,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.rot_G = h.rot_G; p.rot_Gf = h.rot_Gf; p.rot_gl = h.rot_gl;
     int n_chunks = (int)((n + p.chunk - 1) / p.chunk);
     if (region_off) {
-        rad_status st_ = build_chunk_table(h, region_off, region_base, p.chunk, s);
+        rad_status st_ = build_chunk_table(h, region_off, region_base, p.chunk, s, n_steps, step_stride);
         if (st_ != RAD_OK) return st_;
         n_chunks = h.reg_n_chunks;
         p.chunks = h.chunks_d;
@@ -478,6 +484,39 @@ rad_status rad_accumulate_steps(rad_handle *hh, int64_t first_step_index, int32_
         if (!p) return fail(&h, RAD_ERR_INVALID_ARG, "NULL state array");
     return accumulate_device(h, first_step_index, n_particles, arr, (cudaStream_t)cuda_stream, nullptr, 0,
                              n_steps, step_stride);
+}
+
+static rad_status check_regions(Handle &h, int32_t n_regions, const int64_t *off);
+
+rad_status rad_accumulate_steps_regions(rad_handle *hh, int64_t first_step_index, int32_t n_steps,
+                                        int64_t step_stride, int32_t n_regions,
+                                        const int64_t *region_offsets, const void *rx, const void *ry,
+                                        const void *rz, const void *bx, const void *by, const void *bz,
+                                        const void *bdx, const void *bdy, const void *bdz, const void *w,
+                                        void *cuda_stream)
+{
+    rad_status st = check_handle(hh);
+    if (st != RAD_OK) return st;
+    Handle &h = hh->h;
+    st = check_regions(h, n_regions, region_offsets);
+    if (st != RAD_OK) return st;
+    if (n_steps < 0) return fail(&h, RAD_ERR_INVALID_ARG, "n_steps < 0");
+    if (n_steps > 1 && step_stride < region_offsets[n_regions])
+        return fail(&h, RAD_ERR_INVALID_ARG, "step_stride < region_offsets[n_regions]");
+    const long long n = region_offsets[n_regions] - region_offsets[0];
+    if (n == 0 || n_steps == 0) return RAD_OK;
+    const void *arr[10] = {rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w};
+    for (const void *p : arr)
+        if (!p) return fail(&h, RAD_ERR_INVALID_ARG, "NULL state array");
+    if (h.R == 1) {  // one region = the plain multi-step call on the sub-range
+        const size_t esz = h.state_f64 ? 8 : 4;
+        const void *sub[10];
+        for (int i = 0; i < 10; ++i) sub[i] = (const char *)arr[i] + (size_t)region_offsets[0] * esz;
+        return accumulate_device(h, first_step_index, n, sub, (cudaStream_t)cuda_stream, nullptr, 0, n_steps,
+                                 step_stride);
+    }
+    return accumulate_device(h, first_step_index, region_offsets[n_regions], arr, (cudaStream_t)cuda_stream,
+                             region_offsets, 0, n_steps, step_stride);
 }
 
 static rad_status check_regions(Handle &h, int32_t n_regions, const int64_t *off)

@@ -145,7 +145,8 @@ struct Handle {
     // per-region calls: chunk table (pinned host copy + device copy), rebuilt when the
     // caller's offsets or the chunk size change
     std::vector<long long> reg_offsets;   // offsets of the table currently on the device
-    int reg_chunk = 0, reg_n_chunks = 0;
+    int reg_chunk = 0, reg_n_chunks = 0, reg_steps = 1;
+    long long reg_stride = 0;
     ChunkRec *chunks_h = nullptr, *chunks_d = nullptr;   // [reg_cap]
     int *reg_cstart_h = nullptr, *reg_cstart_d = nullptr; // [R+1] first chunk of each region
     size_t reg_cap = 0;

@@ -145,3 +145,32 @@ def test_cfg5r_full_particles_sampled_bins(oracle_mod):
         P.assert_parity(S[r][:, js], Sref[r][:, js], peak=S[r].max(), what=f"cfg5r region {r}")
     P.assert_parity(Stot[:, js], o.spectrum_total()[:, js], peak=Stot.max(), what="cfg5r total")
     assert variant == "general"
+
+
+@pytest.mark.parametrize("flags", [0, 1])
+def test_regions_multi_step_one_launch(oracle_mod, flags):
+    """rad_accumulate_steps_regions == the per-step region calls: 4 steps, ragged regions incl.
+    empty ones and an unassigned head/tail, row stride > n (NaN padding must not be read)."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    w = wl.Workload("reg", 2500, 4, 1e-17, wl.dirs_fibonacci(3), wl.omega_log(200), np.float32,
+                    wl.BASE_SEED + 32, "khi")
+    steps = [(50 + t, st) for t, st in w.steps()]
+    off = np.array([40, 700, 700, 1733, 1734, 2490], dtype=np.int64)
+    R = len(off) - 1
+    ref = _oracle(oracle_mod, w, R, off, steps).spectrum()
+    stride = 2500 + 12
+    state = []
+    for c in range(10):
+        a = np.full((4, stride), np.nan, dtype=np.float32)
+        for i, (_, st) in enumerate(steps):
+            a[i, :2500] = st[c]
+        state.append(torch.from_numpy(a).cuda())
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, n_regions=R, flags=flags) as det:
+        l0 = det.launch_count
+        det.accumulate_steps(50, state, region_offsets=off)
+        if flags == 0:
+            assert det.launch_count - l0 == 1
+        _assert_regions(det.spectrum(), ref, "regions multi-step")
+        with pytest.raises(binding.RadError, match="step_stride"):
+            binding.rad_accumulate_steps_regions(det.handle, 0, 2, 100, off, [a.data_ptr() for a in state], 0)
