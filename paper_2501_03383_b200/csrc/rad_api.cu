@@ -281,6 +281,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
         const long long n_tiles = (n + tile - 1) / tile;
         stream_grid = (int)std::min<long long>(n_tiles, (long long)stream_blocks_per_sm(h.stream_nb) * h.sm_count);
         for (int j = 0; j < 16; ++j) { p.sF[j] = h.sF[j]; p.sFf[j] = h.sFf[j]; p.sfl[j] = h.sfl[j]; }
+        p.sdir[0] = h.sdir[0]; p.sdir[1] = h.sdir[1];
         n_chunks = stream_grid;
     }
     if (h.deterministic) {
@@ -386,6 +387,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         r.e2x = (float)e2[0]; r.e2y = (float)e2[1]; r.e2z = (float)e2[2];
         r.pad[0] = r.pad[1] = r.pad[2] = 0.0f;
     }
+    h.sdir[0] = recs[0]; h.sdir[1] = recs[h.D > 1 ? 1 : 0];
     choose_tile(h);
     h.stream_nb = h.R > 1 ? 0 : stream_shape(h.D, h.W, &h.stream_nd);  // per-region: bin-owner kernels only
     // uniform grid?  w_j = w_0 + j dw to fp64 rounding -> rotation-recurrence kernel (a2')

@@ -28,6 +28,15 @@ __device__ __forceinline__ double to_f64(float x)
 #endif
 }
 
+// fp64 -> fp32 as ONE F2F: with -ftz the plain cast also emits a DSETP + select per conversion
+// to flush fp32 subnormals, which these values (|x| >= 1e-30 or exactly 0) never are.
+__device__ __forceinline__ float to_f32(double x)
+{
+    float f;
+    asm("cvt.rn.f32.f64 %0, %1;" : "=f"(f) : "d"(x));
+    return f;
+}
+
 template <typename ST>
 __device__ __forceinline__ ST ld_state(const void *p, long long k)
 {
@@ -50,7 +59,7 @@ __device__ __forceinline__ void stage_record(const Particle &p, const DirRec &dr
     const double res = s32 - (m - kMagic);
     // Doppler factor d = 1 - n.beta in fp64 (no cancellation error for beta -> 1)
     const double d64 = 1.0 - fma(dr.nx, p.bx, fma(dr.ny, p.by, dr.nz * p.bz));
-    const float d = (float)d64;
+    const float d = to_f32(d64);
     // amplitude: n x ((n-beta) x bd) = (n-beta)(n.bd) - bd (1-n.beta); it is _|_ n, so its
     // components on the transverse basis are a_i = -(e_i.beta)(n.bd) - (e_i.bd) d
     const float g = fmaf(dr.nfx, p.bdx, fmaf(dr.nfy, p.bdy, dr.nfz * p.bdz));
@@ -61,10 +70,10 @@ __device__ __forceinline__ void stage_record(const Particle &p, const DirRec &dr
     const float inv = 1.0f / d;
     const float pre = -p.wdt * inv * inv;  // -w dt / d^2
     rec.x = __uint_as_float(T);
-    rec.y = (float)res * kUnitToRad;
+    rec.y = to_f32(res) * kUnitToRad;
     rec.z = pre * fmaf(e1b, g, e1d * d);
     rec.w = pre * fmaf(e2b, g, e2d * d);
-    sf = (float)s32 * kUnitToRad;
+    sf = to_f32(s32) * kUnitToRad;
     if (T_out) *T_out = T;
 }
 

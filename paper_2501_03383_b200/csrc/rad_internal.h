@@ -86,9 +86,11 @@ struct AccumParams {
     float dt;              // quadrature weight
     double *acc;           // [D][w_pad][4]: A1.re A1.im A2.re A2.im (transverse components)
     double *partial;       // deterministic mode: [n_chunks][D][w_pad][4], else NULL
-    // streaming variant only: per-frequency constants in the parameter constant bank
+    // streaming variant only: per-frequency constants and the (<= 2) direction records in the
+    // parameter constant bank (operands come straight from c[0][..]: no loads, no registers)
     uint32_t sF[16];
     float sFf[16], sfl[16];
+    DirRec sdir[2];
     // uniform-grid variant only: LW*(f_1 - f_0)/f_unit = rot_G + rot_gl (integer + fraction)
     uint32_t rot_G;
     float rot_Gf, rot_gl;
@@ -128,6 +130,7 @@ struct Handle {
     std::vector<double> omega_h;
     uint32_t sF[16] = {0};           // streaming shapes: first 16 frequency constants (host copy)
     float sFf[16] = {0}, sfl[16] = {0};
+    DirRec sdir[2] = {};             // streaming shapes: the direction records (host copy)
     DirRec *dirs_d = nullptr;
     double *basis_d = nullptr;       // [D][6] fp64 e1, e2 (amplitude export/import)
     uint32_t *F_d = nullptr;

@@ -166,7 +166,7 @@ __global__ void __launch_bounds__(kSThreads, NB <= 8 ? RAD_S_MINB : 1) rad_accum
             for (int d = 0; d < ND; ++d) {
                 float4 r4;
                 float sf;
-                stage_record(p, P.dirs[min(d, P.n_dir - 1)], P.ts32, r4, sf);  // a1
+                stage_record(p, P.sdir[d], P.ts32, r4, sf);  // a1 (direction record: constant bank)
 #pragma unroll
                 for (int j = 0; j < WB; ++j) {  // a2
                     const int b = d * WB + j;
