@@ -44,6 +44,8 @@ def _load():
              ctypes.c_double, ctypes.c_double, ctypes.c_longlong, ctypes.c_longlong, ctypes.c_int]
             + [ctypes.c_void_p] * 10
             + [ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p])
+        lib.oracle_accumulate_step_w.restype = ctypes.c_int
+        lib.oracle_accumulate_step_w.argtypes = lib.oracle_accumulate_step.argtypes + [ctypes.c_int, ctypes.c_void_p]
         lib.oracle_accumulate_step_regions.restype = ctypes.c_int
         lib.oracle_accumulate_step_regions.argtypes = (
             [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p,
@@ -51,6 +53,9 @@ def _load():
              ctypes.c_void_p, ctypes.c_int]
             + [ctypes.c_void_p] * 10
             + [ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p])
+        lib.oracle_accumulate_step_regions_w.restype = ctypes.c_int
+        lib.oracle_accumulate_step_regions_w.argtypes = (lib.oracle_accumulate_step_regions.argtypes
+                                                         + [ctypes.c_int, ctypes.c_void_p])
         lib.oracle_spectrum.restype = ctypes.c_int
         lib.oracle_spectrum.argtypes = [ctypes.c_longlong, ctypes.c_void_p, ctypes.c_double,
                                         ctypes.c_void_p]
@@ -66,6 +71,17 @@ def num_threads() -> int:
     return int(_load().oracle_num_threads())
 
 
+WINDOW_TYPES = {"none": 0, "triangle": 1, "hamming": 2}
+
+
+def _window_args(window):
+    """window = None or (type name, origin[3], extent[3]) -> (type code, fp64 array of 6 or None)."""
+    if window is None:
+        return 0, None
+    name, origin, extent = window
+    return WINDOW_TYPES[name], np.ascontiguousarray(list(origin) + list(extent), dtype=np.float64)
+
+
 class Oracle:
     """Same call sequence as the C ABI (create / accumulate_step / spectrum / amplitude).
 
@@ -73,13 +89,14 @@ class Oracle:
     dir*W + j) restricts the computation to a subset of bins; other bins stay zero.
     """
 
-    def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, bins=None):
+    def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, bins=None, window=None):
         self.dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
         self.omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
         self.dt, self.t0, self.scale = float(dt), float(t0), float(scale)
         self.D, self.W = self.dirs.shape[0], self.omega.shape[0]
         self.bins = None if bins is None else np.ascontiguousarray(bins, dtype=np.int64)
         self.A = np.zeros((self.D, self.W, 3, 2), dtype=np.float64)
+        self.win_type, self.win = _window_args(window)
 
     def reset(self):
         self.A[...] = 0.0
@@ -95,10 +112,11 @@ class Oracle:
             raise ValueError("state arrays must be 1-D and of equal length")
         nb = 0 if self.bins is None else self.bins.shape[0]
         bp = None if self.bins is None else self.bins.ctypes.data
-        rc = _load().oracle_accumulate_step(
+        rc = _load().oracle_accumulate_step_w(
             self.D, self.dirs.ctypes.data, self.W, self.omega.ctypes.data, self.dt, self.t0,
             int(step_index), n, int(dt0 == np.dtype(np.float32)),
-            *[a.ctypes.data for a in arrs], nb, bp, self.A.ctypes.data)
+            *[a.ctypes.data for a in arrs], nb, bp, self.A.ctypes.data,
+            self.win_type, None if self.win is None else self.win.ctypes.data)
         if rc != 0:
             raise ValueError("oracle_accumulate_step: bad argument")
 
@@ -119,7 +137,8 @@ class RegionOracle:
     only.  Particles are sorted by region; ``offsets`` [R+1] (non-decreasing) are passed with
     every step.  Same (optional) bin subset in every region."""
 
-    def __init__(self, n_regions, dirs, omega, dt, t0=0.0, scale=0.0, bins=None):
+    def __init__(self, n_regions, dirs, omega, dt, t0=0.0, scale=0.0, bins=None, window=None):
+        self.win_type, self.win = _window_args(window)
         self.dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
         self.omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
         self.dt, self.t0, self.scale = float(dt), float(t0), float(scale)
@@ -144,10 +163,11 @@ class RegionOracle:
             raise ValueError("state arrays must be 1-D, of equal length >= offsets[-1]")
         nb = 0 if self.bins is None else self.bins.shape[0]
         bp = None if self.bins is None else self.bins.ctypes.data
-        rc = _load().oracle_accumulate_step_regions(
+        rc = _load().oracle_accumulate_step_regions_w(
             self.D, self.dirs.ctypes.data, self.W, self.omega.ctypes.data, self.dt, self.t0,
             int(step_index), self.R, offsets.ctypes.data, int(dt0 == np.dtype(np.float32)),
-            *[a.ctypes.data for a in arrs], nb, bp, self.A.ctypes.data)
+            *[a.ctypes.data for a in arrs], nb, bp, self.A.ctypes.data,
+            self.win_type, None if self.win is None else self.win.ctypes.data)
         if rc != 0:
             raise ValueError("oracle_accumulate_step_regions: bad argument")
 

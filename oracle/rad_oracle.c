@@ -42,6 +42,14 @@
  * oracle_accumulate_step_regions() is the same sum restricted to the particles of each
  * region, A_r = sum over k in region r; pins: sum_r A_r = A of all particles, an empty
  * region is exactly zero, regions are independent, masked numpy brute force.
+ *
+ * Spatial window (reading W1 of DESIGN.md; not in the paper, which
+ * only cites the plugin [37]): the macro weight of a particle is multiplied by
+ *   Wn(r) = prod over axes c with extent L_c > 0 of w1((r_c - o_c)/L_c),
+ *   w1(u) = 0 outside [0,1];  TRIANGLE: 1 - |2u - 1|;  HAMMING: 0.54 - 0.46 cos(2 pi u)
+ * evaluated at the particle's position of that step.  Pins: type NONE and all-zero extents
+ * change nothing; closed-form window values times the Dirichlet kernel; outside -> exactly 0;
+ * equals the unwindowed oracle fed w*Wn(r) computed independently in numpy.
  */
 #include <math.h>
 #include <stddef.h>
@@ -79,6 +87,15 @@ static void cross3(const double a[3], const double b[3], double out[3])
     out[2] = a[0] * b[1] - a[1] * b[0];
 }
 
+/* w1(u) of the spatial window, see the header. */
+static double window_1d(int type, double u)
+{
+    if (u < 0.0 || u > 1.0) return 0.0;
+    if (type == 1) return 1.0 - fabs(2.0 * u - 1.0);
+    if (type == 2) return 0.54 - 0.46 * cos(2.0 * 3.14159265358979323846 * u);
+    return 1.0;
+}
+
 /*
  * Accumulate one PIC step into A.
  *   dirs   [n_dir][3]   fp64, any non-zero length (normalised here, Q8)
@@ -89,14 +106,17 @@ static void cross3(const double a[3], const double b[3], double out[3])
  *          NULL -> all bins.  Bins are independent sums, so a subset is exact.
  *   A      [n_dir][n_omega][3][2] (re, im) fp64, accumulated in place (only the
  *          selected bins are touched)
+ *   win_type 0 none / 1 triangle / 2 Hamming; win = {o_x, o_y, o_z, L_x, L_y, L_z} (NULL or
+ *          type 0: no window; L_c <= 0: axis c not windowed)
  * Returns 0, or 1 on a bad argument.
  */
-int oracle_accumulate_step(int n_dir, const double *dirs, int n_omega, const double *omega,
-                           double dt, double t0, long long step_index, long long n_part,
-                           int is_f32, const void *rx, const void *ry, const void *rz,
-                           const void *bx, const void *by, const void *bz, const void *bdx,
-                           const void *bdy, const void *bdz, const void *w,
-                           long long n_bins, const long long *bin_idx, double *A)
+int oracle_accumulate_step_w(int n_dir, const double *dirs, int n_omega, const double *omega,
+                             double dt, double t0, long long step_index, long long n_part,
+                             int is_f32, const void *rx, const void *ry, const void *rz,
+                             const void *bx, const void *by, const void *bz, const void *bdx,
+                             const void *bdy, const void *bdz, const void *w,
+                             long long n_bins, const long long *bin_idx, double *A,
+                             int win_type, const double *win)
 {
     if (n_dir <= 0 || n_omega <= 0 || !dirs || !omega || !A || n_part < 0) return 1;
     const long long total = bin_idx ? n_bins : (long long)n_dir * n_omega;
@@ -118,7 +138,10 @@ int oracle_accumulate_step(int n_dir, const double *dirs, int n_omega, const dou
             const double r[3] = {LOAD(rx, k), LOAD(ry, k), LOAD(rz, k)};
             const double be[3] = {LOAD(bx, k), LOAD(by, k), LOAD(bz, k)};
             const double bd[3] = {LOAD(bdx, k), LOAD(bdy, k), LOAD(bdz, k)};
-            const double wk = LOAD(w, k);
+            double wk = LOAD(w, k);
+            if (win_type != 0 && win)
+                for (int c = 0; c < 3; ++c)
+                    if (win[3 + c] > 0.0) wk *= window_1d(win_type, (r[c] - win[c]) / win[3 + c]);
             const double d = 1.0 - (be[0] * n[0] + be[1] * n[1] + be[2] * n[2]);
             const double nmb[3] = {n[0] - be[0], n[1] - be[1], n[2] - be[2]};
             double inner[3], outer[3];
@@ -141,6 +164,18 @@ int oracle_accumulate_step(int n_dir, const double *dirs, int n_omega, const dou
     return 0;
 }
 
+/* The plain detector: no window. */
+int oracle_accumulate_step(int n_dir, const double *dirs, int n_omega, const double *omega,
+                           double dt, double t0, long long step_index, long long n_part,
+                           int is_f32, const void *rx, const void *ry, const void *rz,
+                           const void *bx, const void *by, const void *bz, const void *bdx,
+                           const void *bdy, const void *bdz, const void *w,
+                           long long n_bins, const long long *bin_idx, double *A)
+{
+    return oracle_accumulate_step_w(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_part, is_f32, rx, ry,
+                                    rz, bx, by, bz, bdx, bdy, bdz, w, n_bins, bin_idx, A, 0, NULL);
+}
+
 /*
  * Per-region detectors: particles are sorted by region, region r owns the particles
  * [offsets[r], offsets[r+1]) (offsets non-decreasing, n_regions+1 entries), and
@@ -149,13 +184,13 @@ int oracle_accumulate_step(int n_dir, const double *dirs, int n_omega, const dou
  * every region.  Written as the definition: one plain oracle_accumulate_step per region
  * on that region's slice of the state arrays.
  */
-int oracle_accumulate_step_regions(int n_dir, const double *dirs, int n_omega, const double *omega,
-                                   double dt, double t0, long long step_index, long long n_regions,
-                                   const long long *offsets, int is_f32, const void *rx,
-                                   const void *ry, const void *rz, const void *bx, const void *by,
-                                   const void *bz, const void *bdx, const void *bdy,
-                                   const void *bdz, const void *w, long long n_bins,
-                                   const long long *bin_idx, double *A)
+int oracle_accumulate_step_regions_w(int n_dir, const double *dirs, int n_omega, const double *omega,
+                                     double dt, double t0, long long step_index, long long n_regions,
+                                     const long long *offsets, int is_f32, const void *rx,
+                                     const void *ry, const void *rz, const void *bx, const void *by,
+                                     const void *bz, const void *bdx, const void *bdy,
+                                     const void *bdz, const void *w, long long n_bins,
+                                     const long long *bin_idx, double *A, int win_type, const double *win)
 {
     if (n_regions <= 0 || !offsets || offsets[0] < 0) return 1;
     for (long long r = 0; r < n_regions; ++r)
@@ -165,14 +200,27 @@ int oracle_accumulate_step_regions(int n_dir, const double *dirs, int n_omega, c
     for (long long r = 0; r < n_regions; ++r) {
         const long long k0 = offsets[r], n_r = offsets[r + 1] - offsets[r];
         double *A_r = A + (size_t)r * n_dir * n_omega * 6;
-        const int rc = oracle_accumulate_step(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_r,
-                                              is_f32, AT(rx, k0), AT(ry, k0), AT(rz, k0), AT(bx, k0),
-                                              AT(by, k0), AT(bz, k0), AT(bdx, k0), AT(bdy, k0),
-                                              AT(bdz, k0), AT(w, k0), n_bins, bin_idx, A_r);
+        const int rc = oracle_accumulate_step_w(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_r,
+                                                is_f32, AT(rx, k0), AT(ry, k0), AT(rz, k0), AT(bx, k0),
+                                                AT(by, k0), AT(bz, k0), AT(bdx, k0), AT(bdy, k0),
+                                                AT(bdz, k0), AT(w, k0), n_bins, bin_idx, A_r, win_type, win);
         if (rc != 0) return rc;
     }
 #undef AT
     return 0;
+}
+
+int oracle_accumulate_step_regions(int n_dir, const double *dirs, int n_omega, const double *omega,
+                                   double dt, double t0, long long step_index, long long n_regions,
+                                   const long long *offsets, int is_f32, const void *rx,
+                                   const void *ry, const void *rz, const void *bx, const void *by,
+                                   const void *bz, const void *bdx, const void *bdy,
+                                   const void *bdz, const void *w, long long n_bins,
+                                   const long long *bin_idx, double *A)
+{
+    return oracle_accumulate_step_regions_w(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_regions, offsets,
+                                            is_f32, rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w, n_bins, bin_idx, A,
+                                            0, NULL);
 }
 
 /* S[n][j] = scale * sum_c |A_c|^2 ; scale == 0 -> SI default (Q4). */

@@ -402,3 +402,71 @@ def test_p11_regions_bin_subset_and_f32(oracle_mod):
     for t, st in steps64:
         f64.accumulate_step(t, off, *st)
     assert np.array_equal(f64.A, full.A)
+
+
+# ------------------------------------------------- P12 spatial window (NEXT-3, reading W1)
+def _win_np(kind, u):
+    inside = (u >= 0.0) & (u <= 1.0)
+    val = 1.0 - np.abs(2.0 * u - 1.0) if kind == "triangle" else 0.54 - 0.46 * np.cos(2.0 * np.pi * u)
+    return np.where(inside, val, 0.0)
+
+
+@pytest.mark.parametrize("kind,u,expect", [("triangle", 0.25, 0.5), ("triangle", 0.5, 1.0), ("triangle", 0.9, 0.2),
+                                            ("hamming", 0.5, 1.0), ("hamming", 0.25, 0.54), ("hamming", 0.0, 0.08),
+                                            ("triangle", 1.0000001, 0.0), ("hamming", -1e-9, 0.0)])
+def test_p12_window_value_scales_the_dirichlet_kernel(oracle_mod, kind, u, expect):
+    """Static particle (pin P2) inside a box window along x only: |A|^2 = W(u)^2 x the Dirichlet
+    kernel; w1 has the textbook values (triangle 1-|2u-1|, Hamming 0.54-0.46 cos 2 pi u), and a
+    particle outside the box contributes exactly nothing."""
+    L, o = 4e-6, -1e-6
+    r0 = (o + u * L, 7e-7, -3e-7)
+    b = np.array([1.0e13, -2.0e13, 0.5e13])
+    T = 9
+    steps = [(t, _const_state(r0, (0, 0, 0), b, w=1.7)) for t in range(T)]
+    win = (kind, (o, 0.0, 0.0), (L, 0.0, -1.0))            # y, z: extent <= 0 -> not windowed
+    ow = oracle_mod.Oracle(DIRS, OMEGA, DT, scale=1.0, window=win)
+    for t, st in steps:
+        ow.accumulate_step(t, *st)
+    S0 = _run(oracle_mod, DIRS, OMEGA, DT, steps).spectrum()
+    if expect == 0.0:
+        assert np.all(ow.A == 0.0)
+    else:
+        assert np.allclose(ow.spectrum(), expect ** 2 * S0, rtol=1e-9 if u != 0.0 else 1e-6)
+        n = UNIT[2]
+        x = OMEGA * DT / 2
+        closed = (1.7 * expect) ** 2 * (b @ b - (n @ b) ** 2) * DT ** 2 * (np.sin(T * x) / np.sin(x)) ** 2
+        assert np.allclose(ow.spectrum()[2], closed, rtol=1e-8)
+
+
+def test_p12_window_equals_reweighting_and_none_is_identity(oracle_mod):
+    """Windowed oracle == plain oracle fed w * W(r) computed here in numpy (product over the
+    windowed axes, positions of each step); type none / zero extents are the identity."""
+    rng = np.random.default_rng(12)
+    steps = _random_steps(rng, 40, 3)
+    o, L = np.array([-2e-6, -1e-6, -4e-6]), np.array([5e-6, 3e-6, 0.0])   # some particles fall outside
+    for kind in ("triangle", "hamming"):
+        ow = oracle_mod.Oracle(DIRS, OMEGA, DT, scale=1.0, window=(kind, o, L))
+        steps_rw = []
+        for t, st in steps:
+            ow.accumulate_step(t, *st)
+            W = np.ones(40)
+            for c in range(2):
+                W = W * _win_np(kind, (st[c] - o[c]) / L[c])
+            steps_rw.append((t, st[:9] + [st[9] * W]))
+        ref = _run(oracle_mod, DIRS, OMEGA, DT, steps_rw)
+        assert np.allclose(ow.A, ref.A, rtol=0, atol=1e-13 * np.abs(ref.A).max())
+        assert 0 < np.count_nonzero(_win_np(kind, (steps[0][1][0] - o[0]) / L[0]) == 0.0) < 40
+    plain = _run(oracle_mod, DIRS, OMEGA, DT, steps)
+    for win in (("none", o, L), ("triangle", o, np.zeros(3))):
+        ow = oracle_mod.Oracle(DIRS, OMEGA, DT, scale=1.0, window=win)
+        for t, st in steps:
+            ow.accumulate_step(t, *st)
+        assert np.array_equal(ow.A, plain.A)
+    # per-region oracle takes the same window
+    off = np.array([0, 15, 40], dtype=np.int64)
+    ro = oracle_mod.RegionOracle(2, DIRS, OMEGA, DT, scale=1.0, window=("hamming", o, L))
+    ow = oracle_mod.Oracle(DIRS, OMEGA, DT, scale=1.0, window=("hamming", o, L))
+    for t, st in steps:
+        ro.accumulate_step(t, off, *st)
+        ow.accumulate_step(t, *st)
+    assert np.allclose(ro.A.sum(0), ow.A, rtol=0, atol=1e-13 * np.abs(ow.A).max())
