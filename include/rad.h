@@ -85,8 +85,21 @@ typedef struct {
     int32_t state_dtype;   /* rad_dtype of the 10 particle arrays                          */
     uint32_t flags;        /* RAD_FLAG_*                                                   */
     int32_t n_regions;     /* 0 or 1: one detector; R > 1: R per-region detectors          */
-    int32_t reserved;      /* must be 0                                                    */
+    int32_t window_type;   /* RAD_WINDOW_*: spatial window on the macro weights (below)    */
+    double window_origin[3]; /* m: lower corner o of the window box                        */
+    double window_extent[3]; /* m: edge lengths L; L_c <= 0: axis c is not windowed        */
 } rad_config;
+
+/* Spatial window (not in the paper, which cites the plugin [37] for such details; reading W1 of
+ * DESIGN.md): with window_type != RAD_WINDOW_NONE the macro weight of every particle is
+ * multiplied, at every step, by
+ *     Wn(r) = product over the axes c with L_c > 0 of w1((r_c - o_c) / L_c),
+ *     w1(u) = 0 for u outside [0, 1];  TRIANGLE: 1 - |2u - 1|;  HAMMING: 0.54 - 0.46 cos(2 pi u),
+ * which tapers the contribution of particles near the faces of the box (particles entering
+ * or leaving a finite simulation volume otherwise ring in the spectrum). */
+#define RAD_WINDOW_NONE 0
+#define RAD_WINDOW_TRIANGLE 1
+#define RAD_WINDOW_HAMMING 2
 
 /* Create a detector: copies dirs/omega, builds the device tables, zeroes A.
  * *out is set to NULL on failure. */

@@ -20,6 +20,8 @@ RAD_OK, RAD_ERR_INVALID_ARG, RAD_ERR_ALLOC, RAD_ERR_CUDA, RAD_ERR_STATE, RAD_ERR
 RAD_F32, RAD_F64 = 0, 1
 RAD_FLAG_DETERMINISTIC, RAD_FLAG_FORCE_GENERAL = 1, 2
 RAD_OUT_HOST, RAD_OUT_DEVICE, RAD_OUT_HOST_ASYNC = 0, 1, 2
+RAD_WINDOW_NONE, RAD_WINDOW_TRIANGLE, RAD_WINDOW_HAMMING = 0, 1, 2
+WINDOW_TYPES = {"none": RAD_WINDOW_NONE, "triangle": RAD_WINDOW_TRIANGLE, "hamming": RAD_WINDOW_HAMMING}
 
 ABI_SYMBOLS = (
     "rad_create", "rad_accumulate_step", "rad_accumulate_steps", "rad_accumulate_steps_regions",
@@ -37,7 +39,8 @@ class rad_config(ctypes.Structure):
         ("dirs", ctypes.c_void_p), ("omega", ctypes.c_void_p),
         ("dt", ctypes.c_double), ("t0", ctypes.c_double), ("scale", ctypes.c_double),
         ("state_dtype", ctypes.c_int32), ("flags", ctypes.c_uint32),
-        ("n_regions", ctypes.c_int32), ("reserved", ctypes.c_int32),
+        ("n_regions", ctypes.c_int32), ("window_type", ctypes.c_int32),
+        ("window_origin", ctypes.c_double * 3), ("window_extent", ctypes.c_double * 3),
     ]
 
 
@@ -116,13 +119,20 @@ def _check(status: int, handle) -> None:
 
 # ------------------------------------------------------------------ ABI-named functions
 def rad_create(dirs, omega, dt: float, t0: float = 0.0, scale: float = 0.0,
-               state_dtype: int = RAD_F32, flags: int = 0, device: int = 0, n_regions: int = 0) -> int:
-    """-> opaque handle (int).  dirs [D,3], omega [W]: HOST fp64 (copied by the library)."""
+               state_dtype: int = RAD_F32, flags: int = 0, device: int = 0, n_regions: int = 0,
+               window=None) -> int:
+    """-> opaque handle (int).  dirs [D,3], omega [W]: HOST fp64 (copied by the library).
+    window: None or (type name | code, origin[3], extent[3])."""
     dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
     omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
     cfg = rad_config(ctypes.sizeof(rad_config), device, dirs.shape[0], omega.shape[0],
                      dirs.ctypes.data, omega.ctypes.data, dt, t0, scale, state_dtype, flags,
                      n_regions, 0)
+    if window is not None:
+        kind, origin, extent = window
+        cfg.window_type = WINDOW_TYPES[kind] if isinstance(kind, str) else int(kind)
+        cfg.window_origin = (ctypes.c_double * 3)(*[float(x) for x in origin])
+        cfg.window_extent = (ctypes.c_double * 3)(*[float(x) for x in extent])
     h = ctypes.c_void_p()
     _check(load().rad_create(ctypes.byref(cfg), ctypes.byref(h)), None)
     return h.value
@@ -210,14 +220,14 @@ class Detector:
     pinned torch CPU tensors (host path, copies inside the library)."""
 
     def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, state_dtype=np.float32, flags=0, device=0,
-                 n_regions=0):
+                 n_regions=0, window=None):
         self.D = int(np.asarray(dirs).reshape(-1, 3).shape[0])
         self.W = int(np.asarray(omega).reshape(-1).shape[0])
         self.R = max(1, int(n_regions))
         self.np_dtype = np.dtype(state_dtype)
         code = {np.dtype(np.float32): RAD_F32, np.dtype(np.float64): RAD_F64}[self.np_dtype]
         self.device = device
-        self.handle = rad_create(dirs, omega, dt, t0, scale, code, flags, device, n_regions)
+        self.handle = rad_create(dirs, omega, dt, t0, scale, code, flags, device, n_regions, window)
 
     def _shape(self, *tail):
         return ((self.R,) if self.R > 1 else ()) + (self.D, self.W) + tail

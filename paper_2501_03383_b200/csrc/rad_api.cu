@@ -257,6 +257,8 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.dirs = h.dirs_d; p.F = h.F_d; p.Ff = h.Ff_d; p.fl = h.fl_d;
     p.ts32 = (h.t0 + (double)step * h.dt) * h.f_unit * kTwo32;
     p.dts32 = h.dt * h.f_unit * kTwo32;
+    p.win_type = h.win_type;
+    for (int c = 0; c < 3; ++c) { p.win_o[c] = h.win_o[c]; p.win_il[c] = h.win_il[c]; }
     p.dt = (float)h.dt;
     p.acc = h.acc_d;
     p.partial = nullptr;
@@ -334,8 +336,13 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         return fail(nullptr, RAD_ERR_INVALID_ARG, "state_dtype must be RAD_F32 or RAD_F64");
     if (cfg->flags & ~(RAD_FLAG_DETERMINISTIC | RAD_FLAG_FORCE_GENERAL))
         return fail(nullptr, RAD_ERR_INVALID_ARG, "unknown flag bits");
-    if (cfg->n_regions < 0 || cfg->reserved != 0)
-        return fail(nullptr, RAD_ERR_INVALID_ARG, "n_regions must be >= 0 and reserved == 0");
+    if (cfg->n_regions < 0) return fail(nullptr, RAD_ERR_INVALID_ARG, "n_regions must be >= 0");
+    if (cfg->window_type < RAD_WINDOW_NONE || cfg->window_type > RAD_WINDOW_HAMMING)
+        return fail(nullptr, RAD_ERR_INVALID_ARG, "unknown window_type");
+    if (cfg->window_type != RAD_WINDOW_NONE)
+        for (int c = 0; c < 3; ++c)
+            if (!std::isfinite(cfg->window_origin[c]) || !std::isfinite(cfg->window_extent[c]))
+                return fail(nullptr, RAD_ERR_INVALID_ARG, "window origin/extent must be finite");
     for (int j = 0; j < cfg->n_omega; ++j) {
         const double w = cfg->omega[j];
         if (!std::isfinite(w) || !(w > 0.0) || (j > 0 && !(w > cfg->omega[j - 1])))
@@ -346,6 +353,12 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     Handle &h = hh->h;
     h.device = cfg->device; h.D = cfg->n_dir; h.W = cfg->n_omega;
     h.R = cfg->n_regions > 1 ? cfg->n_regions : 1;
+    h.win_type = cfg->window_type;
+    for (int c = 0; c < 3; ++c) {
+        h.win_o[c] = cfg->window_origin[c];
+        h.win_il[c] = (h.win_type != RAD_WINDOW_NONE && cfg->window_extent[c] > 0.0) ? 1.0 / cfg->window_extent[c] : 0.0;
+    }
+    if (h.win_il[0] == 0.0 && h.win_il[1] == 0.0 && h.win_il[2] == 0.0) h.win_type = RAD_WINDOW_NONE;
     h.dt = cfg->dt; h.t0 = cfg->t0;
     h.scale = cfg->scale == 0.0 ? default_scale() : cfg->scale;
     h.state_f64 = cfg->state_dtype == RAD_F64;

@@ -120,7 +120,27 @@ __device__ __forceinline__ void phase_sincos_poly(uint32_t F, float Ff, float fl
     cs = __uint_as_float(__float_as_uint(fmaf(pc, r2, 1.0f)) ^ sign);
 }
 
-template <typename ST>
+// Spatial window on the macro weight (rad.h, reading W1): product over the windowed axes of
+// w1((r_c - o_c)/L_c).  Inside/outside is decided in fp64, the window value in fp32.
+__device__ __forceinline__ float window_weight(const AccumParams &P, double rx, double ry, double rz)
+{
+    if (P.win_type == RAD_WINDOW_NONE) return 1.0f;
+    const double r[3] = {rx, ry, rz};
+    float W = 1.0f;
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        if (P.win_il[c] > 0.0) {
+            const double u = (r[c] - P.win_o[c]) * P.win_il[c];
+            const float uf = to_f32(u);
+            const float w1 = P.win_type == RAD_WINDOW_TRIANGLE ? 1.0f - fabsf(fmaf(2.0f, uf, -1.0f))
+                                                               : fmaf(-0.46f, __cosf(kTwoPi * uf), 0.54f);
+            W *= (u >= 0.0 && u <= 1.0) ? w1 : 0.0f;
+        }
+    }
+    return W;
+}
+
+template <typename ST, bool WIN = true>
 __device__ __forceinline__ Particle load_particle(const AccumParams &P, long long k, bool valid)
 {
     Particle p;
@@ -137,6 +157,7 @@ __device__ __forceinline__ Particle load_particle(const AccumParams &P, long lon
         p.bfx = (float)bx; p.bfy = (float)by; p.bfz = (float)bz;
         p.bdx = (float)dx; p.bdy = (float)dy; p.bdz = (float)dz;
         p.wdt = (float)w * P.dt;
+        if (WIN) p.wdt *= window_weight(P, p.rx, p.ry, p.rz);
     } else {  // padding lane: zero amplitude, harmless phase
         p.rx = p.ry = p.rz = p.bx = p.by = p.bz = 0.0;
         p.bfx = p.bfy = p.bfz = p.bdx = p.bdy = p.bdz = p.wdt = 0.0f;

@@ -84,6 +84,9 @@ struct AccumParams {
     double ts32;           // (t0 + step dt) f_unit 2^32
     double dts32;          // dt f_unit 2^32: multi-step calls, chunk time = ts32 + chunk.step * dts32
     float dt;              // quadrature weight
+    int win_type;          // RAD_WINDOW_*; 0: none
+    double win_o[3];       // window box origin
+    double win_il[3];      // 1 / extent, 0: axis not windowed
     double *acc;           // [D][w_pad][4]: A1.re A1.im A2.re A2.im (transverse components)
     double *partial;       // deterministic mode: [n_chunks][D][w_pad][4], else NULL
     // streaming variant only: per-frequency constants and the (<= 2) direction records in the
@@ -122,6 +125,8 @@ struct Handle {
     int stream_nd = 1;
     int stream_nb = 0;               // > 0: D*W <= 16 -> particle-streaming kernel with 8 or 16 bins/thread
     double dt = 0, t0 = 0, scale = 0, f_unit = 0;
+    int win_type = 0;
+    double win_o[3] = {0, 0, 0}, win_il[3] = {0, 0, 0};
     bool state_f64 = false, deterministic = false, uniform = false;
     uint32_t rot_G = 0;              // uniform grid: rotator frequency LW*df in f_unit units
     float rot_Gf = 0, rot_gl = 0;

@@ -76,23 +76,26 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
         : "memory");
 }
 
-template <typename ST>
+template <typename ST, bool WIN>
 __device__ __forceinline__ Particle make_particle(ST rx, ST ry, ST rz, ST bx, ST by, ST bz, ST dx,
-                                                  ST dy, ST dz, ST w, float dt)
+                                                  ST dy, ST dz, ST w, const AccumParams &P)
 {
     Particle p;
     p.rx = to_f64(rx); p.ry = to_f64(ry); p.rz = to_f64(rz);
     p.bx = to_f64(bx); p.by = to_f64(by); p.bz = to_f64(bz);
     p.bfx = (float)bx; p.bfy = (float)by; p.bfz = (float)bz;
     p.bdx = (float)dx; p.bdy = (float)dy; p.bdz = (float)dz;
-    p.wdt = (float)w * dt;
+    p.wdt = (float)w * P.dt;
+    if (WIN) p.wdt *= window_weight(P, p.rx, p.ry, p.rz);
     return p;
 }
 
 // NB bins per thread = ND directions x WB frequencies (compile time; W is padded to WB with
 // zero-frequency bins that are discarded).  Per-bin frequency constants come straight from the
 // kernel-parameter constant bank (P.sF/sFf/sfl), not from registers.
-template <typename ST, int NB, int ND>
+// WIN: spatial window compiled in (kept out of the default instantiation: the streaming kernel
+// is latency bound and loses 3 % to the extra per-particle code even when the window is off)
+template <typename ST, int NB, int ND, bool WIN>
 __global__ void __launch_bounds__(kSThreads, NB <= 8 ? RAD_S_MINB : 1) rad_accum_stream(const AccumParams P, const int use_bulk)
 {
     constexpr int TILE = kSTileBytes / (int)sizeof(ST);  // particles per tile
@@ -155,12 +158,12 @@ __global__ void __launch_bounds__(kSThreads, NB <= 8 ? RAD_S_MINB : 1) rad_accum
             const long long k = t * TILE + kl;
             Particle p;
             if (bulk) {
-                p = make_particle<ST>(sm[0 * TILE + kl], sm[1 * TILE + kl], sm[2 * TILE + kl],
+                p = make_particle<ST, WIN>(sm[0 * TILE + kl], sm[1 * TILE + kl], sm[2 * TILE + kl],
                                       sm[3 * TILE + kl], sm[4 * TILE + kl], sm[5 * TILE + kl],
                                       sm[6 * TILE + kl], sm[7 * TILE + kl], sm[8 * TILE + kl],
-                                      sm[9 * TILE + kl], P.dt);
+                                      sm[9 * TILE + kl], P);
             } else {
-                p = load_particle<ST>(P, k, k < N);
+                p = load_particle<ST, WIN>(P, k, k < N);
             }
 #pragma unroll
             for (int d = 0; d < ND; ++d) {
@@ -210,19 +213,26 @@ __global__ void __launch_bounds__(kSThreads, NB <= 8 ? RAD_S_MINB : 1) rad_accum
     }
 }
 
-template <typename ST, int NB, int ND>
-cudaError_t launch_stream_t(const AccumParams &p, int grid, cudaStream_t s)
+template <typename ST, int NB, int ND, bool WIN>
+cudaError_t launch_stream_w(const AccumParams &p, int grid, cudaStream_t s)
 {
     const size_t smem = (size_t)kSStages * 10 * kSTileBytes;
     // per device and per template instance; the call is a cheap host-side set, so no caching
-    cudaError_t e = cudaFuncSetAttribute(rad_accum_stream<ST, NB, ND>,
+    cudaError_t e = cudaFuncSetAttribute(rad_accum_stream<ST, NB, ND, WIN>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int use_bulk = getenv("RAD_STREAM_PLAIN") ? 0 : 1;  // debug: force the plain-load path
     for (int a = 0; a < 10; ++a)
         if (reinterpret_cast<uintptr_t>(p.st[a]) & 15) use_bulk = 0;
-    rad_accum_stream<ST, NB, ND><<<grid, kSThreads, smem, s>>>(p, use_bulk);
+    rad_accum_stream<ST, NB, ND, WIN><<<grid, kSThreads, smem, s>>>(p, use_bulk);
     return cudaGetLastError();
+}
+
+template <typename ST, int NB, int ND>
+cudaError_t launch_stream_t(const AccumParams &p, int grid, cudaStream_t s)
+{
+    return p.win_type != RAD_WINDOW_NONE ? launch_stream_w<ST, NB, ND, true>(p, grid, s)
+                                         : launch_stream_w<ST, NB, ND, false>(p, grid, s);
 }
 
 template <typename ST>

@@ -411,3 +411,61 @@ def test_relativistic_beam_small_doppler_factor(oracle_mod, dtype):
     for d in range(len(dirs)):      # every direction on its own scale (forward/backward differ by ~1e14)
         P.assert_parity(S[d], ref[d], what=f"beam dir {d}")
     print(f"beam {np.dtype(dtype).name}: min(1-beta.n)={dmin:.2e} relL2={l2:.2e} maxrel={mr:.2e}")
+
+
+@pytest.mark.parametrize("kind,shape", [("triangle", "general"), ("hamming", "general"), ("hamming", "uniform"),
+                                         ("triangle", "stream"), ("hamming", "regions")])
+def test_spatial_window(oracle_mod, kind, shape):
+    """NEXT-3 window functions (rad.h, reading W1) through every accumulate kernel: KHI particles
+    in the 10 um box, window over x and y only (z extent 0), box chosen so that a part of the
+    particles lies outside and gets weight exactly 0; fp32 state."""
+    from paper_2501_03383_b200 import binding
+    L = 10e-6
+    win = (kind, (0.1 * L, -0.2 * L, 0.0), (0.7 * L, 1.1 * L, 0.0))
+    if shape == "uniform":
+        dirs, omega = wl.dirs_fibonacci(6), np.linspace(2e14, 4e16, 128)
+    elif shape == "stream":
+        dirs, omega = wl.dirs_fibonacci(1), wl.omega_log(8)
+    else:
+        dirs, omega = wl.dirs_fibonacci(5), wl.omega_log(96)
+    w = wl.Workload("win", 3000, 2, 1e-17, dirs, omega, np.float32, wl.BASE_SEED + 40, "khi")
+    steps = list(w.steps())
+    if shape == "regions":
+        off = np.array([0, 1000, 1000, 3000], dtype=np.int64)
+        o = oracle_mod.RegionOracle(3, w.dirs, w.omega, w.dt, scale=1.0, window=win)
+        for t, st in steps:
+            o.accumulate_step(t, off, *st)
+        with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, n_regions=3, window=win) as det:
+            for t, st in steps:
+                det.accumulate_step_regions(t, off, P.to_device(st))
+            S = det.spectrum()
+        for r in (0, 2):
+            P.assert_parity(S[r], o.spectrum()[r], what=f"window regions {r}")
+        assert np.all(S[1] == 0.0)
+        return
+    o = oracle_mod.Oracle(w.dirs, w.omega, w.dt, scale=1.0, window=win)
+    for t, st in steps:
+        o.accumulate_step(t, *st)
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, window=win) as det:
+        for t, st in steps:
+            det.accumulate_step(t, P.to_device(st))
+        S, variant = det.spectrum(), det.kernel_variant
+    assert variant == shape
+    l2, mr = P.assert_parity(S, o.spectrum(), what=f"window {kind} {shape}")
+    plain = P.run_oracle(oracle_mod, w, steps).spectrum()
+    assert P.rel_l2(o.spectrum(), plain) > 0.1        # the window really changes the result
+    print(f"window {kind}/{shape}: relL2={l2:.2e} maxrel={mr:.2e}")
+
+
+def test_window_argument_errors_and_identity():
+    from paper_2501_03383_b200 import binding
+    w = wl.make_workload("3c")
+    (t, st), = list(w.steps(n_steps=1, n_particles=400))
+    with pytest.raises(binding.RadError, match="window_type"):
+        binding.Detector(w.dirs, w.omega, w.dt, window=(7, (0, 0, 0), (1, 1, 1)))
+    with pytest.raises(binding.RadError, match="finite"):
+        binding.Detector(w.dirs, w.omega, w.dt, window=("hamming", (0, float("nan"), 0), (1, 1, 1)))
+    S0, _ = P.run_gpu(w, [(t, st)])
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, window=("triangle", (0, 0, 0), (0, -1, 0))) as det:
+        det.accumulate_step(t, P.to_device(st))          # no axis windowed -> identity
+        assert np.array_equal(det.spectrum(), S0)
