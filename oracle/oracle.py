@@ -56,6 +56,8 @@ def _load():
         lib.oracle_accumulate_step_regions_w.restype = ctypes.c_int
         lib.oracle_accumulate_step_regions_w.argtypes = (lib.oracle_accumulate_step_regions.argtypes
                                                          + [ctypes.c_int, ctypes.c_void_p])
+        lib.oracle_set_nyquist.restype = None
+        lib.oracle_set_nyquist.argtypes = [ctypes.c_double]
         lib.oracle_spectrum.restype = ctypes.c_int
         lib.oracle_spectrum.argtypes = [ctypes.c_longlong, ctypes.c_void_p, ctypes.c_double,
                                         ctypes.c_void_p]
@@ -89,7 +91,8 @@ class Oracle:
     dir*W + j) restricts the computation to a subset of bins; other bins stay zero.
     """
 
-    def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, bins=None, window=None):
+    def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, bins=None, window=None, nyquist=0.0):
+        self.nyquist = float(nyquist)
         self.dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
         self.omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
         self.dt, self.t0, self.scale = float(dt), float(t0), float(scale)
@@ -112,6 +115,7 @@ class Oracle:
             raise ValueError("state arrays must be 1-D and of equal length")
         nb = 0 if self.bins is None else self.bins.shape[0]
         bp = None if self.bins is None else self.bins.ctypes.data
+        _load().oracle_set_nyquist(self.nyquist)
         rc = _load().oracle_accumulate_step_w(
             self.D, self.dirs.ctypes.data, self.W, self.omega.ctypes.data, self.dt, self.t0,
             int(step_index), n, int(dt0 == np.dtype(np.float32)),
@@ -137,8 +141,9 @@ class RegionOracle:
     only.  Particles are sorted by region; ``offsets`` [R+1] (non-decreasing) are passed with
     every step.  Same (optional) bin subset in every region."""
 
-    def __init__(self, n_regions, dirs, omega, dt, t0=0.0, scale=0.0, bins=None, window=None):
+    def __init__(self, n_regions, dirs, omega, dt, t0=0.0, scale=0.0, bins=None, window=None, nyquist=0.0):
         self.win_type, self.win = _window_args(window)
+        self.nyquist = float(nyquist)
         self.dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
         self.omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
         self.dt, self.t0, self.scale = float(dt), float(t0), float(scale)
@@ -163,6 +168,7 @@ class RegionOracle:
             raise ValueError("state arrays must be 1-D, of equal length >= offsets[-1]")
         nb = 0 if self.bins is None else self.bins.shape[0]
         bp = None if self.bins is None else self.bins.ctypes.data
+        _load().oracle_set_nyquist(self.nyquist)
         rc = _load().oracle_accumulate_step_regions_w(
             self.D, self.dirs.ctypes.data, self.W, self.omega.ctypes.data, self.dt, self.t0,
             int(step_index), self.R, offsets.ctypes.data, int(dt0 == np.dtype(np.float32)),

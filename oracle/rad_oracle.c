@@ -50,6 +50,16 @@
  * evaluated at the particle's position of that step.  Pins: type NONE and all-zero extents
  * change nothing; closed-form window values times the Dirichlet kernel; outside -> exactly 0;
  * equals the unwindowed oracle fed w*Wn(r) computed independently in numpy.
+ *
+ * Nyquist limiter (NEXT-3, reading N1 of DESIGN.md; at dt = 1e-17 s the top of
+ * the BASELINE.json frequency range is beyond the sampling limit): with nyquist_factor nu > 0
+ * the term of particle k is dropped from bin (n, w_j) when
+ *     w_j * dt * (1 - beta_k.n) >= pi * nu,
+ * i.e. when the phase of the emitted wave, which advances by w (1 - beta.n) dt per step along
+ * the trajectory, is sampled fewer than 2/nu times per period.  Pins: nu = 0 and nu = huge change
+ * nothing; a static particle loses exactly the bins w_j dt >= pi nu; the cut-off of a moving
+ * particle is Doppler shifted by direction; kept bins equal the closed forms.
+ * (oracle_set_nyquist() sets nu for the calls that follow; 0 = off.)
  */
 #include <math.h>
 #include <stddef.h>
@@ -87,6 +97,9 @@ static void cross3(const double a[3], const double b[3], double out[3])
     out[2] = a[0] * b[1] - a[1] * b[0];
 }
 
+static double g_nyquist = 0.0; /* nu of the Nyquist limiter, 0 = off (test-infrastructure state) */
+void oracle_set_nyquist(double nu) { g_nyquist = nu; }
+
 /* w1(u) of the spatial window, see the header. */
 static double window_1d(int type, double u)
 {
@@ -121,6 +134,7 @@ int oracle_accumulate_step_w(int n_dir, const double *dirs, int n_omega, const d
     if (n_dir <= 0 || n_omega <= 0 || !dirs || !omega || !A || n_part < 0) return 1;
     const long long total = bin_idx ? n_bins : (long long)n_dir * n_omega;
     const double t_step = t0 + (double)step_index * dt;
+    const double nyq_lim = 3.14159265358979323846 * g_nyquist;
 
 #define LOAD(p, k) (is_f32 ? (double)((const float *)(p))[k] : ((const double *)(p))[k])
 
@@ -149,6 +163,7 @@ int oracle_accumulate_step_w(int n_dir, const double *dirs, int n_omega, const d
             cross3(n, inner, outer);  /* n x ((n - beta) x betadot)  */
             const double pre = wk * dt / (d * d);
             const double tau = t_step - (n[0] * r[0] + n[1] * r[1] + n[2] * r[2]) / ORACLE_C_LIGHT;
+            if (nyq_lim > 0.0 && om * dt * d >= nyq_lim) continue; /* Nyquist limiter, reading N1 */
             const double ph = om * tau;
             const double cs = cos(ph), sn = sin(ph);
             for (int c = 0; c < 3; ++c) {

@@ -470,3 +470,66 @@ def test_p12_window_equals_reweighting_and_none_is_identity(oracle_mod):
         ro.accumulate_step(t, off, *st)
         ow.accumulate_step(t, *st)
     assert np.allclose(ro.A.sum(0), ow.A, rtol=0, atol=1e-13 * np.abs(ow.A).max())
+
+
+# ------------------------------------------------- P13 Nyquist limiter (NEXT-3, reading N1)
+def test_p13_nyquist_static_particle_loses_exactly_the_undersampled_bins(oracle_mod):
+    """beta = 0 (1 - beta.n = 1): bins with w dt >= pi nu vanish exactly, the others keep the
+    Dirichlet closed form; nu = 0 and a huge nu leave everything in place."""
+    b = np.array([1.0e13, -2.0e13, 0.5e13])
+    T = 7
+    steps = [(t, _const_state((1e-7, 2e-7, 3e-7), (0, 0, 0), b)) for t in range(T)]
+    plain = _run(oracle_mod, DIRS, OMEGA, DT, steps).spectrum()
+    nu = 0.1                                                   # pi nu / dt = 1.57e16 rad/s
+    cut = OMEGA * DT >= np.pi * nu
+    assert cut.tolist() == [False, False, False, False, True]
+    o = oracle_mod.Oracle(DIRS, OMEGA, DT, scale=1.0, nyquist=nu)
+    for t, st in steps:
+        o.accumulate_step(t, *st)
+    S = o.spectrum()
+    assert np.all(S[:, cut] == 0.0) and np.array_equal(S[:, ~cut], plain[:, ~cut])
+    x = OMEGA * DT / 2
+    closed = (b @ b - (UNIT[3] @ b) ** 2) * DT ** 2 * (np.sin(T * x) / np.sin(x)) ** 2
+    assert np.allclose(S[3, ~cut], closed[~cut], rtol=1e-9)
+    for nu_off in (0.0, 1e9):
+        o2 = oracle_mod.Oracle(DIRS, OMEGA, DT, scale=1.0, nyquist=nu_off)
+        for t, st in steps:
+            o2.accumulate_step(t, *st)
+        assert np.array_equal(o2.spectrum(), plain)
+    # the limiter setting of one oracle object does not leak into the next call of another
+    assert np.array_equal(_run(oracle_mod, DIRS, OMEGA, DT, steps).spectrum(), plain)
+
+
+def test_p13_nyquist_cutoff_is_doppler_shifted_by_direction(oracle_mod):
+    """Particle moving with beta = 0.9 x: towards the observer (n = +x) 1 - beta.n = 0.1, so the
+    cut-off frequency pi nu / (dt (1 - beta.n)) is 19x higher than for n = -x.  Kept bins equal
+    pin P4's closed form, and a second, static particle is limited by its own factor only."""
+    beta = np.array([0.9, 0.0, 0.0])
+    b = np.array([0.0, 3.0e13, 1.0e13])
+    r0 = np.array([1e-7, -2e-7, 0.5e-7])
+    T, nu = 6, 0.05
+    dirs = np.array([[1.0, 0, 0], [-1.0, 0, 0], [0, 1.0, 0]])
+    mov = [(t, _const_state(r0 + beta * C * t * DT, beta, b)) for t in range(T)]
+    o = oracle_mod.Oracle(dirs, OMEGA, DT, scale=1.0, nyquist=nu)
+    for t, st in mov:
+        o.accumulate_step(t, *st)
+    S = o.spectrum()
+    for i, n in enumerate(dirs):
+        d = 1.0 - beta @ n
+        cut = OMEGA * DT * d >= np.pi * nu
+        vec = np.cross(n, np.cross(n - beta, b))
+        xp = OMEGA * d * DT / 2
+        closed = (vec @ vec) / d ** 4 * DT ** 2 * (np.sin(T * xp) / np.sin(xp)) ** 2
+        assert np.all(S[i, cut] == 0.0)
+        assert np.allclose(S[i, ~cut], closed[~cut], rtol=1e-8)
+    assert np.count_nonzero(S[0]) > np.count_nonzero(S[1])        # forward keeps more bins than backward
+    # add a static particle: where the mover is cut, the sum equals the static particle alone
+    both = [(t, [np.concatenate([a, s]) for a, s in zip(st, _const_state(-r0, (0, 0, 0), 2 * b))]) for t, st in mov]
+    stat = [(t, _const_state(-r0, (0, 0, 0), 2 * b)) for t in range(T)]
+    ob = oracle_mod.Oracle(dirs, OMEGA, DT, scale=1.0, nyquist=nu)
+    os_ = oracle_mod.Oracle(dirs, OMEGA, DT, scale=1.0, nyquist=nu)
+    for (t, s2), (_, s1) in zip(both, stat):
+        ob.accumulate_step(t, *s2)
+        os_.accumulate_step(t, *s1)
+    cut_mov = OMEGA * DT * 1.9 >= np.pi * nu                     # direction -x
+    assert np.allclose(ob.spectrum()[1, cut_mov], os_.spectrum()[1, cut_mov], rtol=1e-12)
