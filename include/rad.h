@@ -88,7 +88,16 @@ typedef struct {
     int32_t window_type;   /* RAD_WINDOW_*: spatial window on the macro weights (below)    */
     double window_origin[3]; /* m: lower corner o of the window box                        */
     double window_extent[3]; /* m: edge lengths L; L_c <= 0: axis c is not windowed        */
+    double nyquist_factor; /* nu >= 0; 0: off.  Nyquist limiter (below)                      */
 } rad_config;
+
+/* Nyquist limiter (not in the paper; reading N1 of DESIGN.md): with nyquist_factor = nu > 0 the
+ * term of particle k at a step is left out of bin (n, w_j) when
+ *     w_j * dt * (1 - beta_k.n) >= pi * nu,
+ * i.e. when the wave the particle emits towards n, whose phase advances by w (1 - beta.n) dt per
+ * step, is sampled fewer than 2/nu times per period (nu = 1: the Nyquist limit itself).  The
+ * comparison is made in fp64, exactly as written.  Detectors with nu > 0 use the general-grid
+ * kernel for every shape. */
 
 /* Spatial window (not in the paper, which cites the plugin [37] for such details; reading W1 of
  * DESIGN.md): with window_type != RAD_WINDOW_NONE the macro weight of every particle is

@@ -41,6 +41,7 @@ class rad_config(ctypes.Structure):
         ("state_dtype", ctypes.c_int32), ("flags", ctypes.c_uint32),
         ("n_regions", ctypes.c_int32), ("window_type", ctypes.c_int32),
         ("window_origin", ctypes.c_double * 3), ("window_extent", ctypes.c_double * 3),
+        ("nyquist_factor", ctypes.c_double),
     ]
 
 
@@ -120,7 +121,7 @@ def _check(status: int, handle) -> None:
 # ------------------------------------------------------------------ ABI-named functions
 def rad_create(dirs, omega, dt: float, t0: float = 0.0, scale: float = 0.0,
                state_dtype: int = RAD_F32, flags: int = 0, device: int = 0, n_regions: int = 0,
-               window=None) -> int:
+               window=None, nyquist: float = 0.0) -> int:
     """-> opaque handle (int).  dirs [D,3], omega [W]: HOST fp64 (copied by the library).
     window: None or (type name | code, origin[3], extent[3])."""
     dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
@@ -128,6 +129,7 @@ def rad_create(dirs, omega, dt: float, t0: float = 0.0, scale: float = 0.0,
     cfg = rad_config(ctypes.sizeof(rad_config), device, dirs.shape[0], omega.shape[0],
                      dirs.ctypes.data, omega.ctypes.data, dt, t0, scale, state_dtype, flags,
                      n_regions, 0)
+    cfg.nyquist_factor = float(nyquist)
     if window is not None:
         kind, origin, extent = window
         cfg.window_type = WINDOW_TYPES[kind] if isinstance(kind, str) else int(kind)
@@ -220,14 +222,14 @@ class Detector:
     pinned torch CPU tensors (host path, copies inside the library)."""
 
     def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, state_dtype=np.float32, flags=0, device=0,
-                 n_regions=0, window=None):
+                 n_regions=0, window=None, nyquist=0.0):
         self.D = int(np.asarray(dirs).reshape(-1, 3).shape[0])
         self.W = int(np.asarray(omega).reshape(-1).shape[0])
         self.R = max(1, int(n_regions))
         self.np_dtype = np.dtype(state_dtype)
         code = {np.dtype(np.float32): RAD_F32, np.dtype(np.float64): RAD_F64}[self.np_dtype]
         self.device = device
-        self.handle = rad_create(dirs, omega, dt, t0, scale, code, flags, device, n_regions, window)
+        self.handle = rad_create(dirs, omega, dt, t0, scale, code, flags, device, n_regions, window, nyquist)
 
     def _shape(self, *tail):
         return ((self.R,) if self.R > 1 else ()) + (self.D, self.W) + tail

@@ -50,7 +50,7 @@ void free_all(Handle &h)
 {
     cudaFree(h.dirs_d); cudaFree(h.basis_d); cudaFree(h.F_d); cudaFree(h.Ff_d); cudaFree(h.fl_d);
     cudaFree(h.acc_d); cudaFree(h.partial_d); cudaFree(h.stage_d[0]); cudaFree(h.stage_d[1]);
-    cudaFree(h.out_d); cudaFree(h.chunks_d); cudaFree(h.reg_cstart_d);
+    cudaFree(h.out_d); cudaFree(h.chunks_d); cudaFree(h.reg_cstart_d); cudaFree(h.omega_d);
     if (h.chunks_h) cudaFreeHost(h.chunks_h);
     if (h.reg_cstart_h) cudaFreeHost(h.reg_cstart_h);
     if (h.reg_uploaded) cudaEventDestroy(h.reg_uploaded);
@@ -257,6 +257,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.dirs = h.dirs_d; p.F = h.F_d; p.Ff = h.Ff_d; p.fl = h.fl_d;
     p.ts32 = (h.t0 + (double)step * h.dt) * h.f_unit * kTwo32;
     p.dts32 = h.dt * h.f_unit * kTwo32;
+    p.nyq_lim = h.nyq_lim; p.dt64 = h.dt; p.omega64 = h.omega_d;
     p.win_type = h.win_type;
     for (int c = 0; c < 3; ++c) { p.win_o[c] = h.win_o[c]; p.win_il[c] = h.win_il[c]; }
     p.dt = (float)h.dt;
@@ -337,6 +338,8 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     if (cfg->flags & ~(RAD_FLAG_DETERMINISTIC | RAD_FLAG_FORCE_GENERAL))
         return fail(nullptr, RAD_ERR_INVALID_ARG, "unknown flag bits");
     if (cfg->n_regions < 0) return fail(nullptr, RAD_ERR_INVALID_ARG, "n_regions must be >= 0");
+    if (!std::isfinite(cfg->nyquist_factor) || cfg->nyquist_factor < 0.0)
+        return fail(nullptr, RAD_ERR_INVALID_ARG, "nyquist_factor must be finite and >= 0");
     if (cfg->window_type < RAD_WINDOW_NONE || cfg->window_type > RAD_WINDOW_HAMMING)
         return fail(nullptr, RAD_ERR_INVALID_ARG, "unknown window_type");
     if (cfg->window_type != RAD_WINDOW_NONE)
@@ -353,6 +356,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     Handle &h = hh->h;
     h.device = cfg->device; h.D = cfg->n_dir; h.W = cfg->n_omega;
     h.R = cfg->n_regions > 1 ? cfg->n_regions : 1;
+    h.nyq_lim = kPi * cfg->nyquist_factor;
     h.win_type = cfg->window_type;
     for (int c = 0; c < 3; ++c) {
         h.win_o[c] = cfg->window_origin[c];
@@ -402,10 +406,11 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     }
     h.sdir[0] = recs[0]; h.sdir[1] = recs[h.D > 1 ? 1 : 0];
     choose_tile(h);
-    h.stream_nb = h.R > 1 ? 0 : stream_shape(h.D, h.W, &h.stream_nd);  // per-region: bin-owner kernels only
+    // per-region detectors and the Nyquist limiter: bin-owner kernels only
+    h.stream_nb = (h.R > 1 || h.nyq_lim > 0.0) ? 0 : stream_shape(h.D, h.W, &h.stream_nd);
     // uniform grid?  w_j = w_0 + j dw to fp64 rounding -> rotation-recurrence kernel (a2')
     h.uniform = false;
-    if (h.W >= 2 * h.strip && !(cfg->flags & RAD_FLAG_FORCE_GENERAL)) {
+    if (h.W >= 2 * h.strip && !(cfg->flags & RAD_FLAG_FORCE_GENERAL) && h.nyq_lim == 0.0) {
         const double dw = (h.omega_h.back() - h.omega_h.front()) / (h.W - 1);
         bool uni = true;
         for (int j = 0; j < h.W && uni; ++j)
@@ -440,7 +445,8 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
               cudaMalloc(&h.F_d, sizeof(uint32_t) * h.w_pad) == cudaSuccess &&
               cudaMalloc(&h.Ff_d, sizeof(float) * h.w_pad) == cudaSuccess &&
               cudaMalloc(&h.fl_d, sizeof(float) * h.w_pad) == cudaSuccess &&
-              cudaMalloc(&h.acc_d, acc_bytes) == cudaSuccess;
+              cudaMalloc(&h.acc_d, acc_bytes) == cudaSuccess &&
+              (h.nyq_lim == 0.0 || cudaMalloc(&h.omega_d, sizeof(double) * h.W) == cudaSuccess);
     if (!ok) {
         cudaGetLastError(); free_all(h); delete hh;
         return fail(nullptr, RAD_ERR_ALLOC, "cudaMalloc(tables/accumulator) failed");
@@ -451,6 +457,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
          cudaMemcpy(h.Ff_d, Ff.data(), sizeof(float) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemcpy(h.fl_d, fl.data(), sizeof(float) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemset(h.acc_d, 0, acc_bytes) == cudaSuccess &&
+         (!h.omega_d || cudaMemcpy(h.omega_d, h.omega_h.data(), sizeof(double) * h.W, cudaMemcpyHostToDevice) == cudaSuccess) &&
          cudaStreamCreateWithFlags(&h.copy_stream, cudaStreamNonBlocking) == cudaSuccess;
     for (int i = 0; ok && i < 2; ++i)
         ok = cudaEventCreateWithFlags(&h.copied[i], cudaEventDisableTiming) == cudaSuccess &&

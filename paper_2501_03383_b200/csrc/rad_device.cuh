@@ -50,7 +50,8 @@ struct Particle {
 };
 
 __device__ __forceinline__ void stage_record(const Particle &p, const DirRec &dr, double ts32,
-                                             float4 &rec, float &sf, uint32_t *T_out = nullptr)
+                                             float4 &rec, float &sf, uint32_t *T_out = nullptr,
+                                             double *d_out = nullptr)
 {
     // phase: s32 = (t - n.r/c) f_unit 2^32 in fp64, split into integer (mod 2^32) + residual
     const double s32 = ts32 - fma(dr.kx, p.rx, fma(dr.ky, p.ry, dr.kz * p.rz));
@@ -75,6 +76,20 @@ __device__ __forceinline__ void stage_record(const Particle &p, const DirRec &dr
     rec.w = pre * fmaf(e2b, g, e2d * d);
     sf = to_f32(s32) * kUnitToRad;
     if (T_out) *T_out = T;
+    if (d_out) *d_out = d64;
+}
+
+// Nyquist limiter (rad.h, reading N1): number of bins j with w_j dt d < pi nu.  The predicate is
+// the oracle's expression in fp64, monotone in j, so a bisection over the sorted w_j finds it.
+__device__ __forceinline__ int nyquist_count(const AccumParams &P, double d)
+{
+    int lo = 0, hi = P.n_omega;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (__dmul_rn(__dmul_rn(__ldg(P.omega64 + mid), P.dt64), d) < P.nyq_lim) lo = mid + 1;
+        else hi = mid;
+    }
+    return lo;
 }
 
 // exp(i 2 pi f tau) for one frequency f = (F + phi) f_unit from a staged record (integer phase)

@@ -84,6 +84,9 @@ struct AccumParams {
     double ts32;           // (t0 + step dt) f_unit 2^32
     double dts32;          // dt f_unit 2^32: multi-step calls, chunk time = ts32 + chunk.step * dts32
     float dt;              // quadrature weight
+    double nyq_lim;        // pi * nyquist_factor, 0: limiter off
+    double dt64;           // dt in fp64 (limiter comparison)
+    const double *omega64; // [W] fp64 angular frequencies (limiter comparison)
     int win_type;          // RAD_WINDOW_*; 0: none
     double win_o[3];       // window box origin
     double win_il[3];      // 1 / extent, 0: axis not windowed
@@ -125,6 +128,8 @@ struct Handle {
     int stream_nd = 1;
     int stream_nb = 0;               // > 0: D*W <= 16 -> particle-streaming kernel with 8 or 16 bins/thread
     double dt = 0, t0 = 0, scale = 0, f_unit = 0;
+    double nyq_lim = 0;              // pi * nyquist_factor
+    double *omega_d = nullptr;       // [W] fp64 (Nyquist limiter only)
     int win_type = 0;
     double win_o[3] = {0, 0, 0}, win_il[3] = {0, 0, 0};
     bool state_f64 = false, deterministic = false, uniform = false;

@@ -92,15 +92,20 @@ __device__ __forceinline__ bool decode_task(const AccumParams &P, int warp, int 
 // steps forwards (rot) and S/2-1 backwards (conj rot): 1 sincos + (S-1) complex rotations per S
 // updates instead of S sincos.  Chain length <= S/2 keeps the recurrence drift (~6e-8 per
 // rotation) below the MUFU error, which is the periodic re-anchoring BASELINE.json asks for.
-template <typename ST, int LW, int S, int MINB, bool UNI>
+// NYQ (general grid only): Nyquist limiter -- the staging lane also finds, per (particle,
+// direction), how many bins lie below the cut-off (nyquist_count); the sweep accumulates bin j
+// only if j < that count (one ISETP per update, the FFMAs and MUFUs are predicated).
+template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ>
 __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
 {
+    static_assert(!(UNI && NYQ), "the limiter runs on the general-grid kernel");
     constexpr int DPW = 32 / LW;
     constexpr int NC = UNI ? 1 : S;  // per-thread frequency constants held in registers
     constexpr int MID = S / 2 - 1;   // anchor bin of the uniform-grid chain
     __shared__ float4 s_rec[kWarpsPerBlock][kBatch * DPW];
     __shared__ float s_sf[kWarpsPerBlock][kBatch * DPW];
     __shared__ float2 s_rot[UNI ? kWarpsPerBlock : 1][UNI ? kBatch * DPW : 1];
+    __shared__ int s_jc[NYQ ? kWarpsPerBlock : 1][NYQ ? kBatch * DPW : 1];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int wt, ci, region;
@@ -126,6 +131,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
     float4 *rec = s_rec[warp];
     float *sfs = s_sf[warp];
     float2 *rots = s_rot[UNI ? warp : 0];
+    int *jcs = s_jc[NYQ ? warp : 0];
 
     for (long long kb = k0; kb < k1; kb += kBatch) {
         {  // a1: stage
@@ -137,9 +143,11 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 float4 r4;
                 float sf;
                 uint32_t T;
-                stage_record(p, P.dirs[dir], ts32, r4, sf, &T);
+                double d64;
+                stage_record(p, P.dirs[dir], ts32, r4, sf, &T, &d64);
                 rec[lane * DPW + dd] = r4;
                 sfs[lane * DPW + dd] = sf;
+                if (NYQ) jcs[lane * DPW + dd] = nyquist_count(P, d64);
                 if (UNI) {
                     float sn, cs;
                     phase_sincos(P.rot_G, P.rot_Gf, P.rot_gl, T, r4.y, sf, sn, cs);
@@ -190,8 +198,10 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 const float4 r4 = rec[kk * DPW + ld];
                 const float sf = sfs[kk * DPW + ld];
                 const uint32_t T = __float_as_uint(r4.x);
+                const int m = NYQ ? jcs[kk * DPW + ld] - jbase : 0;  // bins jbase + i*LW < count are kept
 #pragma unroll
                 for (int i = 0; i < S; ++i) {
+                    if (NYQ && i * LW >= m) continue;
                     float sn, cs;
                     if (i >= S - n_poly)
                         phase_sincos_poly(F[i % NC], Ff[i % NC], fl[i % NC], T, r4.y, sf, sn, cs);
@@ -216,23 +226,23 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
 
 // ------------------------------------------------------------------------------------------
 // Launch logic.
-template <typename ST, int LW, int S, int MINB, bool UNI>
+template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ>
 static cudaError_t launch_one(const AccumParams &p, cudaStream_t s)
 {
     const long long n_tasks = (long long)p.n_wtiles * p.n_chunks;
     const unsigned grid = (unsigned)((n_tasks + kWarpsPerBlock - 1) / kWarpsPerBlock);
-    rad_accum<ST, LW, S, MINB, UNI><<<grid, kThreads, 0, s>>>(p);
+    rad_accum<ST, LW, S, MINB, UNI, NYQ><<<grid, kThreads, 0, s>>>(p);
     return cudaGetLastError();
 }
 
-template <typename ST, bool UNI>
+template <typename ST, bool UNI, bool NYQ>
 static cudaError_t dispatch(const Handle &h, const AccumParams &p, cudaStream_t s)
 {
     switch (h.lw) {
-        case 32: return launch_one<ST, 32, kStrip, kMinBlocks, UNI>(p, s);
-        case 16: return launch_one<ST, 16, kStrip, kMinBlocks, UNI>(p, s);
-        case 8: return launch_one<ST, 8, kStrip, kMinBlocks, UNI>(p, s);
-        default: return launch_one<ST, 4, kStrip, kMinBlocks, UNI>(p, s);
+        case 32: return launch_one<ST, 32, kStrip, kMinBlocks, UNI, NYQ>(p, s);
+        case 16: return launch_one<ST, 16, kStrip, kMinBlocks, UNI, NYQ>(p, s);
+        case 8: return launch_one<ST, 8, kStrip, kMinBlocks, UNI, NYQ>(p, s);
+        default: return launch_one<ST, 4, kStrip, kMinBlocks, UNI, NYQ>(p, s);
     }
 }
 
@@ -242,10 +252,14 @@ cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_
     *n_launches = 1;
     if (h.uniform) {
         *variant = "uniform";
-        return state_f64 ? dispatch<double, true>(h, p, s) : dispatch<float, true>(h, p, s);
+        return state_f64 ? dispatch<double, true, false>(h, p, s) : dispatch<float, true, false>(h, p, s);
+    }
+    if (p.nyq_lim > 0.0) {
+        *variant = "general+nyquist";
+        return state_f64 ? dispatch<double, false, true>(h, p, s) : dispatch<float, false, true>(h, p, s);
     }
     *variant = "general";
-    return state_f64 ? dispatch<double, false>(h, p, s) : dispatch<float, false>(h, p, s);
+    return state_f64 ? dispatch<double, false, false>(h, p, s) : dispatch<float, false, false>(h, p, s);
 }
 
 }  // namespace rad

@@ -469,3 +469,53 @@ def test_window_argument_errors_and_identity():
     with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, window=("triangle", (0, 0, 0), (0, -1, 0))) as det:
         det.accumulate_step(t, P.to_device(st))          # no axis windowed -> identity
         assert np.array_equal(det.spectrum(), S0)
+
+
+@pytest.mark.parametrize("D,W,dtype,nu", [(6, 300, np.float32, 0.5), (33, 64, np.float32, 1.0), (4, 1024, np.float64, 0.25),
+                                          (1, 8, np.float32, 0.5)])
+def test_nyquist_limiter(oracle_mod, D, W, dtype, nu):
+    """NEXT-3 Nyquist limiter (rad.h, reading N1): at dt = 1e-17 s and w up to 1e18 rad/s the
+    cut-off pi nu / (dt (1 - beta.n)) falls inside the grid and differs per particle and
+    direction (beta_x = +-0.2 streams); the GPU must take the same keep/drop decisions as the
+    oracle (fp64 on both sides), so the usual tolerances apply to every bin."""
+    from paper_2501_03383_b200 import binding
+    w = wl.Workload("nyq", 2000, 3, 1e-17, wl.dirs_fibonacci(D), wl.omega_log(W), dtype, wl.BASE_SEED + 50, "khi")
+    steps = list(w.steps())
+    o = oracle_mod.Oracle(w.dirs, w.omega, w.dt, scale=1.0, nyquist=nu)
+    for t, st in steps:
+        o.accumulate_step(t, *st)
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, state_dtype=dtype, nyquist=nu) as det:
+        for t, st in steps:
+            det.accumulate_step(t, P.to_device(st))
+        S, variant = det.spectrum(), det.kernel_variant
+    assert variant == "general+nyquist"
+    ref = o.spectrum()
+    plain = P.run_oracle(oracle_mod, w, steps).spectrum()
+    assert np.array_equal(ref[:, 0], plain[:, 0]) and not np.allclose(ref[:, -1], plain[:, -1], rtol=1e-3)
+    # bins every particle is cut from are exactly zero on both sides
+    dead = ref == 0.0
+    assert np.array_equal(S == 0.0, dead)
+    l2, mr = P.assert_parity(S, ref, what=f"nyquist {D}x{W}")
+    for d in range(D):
+        P.assert_parity(S[d], ref[d], what=f"nyquist dir {d}")
+    print(f"nyquist {D}x{W} nu={nu}: dead bins {int(dead.sum())}, relL2={l2:.2e} maxrel={mr:.2e}")
+
+
+def test_nyquist_linear_grid_regions_and_errors(oracle_mod):
+    from paper_2501_03383_b200 import binding
+    # a linear grid with the limiter on runs the general kernel (no recurrence variant)
+    w = wl.Workload("nyq", 1500, 2, 1e-17, wl.dirs_fibonacci(5), np.linspace(1e16, 9e17, 160), np.float32,
+                    wl.BASE_SEED + 51, "khi")
+    steps = list(w.steps())
+    off = np.array([0, 400, 1500], dtype=np.int64)
+    o = oracle_mod.RegionOracle(2, w.dirs, w.omega, w.dt, scale=1.0, nyquist=0.7)
+    for t, st in steps:
+        o.accumulate_step(t, off, *st)
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, n_regions=2, nyquist=0.7) as det:
+        for t, st in steps:
+            det.accumulate_step_regions(t, off, P.to_device(st))
+        assert det.kernel_variant == "general+nyquist"
+        for r in range(2):
+            P.assert_parity(det.spectrum()[r], o.spectrum()[r], what=f"nyquist region {r}")
+    with pytest.raises(binding.RadError, match="nyquist_factor"):
+        binding.Detector(w.dirs, w.omega, w.dt, nyquist=-1.0)
