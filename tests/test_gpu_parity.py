@@ -519,3 +519,37 @@ def test_nyquist_linear_grid_regions_and_errors(oracle_mod):
             P.assert_parity(det.spectrum()[r], o.spectrum()[r], what=f"nyquist region {r}")
     with pytest.raises(binding.RadError, match="nyquist_factor"):
         binding.Detector(w.dirs, w.omega, w.dt, nyquist=-1.0)
+
+
+@pytest.mark.parametrize("cfg,n", [("3c", 2000), ("4b", 6000), ("0", 256)])
+def test_calls_are_cuda_graph_capturable(oracle_mod, cfg, n):
+    """Steady-state calls (accumulate on device state, spectrum to a device buffer) do no
+    allocation and no synchronisation, so a caller can capture a block of steps in a CUDA graph
+    and replay it (the remedy for launch-bound small steps when the state is produced on the
+    fly); the replayed graph must give the oracle's spectrum."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    w = wl.make_workload(cfg)
+    steps = list(w.steps(n_steps=4, n_particles=n))
+    dev = [P.to_device(st) for _, st in steps]
+    out = torch.zeros(w.n_dir, w.n_omega, dtype=torch.float64, device="cuda")
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, state_dtype=w.state_dtype) as det:
+        det.accumulate_step(0, dev[0])          # warm-up outside the capture (lazy set-up paths)
+        det.spectrum(out=out)
+        det.reset()
+        torch.cuda.synchronize()
+        side = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(g, stream=side):
+                for i, (t, _) in enumerate(steps):
+                    det.accumulate_step(t, dev[i])
+                det.spectrum(out=out)
+        torch.cuda.synchronize()
+        det.reset()
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        S = out.cpu().numpy()
+    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    P.assert_parity(S, ref, what=f"graph replay cfg{cfg}")
