@@ -206,9 +206,6 @@ rad_status check_handle(rad_handle *hh)
     return RAD_OK;
 }
 
-// st: DEVICE arrays.  region_off == NULL: particles [0, n) of the one detector; else n_regions+1
-// HOST offsets into arrays whose element 0 is particle `region_base` of the caller's numbering
-// and n = particles spanned by the regions.
 // Multi-step calls: chunk table over (step, particle chunk), all folding into region 0.
 rad_status build_step_table(Handle &h, int n_steps, long long n, long long stride, int chunk, cudaStream_t s)
 {
@@ -228,6 +225,10 @@ rad_status build_step_table(Handle &h, int n_steps, long long n, long long strid
     return RAD_OK;
 }
 
+// st: DEVICE arrays.  region_off == NULL: particles [0, n) of the one detector; else n_regions+1
+// HOST offsets into arrays whose element 0 is particle `region_base` of the caller's numbering
+// and n = particles spanned by the regions.
+// n_steps > 1: step t of every array starts step_stride elements after step t-1.
 rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *const st[10], cudaStream_t s,
                              const int64_t *region_off = nullptr, long long region_base = 0,
                              int n_steps = 1, long long step_stride = 0)
