@@ -89,8 +89,9 @@ int choose_chunk(const Handle &h, long long n)
     auto blocks_at = [&](long long chunk) {
         return (h.n_wtiles * ((n + chunk - 1) / chunk) + kWarpsPerBlock - 1) / kWarpsPerBlock;
     };
-    if (blocks_at(256) >= 4 * cap) {  // large input: ~8 waves keep the tail of the grid small
-        const long long want_tasks = 8 * cap * kWarpsPerBlock;
+    if (blocks_at(256) >= 4 * cap) {  // large input: ~4 waves of full-length chunks; the tapered
+                                      // chunk table (build_tapered_table) evens out the tail
+        const long long want_tasks = 4 * cap * kWarpsPerBlock;
         const long long n_chunks = (want_tasks + h.n_wtiles - 1) / h.n_wtiles;
         long long chunk = (n + n_chunks - 1) / n_chunks;
         chunk = (chunk + kBatch - 1) / kBatch * kBatch;
@@ -225,6 +226,39 @@ rad_status build_step_table(Handle &h, int n_steps, long long n, long long strid
     return RAD_OK;
 }
 
+// Plain single-step calls on large inputs: tapered chunk table ("guided" schedule).  The grid is
+// ~8 waves of equal blocks; the last wave ends ragged while SMs idle.  Chunks keep the nominal
+// length until ~2 waves of work are left, then each takes 1/taper of what remains (down to 128
+// particles), so the blocks scheduled last are short and the tail of the grid is even.
+// Cached per (n, chunk): no upload in the steady state.
+rad_status build_tapered_table(Handle &h, long long n, int chunk, cudaStream_t s)
+{
+    if (h.tap_n == n && h.tap_chunk == chunk && h.reg_chunk == -1) return RAD_OK;
+    const long long gx = (h.n_wtiles + kWarpsPerBlock - 1) / kWarpsPerBlock;   // blocks per chunk
+    const double chunks_per_wave = (double)h.sm_count * kMinBlocks / (double)gx;
+    const double tk = getenv("RAD_TAPER_K") ? atof(getenv("RAD_TAPER_K")) : 1.0;
+    const long long tmin = getenv("RAD_TAPER_MIN") ? atoll(getenv("RAD_TAPER_MIN")) : 128;
+    const double taper = std::max(2.0, tk * chunks_per_wave);
+    std::vector<ChunkRec> recs;
+    long long k = 0;
+    while (k < n) {
+        long long len = std::min<long long>(chunk, (long long)((double)(n - k) / taper));
+        len = std::max<long long>(len, tmin) / kBatch * kBatch;
+        len = std::min(len, n - k);
+        recs.push_back(ChunkRec{k, (int)len, 0, 0, 0});
+        k += len;
+    }
+    rad_status st_cap = ensure_chunk_capacity(h, recs.size());
+    if (st_cap != RAD_OK) return st_cap;
+    std::copy(recs.begin(), recs.end(), h.chunks_h);
+    h.reg_n_chunks = (int)recs.size();
+    h.reg_chunk = -1; h.reg_offsets.clear();     // marks "tapered table on the device"
+    h.tap_n = n; h.tap_chunk = chunk;
+    RAD_CUDA(&h, cudaMemcpyAsync(h.chunks_d, h.chunks_h, recs.size() * sizeof(ChunkRec), cudaMemcpyHostToDevice, s));
+    RAD_CUDA(&h, cudaEventRecord(h.reg_uploaded, s));
+    return RAD_OK;
+}
+
 // st: DEVICE arrays.  region_off == NULL: particles [0, n) of the one detector; else n_regions+1
 // HOST offsets into arrays whose element 0 is particle `region_base` of the caller's numbering
 // and n = particles spanned by the regions.
@@ -274,6 +308,12 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
         if (n_chunks == 0) return RAD_OK;
     } else if (n_steps > 1) {
         rad_status st_ = build_step_table(h, n_steps, n, step_stride, p.chunk, s);
+        if (st_ != RAD_OK) return st_;
+        n_chunks = h.reg_n_chunks;
+        p.chunks = h.chunks_d;
+    } else if (!h.stream_nb && !h.deterministic && !getenv("RAD_NO_TAPER") &&
+               (long long)n_chunks * h.n_wtiles >= 4LL * h.sm_count * kMinBlocks * kWarpsPerBlock) {
+        rad_status st_ = build_tapered_table(h, n, p.chunk, s);
         if (st_ != RAD_OK) return st_;
         n_chunks = h.reg_n_chunks;
         p.chunks = h.chunks_d;

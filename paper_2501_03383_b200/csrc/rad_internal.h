@@ -160,6 +160,8 @@ struct Handle {
     std::vector<long long> reg_offsets;   // offsets of the table currently on the device
     int reg_chunk = 0, reg_n_chunks = 0, reg_steps = 1;
     long long reg_stride = 0;
+    long long tap_n = -1;                 // tapered plain-call table on the device: its n and chunk
+    int tap_chunk = 0;
     ChunkRec *chunks_h = nullptr, *chunks_d = nullptr;   // [reg_cap]
     int *reg_cstart_h = nullptr, *reg_cstart_d = nullptr; // [R+1] first chunk of each region
     size_t reg_cap = 0;
