@@ -553,3 +553,27 @@ def test_calls_are_cuda_graph_capturable(oracle_mod, cfg, n):
         S = out.cpu().numpy()
     ref = P.run_oracle(oracle_mod, w, steps).spectrum()
     P.assert_parity(S, ref, what=f"graph replay cfg{cfg}")
+
+
+def test_checkpoint_resume_through_amplitude_export(oracle_mod):
+    """SURVEY section 5 (checkpoint / resume): the whole state of a detector is its amplitude.
+    Export it after two steps (rad_amplitude to the host), start a fresh handle, import it
+    (rad_add_amplitude) and continue: same spectrum as the uninterrupted run and the oracle."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    w = wl.make_workload("3b")
+    steps = list(w.steps(n_steps=4, n_particles=1200))
+    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0) as a:
+        for t, st in steps[:2]:
+            a.accumulate_step(t, P.to_device(st))
+        ckpt = a.amplitude()                                  # numpy complex [D, W, 3] on the host
+    saved = np.stack([ckpt.real, ckpt.imag], axis=-1).copy()  # what a checkpoint file would hold
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0) as b:
+        b.add_amplitude(torch.from_numpy(saved).cuda())
+        for t, st in steps[2:]:
+            b.accumulate_step(t, P.to_device(st))
+        S_resumed = b.spectrum()
+    S_straight, _ = P.run_gpu(w, steps)
+    assert P.rel_l2(S_resumed, S_straight) < 1e-12 + 1e-7
+    P.assert_parity(S_resumed, ref, what="resumed run")
