@@ -293,6 +293,9 @@ def run_ours(args):
                     "frac": achieved / peak, "traffic": traffic,
                     "peak_how": f"{n_sm} SMs x {per_clk_sm:g} updates/clk/SM x {sm_max:.0f} MHz (max SM clock, "
                                 f"{peaks_src}); DESIGN.md section 5"}
+    if variant == "uniform":
+        # plain FFMA issues at 84-87 thread-instr/clk/SM on B200 (BASELINE.md note vii), not the nominal 128
+        roofline["frac_of_measured_ffma_rate"] = achieved / (n_sm * 87.0 / 8.0 * sm_max * 1e6 / 1e9)
     roofline.update({"kernel": f"rad_accum_{variant}", "kernel_ms": kernel_ms,
                      "algorithmic_bytes": int(bytes_per_step), "updates_per_launch": int(updates_per_step),
                      "gupdates_per_s": achieved, "hbm_gbs_achieved": hbm_achieved, "hbm_gbs_peak": hbm_peak})
