@@ -236,6 +236,11 @@ def make_workload(cfg: str) -> Workload:
     if cfg == "4b":
         return Workload("cfg4b_streaming_1x8", 16777216, 4, 1e-17, dirs_fibonacci(1),
                         omega_log(8), np.float32, BASE_SEED + 4, "khi")
+    if cfg == "1u":
+        # config 1 on a LINEAR frequency grid (not a BASELINE.json config): the shape on which the
+        # uniform-grid rotation-recurrence kernel (a2') is measured
+        return Workload("cfg1u_khi_linear_grid", 65536, 1000, 1e-17, dirs_fibonacci(128),
+                        omega_linear(512, 1e17), np.float32, BASE_SEED + 1, "khi")
     if cfg == "5r":
         # smallest KHI run = 192 x 256 x 12 cells x 9 particles per cell on 16
         # GPUs -> 331 776 particles per GPU; line 196: one ML sample = the ~3e4 particles of a
@@ -245,4 +250,4 @@ def make_workload(cfg: str) -> Workload:
     raise KeyError(cfg)
 
 
-ALL_CONFIGS = ("0", "1", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r")
+ALL_CONFIGS = ("0", "1", "1u", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r")
