@@ -577,3 +577,11 @@ def test_checkpoint_resume_through_amplitude_export(oracle_mod):
     S_straight, _ = P.run_gpu(w, steps)
     assert P.rel_l2(S_resumed, S_straight) < 1e-12 + 1e-7
     P.assert_parity(S_resumed, ref, what="resumed run")
+
+
+@pytest.mark.skipif(__import__("os").environ.get("RAD_SLOW") != "1",
+                    reason="~10 min: the whole production-like config; run with RAD_SLOW=1")
+def test_cfg2_full_workload_all_2000_steps(oracle_mod):
+    """BASELINE.json configs[2] in full (1 048 576 particles x 2000 steps x 256 x 1024 bins =
+    5.5e14 updates on the GPU); the oracle follows on 12 stratified bins (2.5e10 updates)."""
+    _full_size_sampled(oracle_mod, "2", 2000, n_dir=3, n_om=4)
