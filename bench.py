@@ -48,6 +48,7 @@ def parse_args():
     ap.add_argument("--particles", type=int, default=None, help="override particle count (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-overlap", action="store_true", help="create the detector without RAD_FLAG_OVERLAP_STEPS")
     return ap.parse_args()
 
 
@@ -207,12 +208,18 @@ def run_ours(args):
 
     R = w.n_regions
     off = w.region_offsets(n) if R > 1 else None
+    # RAD_FLAG_OVERLAP_STEPS: consecutive calls may overlap on the device (programmatic dependent
+    # launches).  Its contract -- a call's input arrays are complete when the call is made -- holds
+    # here: device-resident inputs are uploaded and synchronised before the timed region, host inputs
+    # reach the kernels through an event of the library's copy stream.
+    flags = 0 if args.no_overlap else binding.RAD_FLAG_OVERLAP_STEPS
     det = binding.Detector(w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0, state_dtype=w.state_dtype,
-                           device=local, n_regions=R if R > 1 else 0)
+                           device=local, n_regions=R if R > 1 else 0, flags=flags)
     spec_dev = torch.empty(R * w.n_dir, w.n_omega, dtype=torch.float64, device="cuda")
     if world > 1:
         det_glob = binding.Detector(w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0,
-                                    state_dtype=w.state_dtype, device=local, n_regions=R if R > 1 else 0)
+                                    state_dtype=w.state_dtype, device=local, n_regions=R if R > 1 else 0,
+                                    flags=flags)
         amp_buf = torch.empty(R * w.n_dir, w.n_omega, 3, 2, dtype=torch.float64, device="cuda")
 
     def accumulate(i, host=False):
@@ -378,6 +385,7 @@ def run_ours(args):
             "config": {"workload": w.name, "n_particles_per_gpu": n, "n_regions": R, "n_dir": w.n_dir,
                        "n_omega": w.n_omega,
                        "state_dtype": np.dtype(w.state_dtype).name, "parallelism": f"particle-shard x{world}",
+                       "flags": "none" if args.no_overlap else "RAD_FLAG_OVERLAP_STEPS",
                        "l2": f"ring of {ring} distinct step inputs ({ring * bytes_per_step / 2**20:.0f} MiB) + "
                              f"L2 flush before the timed region"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,

@@ -376,7 +376,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         return fail(nullptr, RAD_ERR_INVALID_ARG, "dt must be finite and > 0; t0, scale finite; scale >= 0");
     if (cfg->state_dtype != RAD_F32 && cfg->state_dtype != RAD_F64)
         return fail(nullptr, RAD_ERR_INVALID_ARG, "state_dtype must be RAD_F32 or RAD_F64");
-    if (cfg->flags & ~(RAD_FLAG_DETERMINISTIC | RAD_FLAG_FORCE_GENERAL))
+    if (cfg->flags & ~(RAD_FLAG_DETERMINISTIC | RAD_FLAG_FORCE_GENERAL | RAD_FLAG_OVERLAP_STEPS))
         return fail(nullptr, RAD_ERR_INVALID_ARG, "unknown flag bits");
     if (cfg->n_regions < 0) return fail(nullptr, RAD_ERR_INVALID_ARG, "n_regions must be >= 0");
     if (!std::isfinite(cfg->nyquist_factor) || cfg->nyquist_factor < 0.0)
@@ -408,6 +408,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     h.scale = cfg->scale == 0.0 ? default_scale() : cfg->scale;
     h.state_f64 = cfg->state_dtype == RAD_F64;
     h.deterministic = (cfg->flags & RAD_FLAG_DETERMINISTIC) != 0;
+    h.overlap = (cfg->flags & RAD_FLAG_OVERLAP_STEPS) != 0;
 
     // directions: normalise in fp64 (Q8), build e1, e2 with e1 x e2 = n
     h.dirs_h.resize((size_t)h.D * 3);

@@ -11,6 +11,12 @@ constexpr double kMagic = 6755399441055744.0;  // 1.5 * 2^52: fp64 round-to-inte
 constexpr float kTwoPi = 6.283185307179586f;
 constexpr float kUnitToRad = 1.4629180792671596e-09f;  // 2 pi / 2^32
 
+// Programmatic dependent launch (RAD_FLAG_OVERLAP_STEPS; no-ops in a normally launched grid):
+// pdl_trigger() lets the next kernel of the stream start once every block of this grid has
+// started; pdl_wait() blocks until all work queued before this grid has completed and is visible.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // state element -> fp64.  fp32 -> fp64 by integer ops (exponent re-bias) instead of F2F.F64.F32:
 // the conversion unit shares the XU pipe with MUFU.SIN/COS, the bound of the whole path, while
 // the integer pipe idles.  Exact for normal numbers; 0 maps to 2^-127 (5.9e-39, harmless: the

@@ -3,6 +3,7 @@
 // All fp64, one thread per (direction, frequency) bin; bandwidth-trivial (<= a few MB).
 // Per-region handles: "row" = region * D + direction runs over R*D rows; the basis of a row is
 // that of direction row mod D.
+#include "rad_device.cuh"
 #include "rad_internal.h"
 
 namespace rad {
@@ -14,6 +15,8 @@ namespace {
 __global__ void rad_spectrum_kernel(const double *__restrict__ acc, double *__restrict__ out,
                                     int D, int W, int w_pad, double scale)
 {
+    dev::pdl_trigger();
+    dev::pdl_wait();  // A belongs to the accumulate kernels queued before
     const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= (long long)D * W) return;
     const int d = (int)(b / W), j = (int)(b - (long long)d * W);
@@ -27,6 +30,8 @@ __global__ void rad_amplitude_kernel(const double *__restrict__ acc, const DirRe
                                      const double *__restrict__ basis, double *__restrict__ out,
                                      int rows, int D, int W, int w_pad)
 {
+    dev::pdl_trigger();
+    dev::pdl_wait();  // A belongs to the accumulate kernels queued before
     const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= (long long)rows * W) return;
     const int d = (int)(b / W), j = (int)(b - (long long)d * W);
@@ -82,6 +87,8 @@ __global__ void rad_reduce_partials_kernel(double *__restrict__ acc, const doubl
 __global__ void rad_spectrum_total_kernel(const double *__restrict__ acc, double *__restrict__ out,
                                           int R, int D, int W, int w_pad, double scale)
 {
+    dev::pdl_trigger();
+    dev::pdl_wait();  // A belongs to the accumulate kernels queued before
     const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= (long long)D * W) return;
     const int d = (int)(b / W), j = (int)(b - (long long)d * W);
@@ -101,16 +108,15 @@ inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) /
 cudaError_t launch_spectrum(const Handle &h, double *out_dev, cudaStream_t s)
 {
     const long long n = (long long)h.R * h.D * h.W;
-    rad_spectrum_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, out_dev, h.R * h.D, h.W, h.w_pad, h.scale);
-    return cudaGetLastError();
+    return launch_kernel(rad_spectrum_kernel, dim3(blocks_for(n, 256)), dim3(256), 0, s, h.overlap, h.acc_d, out_dev,
+                         h.R * h.D, h.W, h.w_pad, h.scale);
 }
 
 cudaError_t launch_amplitude(const Handle &h, double *out_dev, cudaStream_t s)
 {
     const long long n = (long long)h.R * h.D * h.W;
-    rad_amplitude_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, h.dirs_d, h.basis_d, out_dev,
-                                                            h.R * h.D, h.D, h.W, h.w_pad);
-    return cudaGetLastError();
+    return launch_kernel(rad_amplitude_kernel, dim3(blocks_for(n, 256)), dim3(256), 0, s, h.overlap, h.acc_d,
+                         h.dirs_d, h.basis_d, out_dev, h.R * h.D, h.D, h.W, h.w_pad);
 }
 
 cudaError_t launch_add_amplitude(const Handle &h, const double *amp_dev, cudaStream_t s)
@@ -134,9 +140,8 @@ cudaError_t launch_reduce_partials(const Handle &h, const double *partial, int n
 cudaError_t launch_spectrum_total(const Handle &h, double *out_dev, cudaStream_t s)
 {
     const long long n = (long long)h.D * h.W;
-    rad_spectrum_total_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, out_dev, h.R, h.D, h.W, h.w_pad,
-                                                                 h.scale);
-    return cudaGetLastError();
+    return launch_kernel(rad_spectrum_total_kernel, dim3(blocks_for(n, 256)), dim3(256), 0, s, h.overlap, h.acc_d,
+                         out_dev, h.R, h.D, h.W, h.w_pad, h.scale);
 }
 
 }  // namespace rad

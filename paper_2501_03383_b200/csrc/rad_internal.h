@@ -104,6 +104,22 @@ struct AccumParams {
 
 struct Handle;
 
+// Kernel launch, optionally with programmatic stream serialization (RAD_FLAG_OVERLAP_STEPS):
+// the grid may start while its predecessor in the stream drains; the kernels call
+// dev::pdl_wait() before they touch memory that earlier work writes.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_kernel(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
+                                 bool overlap, Args &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = overlap ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
 // kernels/launchers (rad_kernels.cu, rad_finalize.cu)
 cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_f64,
                               cudaStream_t s, int *n_launches, const char **variant);
@@ -133,6 +149,7 @@ struct Handle {
     int win_type = 0;
     double win_o[3] = {0, 0, 0}, win_il[3] = {0, 0, 0};
     bool state_f64 = false, deterministic = false, uniform = false;
+    bool overlap = false;            // RAD_FLAG_OVERLAP_STEPS
     uint32_t rot_G = 0;              // uniform grid: rotator frequency LW*df in f_unit units
     float rot_Gf = 0, rot_gl = 0;
     int sm_count = 148;

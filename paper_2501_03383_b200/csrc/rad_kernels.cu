@@ -111,6 +111,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
     int wt, ci, region;
     long long k0, k1;
     double ts32;
+    pdl_trigger();
     if (!decode_task(P, warp, wt, ci, k0, k1, region, ts32)) return;  // whole warp leaves; no block barrier below
     const int dg = wt / P.n_ftiles, ft = wt - dg * P.n_ftiles;
     const int ld = lane / LW, lf = lane - ld * LW;
@@ -231,28 +232,28 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
         }
         __syncwarp();
     }
+    pdl_wait();  // the accumulator (and the deterministic workspace) belong to earlier work until here
     fold<S, LW>(P, acc, dg * DPW + ld, jbase, ci, region);
 }
 
 // ------------------------------------------------------------------------------------------
 // Launch logic.
 template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ>
-static cudaError_t launch_one(const AccumParams &p, cudaStream_t s)
+static cudaError_t launch_one(const AccumParams &p, cudaStream_t s, bool overlap)
 {
     const long long n_tasks = (long long)p.n_wtiles * p.n_chunks;
     const unsigned grid = (unsigned)((n_tasks + kWarpsPerBlock - 1) / kWarpsPerBlock);
-    rad_accum<ST, LW, S, MINB, UNI, NYQ><<<grid, kThreads, 0, s>>>(p);
-    return cudaGetLastError();
+    return launch_kernel(rad_accum<ST, LW, S, MINB, UNI, NYQ>, dim3(grid), dim3(kThreads), 0, s, overlap, p);
 }
 
 template <typename ST, bool UNI, bool NYQ>
 static cudaError_t dispatch(const Handle &h, const AccumParams &p, cudaStream_t s)
 {
     switch (h.lw) {
-        case 32: return launch_one<ST, 32, kStrip, kMinBlocks, UNI, NYQ>(p, s);
-        case 16: return launch_one<ST, 16, kStrip, kMinBlocks, UNI, NYQ>(p, s);
-        case 8: return launch_one<ST, 8, kStrip, kMinBlocks, UNI, NYQ>(p, s);
-        default: return launch_one<ST, 4, kStrip, kMinBlocks, UNI, NYQ>(p, s);
+        case 32: return launch_one<ST, 32, kStrip, kMinBlocks, UNI, NYQ>(p, s, h.overlap);
+        case 16: return launch_one<ST, 16, kStrip, kMinBlocks, UNI, NYQ>(p, s, h.overlap);
+        case 8: return launch_one<ST, 8, kStrip, kMinBlocks, UNI, NYQ>(p, s, h.overlap);
+        default: return launch_one<ST, 4, kStrip, kMinBlocks, UNI, NYQ>(p, s, h.overlap);
     }
 }
 

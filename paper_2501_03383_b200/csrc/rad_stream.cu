@@ -107,6 +107,7 @@ __global__ void __launch_bounds__(kSThreads, NB <= 8 ? RAD_S_MINB : 1) rad_accum
     __shared__ float s_red[kSThreads / 32][NB * 4];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    pdl_trigger();
     float acc[NB][4];
 #pragma unroll
     for (int b = 0; b < NB; ++b) acc[b][0] = acc[b][1] = acc[b][2] = acc[b][3] = 0.0f;
@@ -197,6 +198,7 @@ __global__ void __launch_bounds__(kSThreads, NB <= 8 ? RAD_S_MINB : 1) rad_accum
             if (lane == 0) s_red[warp][b * 4 + c] = v;
         }
     __syncthreads();
+    pdl_wait();  // the accumulator belongs to earlier work until here
     if (tid < NB * 4) {
         const int b = tid >> 2, c = tid & 3;
         const int d = b / WB, j = b - d * WB;
@@ -214,7 +216,7 @@ __global__ void __launch_bounds__(kSThreads, NB <= 8 ? RAD_S_MINB : 1) rad_accum
 }
 
 template <typename ST, int NB, int ND, bool WIN>
-cudaError_t launch_stream_w(const AccumParams &p, int grid, cudaStream_t s)
+cudaError_t launch_stream_w(const AccumParams &p, int grid, cudaStream_t s, bool overlap)
 {
     const size_t smem = (size_t)kSStages * 10 * kSTileBytes;
     // per device and per template instance; the call is a cheap host-side set, so no caching
@@ -224,22 +226,21 @@ cudaError_t launch_stream_w(const AccumParams &p, int grid, cudaStream_t s)
     int use_bulk = getenv("RAD_STREAM_PLAIN") ? 0 : 1;  // debug: force the plain-load path
     for (int a = 0; a < 10; ++a)
         if (reinterpret_cast<uintptr_t>(p.st[a]) & 15) use_bulk = 0;
-    rad_accum_stream<ST, NB, ND, WIN><<<grid, kSThreads, smem, s>>>(p, use_bulk);
-    return cudaGetLastError();
+    return launch_kernel(rad_accum_stream<ST, NB, ND, WIN>, dim3(grid), dim3(kSThreads), smem, s, overlap, p, use_bulk);
 }
 
 template <typename ST, int NB, int ND>
-cudaError_t launch_stream_t(const AccumParams &p, int grid, cudaStream_t s)
+cudaError_t launch_stream_t(const AccumParams &p, int grid, cudaStream_t s, bool overlap)
 {
-    return p.win_type != RAD_WINDOW_NONE ? launch_stream_w<ST, NB, ND, true>(p, grid, s)
-                                         : launch_stream_w<ST, NB, ND, false>(p, grid, s);
+    return p.win_type != RAD_WINDOW_NONE ? launch_stream_w<ST, NB, ND, true>(p, grid, s, overlap)
+                                         : launch_stream_w<ST, NB, ND, false>(p, grid, s, overlap);
 }
 
 template <typename ST>
 cudaError_t dispatch_stream(const Handle &h, const AccumParams &p, int grid, cudaStream_t s)
 {
-    if (h.stream_nb == 8) return h.stream_nd == 1 ? launch_stream_t<ST, 8, 1>(p, grid, s) : launch_stream_t<ST, 8, 2>(p, grid, s);
-    return h.stream_nd == 1 ? launch_stream_t<ST, 16, 1>(p, grid, s) : launch_stream_t<ST, 16, 2>(p, grid, s);
+    if (h.stream_nb == 8) return h.stream_nd == 1 ? launch_stream_t<ST, 8, 1>(p, grid, s, h.overlap) : launch_stream_t<ST, 8, 2>(p, grid, s, h.overlap);
+    return h.stream_nd == 1 ? launch_stream_t<ST, 16, 1>(p, grid, s, h.overlap) : launch_stream_t<ST, 16, 2>(p, grid, s, h.overlap);
 }
 
 }  // namespace

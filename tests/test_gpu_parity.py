@@ -585,3 +585,49 @@ def test_cfg2_full_workload_all_2000_steps(oracle_mod):
     """BASELINE.json configs[2] in full (1 048 576 particles x 2000 steps x 256 x 1024 bins =
     5.5e14 updates on the GPU); the oracle follows on 12 stratified bins (2.5e10 updates)."""
     _full_size_sampled(oracle_mod, "2", 2000, n_dir=3, n_om=4)
+
+
+@pytest.mark.parametrize("cfg,n", [("5r", 40000), ("3c", 9000), ("4b", 50000), ("0", 256), ("3d", 3000)])
+def test_overlap_steps_flag_keeps_every_intermediate_spectrum(oracle_mod, cfg, n):
+    """RAD_FLAG_OVERLAP_STEPS (programmatic dependent launches): kernels of consecutive calls
+    overlap, so the spectrum taken after step i must still contain steps 0..i and nothing of
+    step i+1 (the accumulate kernels wait before their fold, the result kernels before they
+    read A).  Every intermediate spectrum is compared with a run without the flag, the last one
+    with the oracle; many short steps back to back make the overlap real."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    w = wl.make_workload(cfg)
+    T = 12
+    steps = list(w.steps(n_steps=T, n_particles=n))
+    dev = [P.to_device(st) for _, st in steps]
+    R = w.n_regions
+    off = w.region_offsets(n) if R > 1 else None
+
+    def run(flags):
+        outs = [torch.zeros(R * w.n_dir, w.n_omega, dtype=torch.float64, device="cuda") for _ in range(T)]
+        with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, state_dtype=w.state_dtype, flags=flags,
+                              n_regions=R if R > 1 else 0) as det:
+            for rep in range(2):                      # second pass: everything warm, launches back to back
+                det.reset()
+                for i, (t, _) in enumerate(steps):
+                    if R > 1:
+                        det.accumulate_step_regions(t, off, dev[i])
+                    else:
+                        det.accumulate_step(t, dev[i])
+                    det.spectrum(out=outs[i])
+            torch.cuda.synchronize()
+        return [o.cpu().numpy() for o in outs]
+
+    plain, over = run(0), run(binding.RAD_FLAG_OVERLAP_STEPS)
+    for i in range(T):
+        assert np.allclose(over[i], plain[i], rtol=1e-9, atol=1e-12 * plain[-1].max()), f"step {i}"
+    if R > 1:
+        o = oracle_mod.RegionOracle(R, w.dirs, w.omega, w.dt, scale=1.0)
+        for t, st in steps:
+            o.accumulate_step(t, off, *st)
+        ref = o.spectrum().reshape(R * w.n_dir, w.n_omega)
+    else:
+        ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    for r in range(R):
+        sl = slice(r * w.n_dir, (r + 1) * w.n_dir)
+        P.assert_parity(over[-1][sl], ref[sl], what=f"overlap cfg{cfg} region {r}")
