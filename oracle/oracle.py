@@ -45,7 +45,8 @@ def _load():
             + [ctypes.c_void_p] * 10
             + [ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p])
         lib.oracle_accumulate_step_w.restype = ctypes.c_int
-        lib.oracle_accumulate_step_w.argtypes = lib.oracle_accumulate_step.argtypes + [ctypes.c_int, ctypes.c_void_p]
+        lib.oracle_accumulate_step_w.argtypes = (lib.oracle_accumulate_step.argtypes
+                                                 + [ctypes.c_int, ctypes.c_void_p, ctypes.c_double])
         lib.oracle_accumulate_step_regions.restype = ctypes.c_int
         lib.oracle_accumulate_step_regions.argtypes = (
             [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p,
@@ -55,9 +56,7 @@ def _load():
             + [ctypes.c_longlong, ctypes.c_void_p, ctypes.c_void_p])
         lib.oracle_accumulate_step_regions_w.restype = ctypes.c_int
         lib.oracle_accumulate_step_regions_w.argtypes = (lib.oracle_accumulate_step_regions.argtypes
-                                                         + [ctypes.c_int, ctypes.c_void_p])
-        lib.oracle_set_nyquist.restype = None
-        lib.oracle_set_nyquist.argtypes = [ctypes.c_double]
+                                                         + [ctypes.c_int, ctypes.c_void_p, ctypes.c_double])
         lib.oracle_spectrum.restype = ctypes.c_int
         lib.oracle_spectrum.argtypes = [ctypes.c_longlong, ctypes.c_void_p, ctypes.c_double,
                                         ctypes.c_void_p]
@@ -115,12 +114,11 @@ class Oracle:
             raise ValueError("state arrays must be 1-D and of equal length")
         nb = 0 if self.bins is None else self.bins.shape[0]
         bp = None if self.bins is None else self.bins.ctypes.data
-        _load().oracle_set_nyquist(self.nyquist)
         rc = _load().oracle_accumulate_step_w(
             self.D, self.dirs.ctypes.data, self.W, self.omega.ctypes.data, self.dt, self.t0,
             int(step_index), n, int(dt0 == np.dtype(np.float32)),
             *[a.ctypes.data for a in arrs], nb, bp, self.A.ctypes.data,
-            self.win_type, None if self.win is None else self.win.ctypes.data)
+            self.win_type, None if self.win is None else self.win.ctypes.data, self.nyquist)
         if rc != 0:
             raise ValueError("oracle_accumulate_step: bad argument")
 
@@ -168,12 +166,11 @@ class RegionOracle:
             raise ValueError("state arrays must be 1-D, of equal length >= offsets[-1]")
         nb = 0 if self.bins is None else self.bins.shape[0]
         bp = None if self.bins is None else self.bins.ctypes.data
-        _load().oracle_set_nyquist(self.nyquist)
         rc = _load().oracle_accumulate_step_regions_w(
             self.D, self.dirs.ctypes.data, self.W, self.omega.ctypes.data, self.dt, self.t0,
             int(step_index), self.R, offsets.ctypes.data, int(dt0 == np.dtype(np.float32)),
             *[a.ctypes.data for a in arrs], nb, bp, self.A.ctypes.data,
-            self.win_type, None if self.win is None else self.win.ctypes.data)
+            self.win_type, None if self.win is None else self.win.ctypes.data, self.nyquist)
         if rc != 0:
             raise ValueError("oracle_accumulate_step_regions: bad argument")
 

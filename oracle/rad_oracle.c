@@ -59,7 +59,7 @@
  * the trajectory, is sampled fewer than 2/nu times per period.  Pins: nu = 0 and nu = huge change
  * nothing; a static particle loses exactly the bins w_j dt >= pi nu; the cut-off of a moving
  * particle is Doppler shifted by direction; kept bins equal the closed forms.
- * (oracle_set_nyquist() sets nu for the calls that follow; 0 = off.)
+ * (nu is the last argument of the _w entry points; 0 = off.)
  */
 #include <math.h>
 #include <stddef.h>
@@ -97,9 +97,6 @@ static void cross3(const double a[3], const double b[3], double out[3])
     out[2] = a[0] * b[1] - a[1] * b[0];
 }
 
-static double g_nyquist = 0.0; /* nu of the Nyquist limiter, 0 = off (test-infrastructure state) */
-void oracle_set_nyquist(double nu) { g_nyquist = nu; }
-
 /* w1(u) of the spatial window, see the header. */
 static double window_1d(int type, double u)
 {
@@ -121,6 +118,7 @@ static double window_1d(int type, double u)
  *          selected bins are touched)
  *   win_type 0 none / 1 triangle / 2 Hamming; win = {o_x, o_y, o_z, L_x, L_y, L_z} (NULL or
  *          type 0: no window; L_c <= 0: axis c not windowed)
+ *   nyquist nu of the Nyquist limiter (0: off)
  * Returns 0, or 1 on a bad argument.
  */
 int oracle_accumulate_step_w(int n_dir, const double *dirs, int n_omega, const double *omega,
@@ -129,12 +127,12 @@ int oracle_accumulate_step_w(int n_dir, const double *dirs, int n_omega, const d
                              const void *bx, const void *by, const void *bz, const void *bdx,
                              const void *bdy, const void *bdz, const void *w,
                              long long n_bins, const long long *bin_idx, double *A,
-                             int win_type, const double *win)
+                             int win_type, const double *win, double nyquist)
 {
     if (n_dir <= 0 || n_omega <= 0 || !dirs || !omega || !A || n_part < 0) return 1;
     const long long total = bin_idx ? n_bins : (long long)n_dir * n_omega;
     const double t_step = t0 + (double)step_index * dt;
-    const double nyq_lim = 3.14159265358979323846 * g_nyquist;
+    const double nyq_lim = 3.14159265358979323846 * nyquist; /* pi nu; 0 = limiter off */
 
 #define LOAD(p, k) (is_f32 ? (double)((const float *)(p))[k] : ((const double *)(p))[k])
 
@@ -188,7 +186,7 @@ int oracle_accumulate_step(int n_dir, const double *dirs, int n_omega, const dou
                            long long n_bins, const long long *bin_idx, double *A)
 {
     return oracle_accumulate_step_w(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_part, is_f32, rx, ry,
-                                    rz, bx, by, bz, bdx, bdy, bdz, w, n_bins, bin_idx, A, 0, NULL);
+                                    rz, bx, by, bz, bdx, bdy, bdz, w, n_bins, bin_idx, A, 0, NULL, 0.0);
 }
 
 /*
@@ -205,7 +203,8 @@ int oracle_accumulate_step_regions_w(int n_dir, const double *dirs, int n_omega,
                                      const void *ry, const void *rz, const void *bx, const void *by,
                                      const void *bz, const void *bdx, const void *bdy,
                                      const void *bdz, const void *w, long long n_bins,
-                                     const long long *bin_idx, double *A, int win_type, const double *win)
+                                     const long long *bin_idx, double *A, int win_type, const double *win,
+                                     double nyquist)
 {
     if (n_regions <= 0 || !offsets || offsets[0] < 0) return 1;
     for (long long r = 0; r < n_regions; ++r)
@@ -218,7 +217,7 @@ int oracle_accumulate_step_regions_w(int n_dir, const double *dirs, int n_omega,
         const int rc = oracle_accumulate_step_w(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_r,
                                                 is_f32, AT(rx, k0), AT(ry, k0), AT(rz, k0), AT(bx, k0),
                                                 AT(by, k0), AT(bz, k0), AT(bdx, k0), AT(bdy, k0),
-                                                AT(bdz, k0), AT(w, k0), n_bins, bin_idx, A_r, win_type, win);
+                                                AT(bdz, k0), AT(w, k0), n_bins, bin_idx, A_r, win_type, win, nyquist);
         if (rc != 0) return rc;
     }
 #undef AT
@@ -235,7 +234,7 @@ int oracle_accumulate_step_regions(int n_dir, const double *dirs, int n_omega, c
 {
     return oracle_accumulate_step_regions_w(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_regions, offsets,
                                             is_f32, rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w, n_bins, bin_idx, A,
-                                            0, NULL);
+                                            0, NULL, 0.0);
 }
 
 /* S[n][j] = scale * sum_c |A_c|^2 ; scale == 0 -> SI default (Q4). */
