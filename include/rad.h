@@ -84,7 +84,8 @@ typedef enum { RAD_F32 = 0, RAD_F64 = 1 } rad_dtype;
  * or by work on another stream that cuda_stream waits for through an event (as the *_host
  * entry points do internally), not by a kernel queued on cuda_stream directly before the call.
  * Worth 1 % on steps of several 1e9 updates and up to 25 % on steps that fill the GPU only
- * once (a few 1e8 updates). */
+ * once (a few 1e8 updates).  Combines with RAD_FLAG_DETERMINISTIC (results stay bit-identical);
+ * not exercised under CUDA stream capture (capture handles without this flag). */
 
 typedef struct {
     uint32_t struct_size;  /* = sizeof(rad_config); ABI versioning                         */
