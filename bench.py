@@ -1,13 +1,17 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the radiation-detector hot path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path over one PIC step of synthetic input:
 rad_accumulate_step (stage + accumulate + fold) followed by
 rad_spectrum (a4).  Metric (BASELINE.json): particle*direction*frequency updates per second,
-in G/s, whole job.  Default workload = BASELINE.json configs[1] ("KHI-like shear", 65 536
-electrons x 128 directions x 512 log-spaced frequencies, fp32 state).
+in G/s, whole job.  Headline workload = BASELINE.json configs[2] ("production-like": 1 048 576
+electrons x 256 directions x 1024 log-spaced frequencies, fp32 state), the largest single-GPU
+configuration.  The same invocation also runs short legs of every other configuration (1, 3a-d,
+4, 4b, 5r, 0, 1u) and reports them under "configs", runs the pipe microbenchmarks
+(librad_ubench.so) and reports the measured ALU peaks under "alu_peaks", and compares the
+spectrum left by the timed region with the fp64 oracle on sampled bins ("parity").
 
 `--impl reference` times the fp64 CPU oracle (oracle/) as it stands on the host cores, on a
 bounded sample of the same workload (the paper has no code to install: DESIGN.md).
@@ -33,21 +37,30 @@ from paper_2501_03383_b200 import workloads as wl  # noqa: E402
 
 METRIC = "particle*direction*frequency updates/sec"
 UNIT = "Gupdates/s"
-MUFU_LANES_PER_SM = 16      # B200_PROFILING / microbenchmark: 16 MUFU results per clk per SM
+HEADLINE = "2"
+# nominal pipe widths per SM per clock (B200: 4 sub-partitions x 4 MUFU lanes, x 32 FP32 lanes);
+# the measured rates come from the microbenchmarks ("alu_peaks")
+MUFU_LANES_PER_SM = 16
+FP32_LANES_PER_SM = 128
 MUFU_PER_UPDATE = 2         # sin + cos: no recurrence exists on a non-uniform grid
+FP32_PER_UPDATE_UNIFORM = 8  # 4 (complex rotation) + 4 (accumulate) FMA-pipe instructions
 L2_BYTES = 126 * 2 ** 20
+# short legs run after the headline: (config, timed steps, warm-up steps)
+LEGS = (("1", 20, 3), ("3a", 10, 3), ("3b", 10, 3), ("3c", 10, 3), ("3d", 10, 3), ("4", 3, 1), ("4b", 20, 3),
+        ("5r", 30, 5), ("0", 50, 5), ("1u", 20, 3))
 
 
 def parse_args():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", default="1", choices=wl.ALL_CONFIGS)
+    ap.add_argument("--config", default=HEADLINE, choices=wl.ALL_CONFIGS)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--particles", type=int, default=None, help="override particle count (debug)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-legs", action="store_true", help="headline configuration only")
     ap.add_argument("--no-overlap", action="store_true", help="create the detector without RAD_FLAG_OVERLAP_STEPS")
     return ap.parse_args()
 
@@ -63,9 +76,9 @@ def measured_peaks():
 
 
 class ClockSampler(threading.Thread):
-    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+    """Samples SM clock and throttle reasons through NVML while a timed region runs."""
 
-    def __init__(self, index: int, period: float = 0.05):
+    def __init__(self, index: int, period: float = 0.005):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.reasons, self.max_mhz = [], set(), None
@@ -109,7 +122,21 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
-# ------------------------------------------------------------------------- oracle timing
+# ------------------------------------------------------------------------- oracle legs
+def oracle_for(w, bins):
+    from oracle import oracle
+    if w.n_regions > 1:
+        return oracle.RegionOracle(w.n_regions, w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=bins)
+    return oracle.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=bins)
+
+
+def oracle_step(o, w, step_index, state, n):
+    if w.n_regions > 1:
+        o.accumulate_step(step_index, w.region_offsets(n), *state)
+    else:
+        o.accumulate_step(step_index, *state)
+
+
 def time_oracle(w, state, n_bins_target=None, budget_s=15.0):
     """Oracle rate (updates/s) on one PIC step of `state`, all particles, a bin subset sized
     for about `budget_s` seconds (or exactly n_bins_target bins).  -> (rate, seconds, bins)."""
@@ -119,15 +146,9 @@ def time_oracle(w, state, n_bins_target=None, budget_s=15.0):
 
     def run(nb):
         bins = np.unique(np.linspace(0, total - 1, nb).round().astype(np.int64))
-        if w.n_regions > 1:       # per-region detectors: every particle feeds its own region's bins
-            o = oracle.RegionOracle(w.n_regions, w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=bins)
-            off = w.region_offsets(n)
-            t0 = time.perf_counter()
-            o.accumulate_step(0, off, *state)
-        else:
-            o = oracle.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=bins)
-            t0 = time.perf_counter()
-            o.accumulate_step(0, *state)
+        o = oracle_for(w, bins)
+        t0 = time.perf_counter()
+        oracle_step(o, w, 0, state, n)
         dt = time.perf_counter() - t0
         return bins.shape[0] * n / dt, dt, bins.shape[0]
 
@@ -136,6 +157,30 @@ def time_oracle(w, state, n_bins_target=None, budget_s=15.0):
         rate, _, _ = run(min(total, max(cores * 2, 16)))       # calibration
         n_bins_target = int(min(total, max(cores, rate * budget_s / max(n, 1))))
     return run(max(1, n_bins_target))
+
+
+def parity_vs_oracle(w, n, host_states, ring, n_steps_done, S_gpu, budget_updates=1.5e9):
+    """The spectrum the timed region left on the device (steps 0 .. n_steps_done-1, step i fed with
+    ring state i % ring) against the oracle on a stratified bin sample + the GPU arg-max bin;
+    north_star's two error measures.  Runs outside every timed region."""
+    total = w.n_regions * w.n_dir * w.n_omega
+    per_bin = n * n_steps_done
+    nb = int(max(4, min(64, budget_updates // max(per_bin, 1))))
+    DW = w.n_dir * w.n_omega
+    bins = np.unique(np.concatenate([np.linspace(0, DW - 1, nb).round().astype(np.int64),
+                                     [int(np.argmax(S_gpu.reshape(-1, DW).max(axis=0)))]]))
+    o = oracle_for(w, bins)
+    for i in range(n_steps_done):
+        oracle_step(o, w, i, [np.asarray(a) for a in host_states[i % ring]], n)
+    ref = o.spectrum().reshape(-1, DW)[:, bins].ravel()
+    got = S_gpu.reshape(-1, DW)[:, bins].ravel()
+    den = float(np.linalg.norm(ref))
+    rel_l2 = float(np.linalg.norm(got - ref) / den) if den > 0 else float(np.linalg.norm(got))
+    m = ref >= 1e-6 * float(S_gpu.max())
+    maxrel = float(np.max(np.abs(got[m] - ref[m]) / ref[m])) if m.any() else 0.0
+    return {"relL2": rel_l2, "maxrel": maxrel, "bins": int(bins.shape[0] * w.n_regions), "of_bins": int(total),
+            "steps": int(n_steps_done), "tolerance": {"relL2": 1e-4, "maxrel": 1e-3},
+            "ok": bool(rel_l2 <= 1e-4 and maxrel <= 1e-3 and np.isfinite(got).all())}
 
 
 def run_reference(args):
@@ -167,42 +212,75 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": el / max(args.steps, 1) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": {"workload": w.name, "n_particles": n, "n_regions": w.n_regions,
-                                        "n_dir": w.n_dir, "n_omega": w.n_omega,
-                                        "state_dtype": np.dtype(w.state_dtype).name},
+        "data": "synthetic", "config": workload_config(w, n, 1, None, None),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
 
 
+def workload_config(w, n, world, flags, l2):
+    """The `config` object: the same keys in both arms (the reference arm leaves the GPU-only ones null)."""
+    return {"workload": w.name, "n_particles_per_gpu": n, "n_regions": w.n_regions, "n_dir": w.n_dir,
+            "n_omega": w.n_omega, "state_dtype": np.dtype(w.state_dtype).name,
+            "parallelism": f"particle-shard x{world}", "flags": flags, "l2": l2}
+
+
 # ------------------------------------------------------------------------------ our arm
-def run_ours(args):
+_state_cache = {}
+
+
+def host_states_for(w, n, ring):
+    """Ring of `ring` consecutive PIC steps of workload w (numpy); workloads that share a
+    generator (the four sweep shapes; configs 4 and 4b) share the arrays."""
+    key = (w.kind, w.seed, n, w.dt, np.dtype(w.state_dtype).name, repr(sorted(w.extra.items())))
+    have = _state_cache.get(key, [])
+    if len(have) < ring:
+        have = [st for _, st in w.steps(n_steps=ring, n_particles=n)]
+        _state_cache.clear()                     # one generator's arrays at a time (config 4: 0.7 GB per step)
+        _state_cache[key] = have
+    return have[:ring]
+
+
+def alu_peaks(device, sm_mhz_hint):
+    """Pipe microbenchmarks (librad_ubench.so): measured results per clock per SM."""
+    from paper_2501_03383_b200 import ubench
+    res = ubench.run_all(device, blocks_per_sm=4, reps=3)
+    g = lambda k: res[k]["per_clk_sm"]      # noqa: E731
+    return {
+        "mufu_per_clk_sm": g("mufu_ex2"), "sin_per_clk_sm": g("mufu_sin"),
+        "sincos_pairs_per_clk_sm": g("sincos_pairs"), "ffma_per_clk_sm": g("ffma"),
+        "ffma_imm_per_clk_sm": g("ffma_imm"), "ffma2_instr_per_clk_sm": g("ffma2_instr"),
+        "ffma2_fma_per_clk_sm": 2.0 * g("ffma2_instr"), "dfma_per_clk_sm": g("dfma"),
+        "f2f_f32_from_f64_per_clk_sm": g("f2f_f32_from_f64"), "f2f_f64_from_f32_per_clk_sm": g("f2f_f64_from_f32"),
+        "imad_per_clk_sm": g("imad"),
+        "sincos_pairs_gops": res["sincos_pairs"]["gops"], "ffma_gops": res["ffma"]["gops"],
+        "sm_mhz": sm_mhz_hint,
+        "how": "librad_ubench.so (csrc/rad_ubench.cu): 8 independent chains per thread, 4 x 256 threads per SM; "
+               "per_clk_sm from clock64() inside the kernel, gops from CUDA events",
+    }
+
+
+def measure(cfg, K, W, args, ctx, headline):
+    """One leg: W warm-up + K timed steps (accumulate + spectrum) of workload `cfg`, the accumulate
+    kernel alone, parity of the spectrum left behind; the headline leg adds multi-step and e2e."""
     import torch
     import torch.distributed as dist
-    from paper_2501_03383_b200 import binding, build as rad_build, multi
+    from paper_2501_03383_b200 import binding, multi
+    rank, world, local = ctx["rank"], ctx["world"], ctx["local"]
+    peaks, peaks_src, peaks_alu = ctx["peaks"], ctx["peaks_src"], ctx["alu_peaks"]
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    rad_build.build()
-    peaks, peaks_src = measured_peaks()
-
-    w = wl.make_workload(args.config)
+    w = wl.make_workload(cfg)
     w.seed += 1000 * rank                       # weak scaling: every rank owns its own particles
-    n = args.particles or w.n_particles
-    K, W = args.steps, args.warmup
-    bytes_per_step = n * 10 * np.dtype(w.state_dtype).itemsize
-    # ring of distinct step inputs, larger than L2 so that no timed step finds its input cached
-    ring = min(max(K + W, 1), w.n_steps, max(8, int(2 * L2_BYTES // bytes_per_step) + 1), 256)
-    host_states = []
-    for t, st in w.steps(n_steps=ring, n_particles=n):
-        host_states.append([torch.from_numpy(a).pin_memory() for a in st])
+    n = (args.particles if headline else None) or w.n_particles
+    esz = np.dtype(w.state_dtype).itemsize
+    bytes_per_step = n * 10 * esz
+    # ring of distinct step inputs: either every step of the leg has its own input (read once, after
+    # the L2 flush that precedes the timed region), or the ring is more than twice the L2
+    ring = int(min(max(K + W, 1), w.n_steps, max(2, 2 * L2_BYTES // bytes_per_step + 1), 256))
+    states_np = host_states_for(w, n, ring)
+    pin = headline and not args.no_e2e
+    host_states = [[torch.from_numpy(a).pin_memory() if pin else torch.from_numpy(a) for a in st] for st in states_np]
     dev_states = [[a.cuda(non_blocking=True) for a in st] for st in host_states]
     torch.cuda.synchronize()
 
@@ -216,11 +294,7 @@ def run_ours(args):
     det = binding.Detector(w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0, state_dtype=w.state_dtype,
                            device=local, n_regions=R if R > 1 else 0, flags=flags)
     spec_dev = torch.empty(R * w.n_dir, w.n_omega, dtype=torch.float64, device="cuda")
-    if world > 1:
-        det_glob = binding.Detector(w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0,
-                                    state_dtype=w.state_dtype, device=local, n_regions=R if R > 1 else 0,
-                                    flags=flags)
-        amp_buf = torch.empty(R * w.n_dir, w.n_omega, 3, 2, dtype=torch.float64, device="cuda")
+    reducer = multi.AmplitudeAllReduce(det) if world > 1 else None
 
     def accumulate(i, host=False):
         st = (host_states if host else dev_states)[i % ring]
@@ -231,8 +305,8 @@ def run_ours(args):
 
     def step(i):
         accumulate(i)
-        if world > 1:   # the one exchange of the path: sum complex amplitudes, then |A|^2
-            multi.global_spectrum(det, det_glob, amp_buf, out=spec_dev)
+        if world > 1:   # the one exchange of the path: sum complex amplitudes over ranks, then |A|^2
+            reducer.global_spectrum(out=spec_dev)
         else:
             det.spectrum(out=spec_dev)
 
@@ -241,7 +315,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    flush = torch.empty(2 * L2_BYTES // 4, dtype=torch.float32, device="cuda")
+    flush = ctx["flush"]
     for i in range(W):
         step(i)
     flush.fill_(1.0)                            # evict inputs/tables left in L2 by set-up and warm-up
@@ -249,21 +323,23 @@ def run_ours(args):
     sampler = ClockSampler(local)
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    l0 = det.launch_count + (det_glob.launch_count if world > 1 else 0)
+    l0 = det.launch_count
     e0.record()
     for i in range(W, W + K):
         step(i)
+    if reducer:
+        reducer.wait()                          # the timed region ends when the last exchange has landed
     e1.record()
     barrier()
     clocks = sampler.stop()
-    launches = det.launch_count + (det_glob.launch_count if world > 1 else 0) - l0
+    launches = det.launch_count - l0
     ms_total = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(ms_total, op=dist.ReduceOp.MAX)
     ms_total = float(ms_total.item())
     updates_per_step = n * w.n_dir * w.n_omega
     value = world * updates_per_step * K / (ms_total * 1e-3) / 1e9
-    spectrum_check = float(spec_dev.sum().item())
+    S_after = spec_dev.cpu().numpy().copy()     # what the timed region left behind: checked below
 
     # dominant kernel alone (accumulate), same launch configuration, CUDA events on its stream
     flush.fill_(2.0)
@@ -279,7 +355,11 @@ def run_ours(args):
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     n_sm = torch.cuda.get_device_properties(local).multi_processor_count
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-    hbm_achieved = bytes_per_step / (kernel_ms * 1e-3) / 1e9
+    # algorithmic bytes per launch: the particle state read once + one
+    # read-modify-write pass over the fp64 accumulator for the fold (D*W*4 doubles = 32 B per bin)
+    fold_bytes = R * w.n_dir * w.n_omega * 32
+    algorithmic_bytes = bytes_per_step + fold_bytes
+    hbm_achieved = algorithmic_bytes / (kernel_ms * 1e-3) / 1e9
     traffic = None
     try:
         traffic = json.loads((ROOT / "profiles" / "traffic.json").read_text()).get(w.name, {}).get("bytes")
@@ -292,108 +372,162 @@ def run_ours(args):
                     "peak_how": f"MEASURED_PEAKS.json hbm_gbs ({peaks_src})"}
     else:
         if variant == "uniform":  # rotation recurrence: 4 FP32 rotate + 4 FMA accumulate per update
-            per_clk_sm, pipe = 128.0 / 8.0, "FP32 (8 FMA-pipe instr per update)"
+            per_clk_sm, pipe = FP32_LANES_PER_SM / FP32_PER_UPDATE_UNIFORM, "FP32 (8 FMA-pipe instr per update)"
+            measured = peaks_alu["ffma_per_clk_sm"] / FP32_PER_UPDATE_UNIFORM if peaks_alu else None
         else:                     # general grid: sin + cos per update on the 16-lane MUFU
             per_clk_sm, pipe = MUFU_LANES_PER_SM / MUFU_PER_UPDATE, "MUFU (sin+cos per update)"
+            measured = peaks_alu["sincos_pairs_per_clk_sm"] if peaks_alu else None
         peak = n_sm * per_clk_sm * sm_max * 1e6 / 1e9
         roofline = {"bound": "alu", "pipe": pipe, "achieved": achieved, "peak": peak, "unit": UNIT,
                     "frac": achieved / peak, "traffic": traffic,
-                    "peak_how": f"{n_sm} SMs x {per_clk_sm:g} updates/clk/SM x {sm_max:.0f} MHz (max SM clock, "
+                    "peak_how": f"nominal: {n_sm} SMs x {per_clk_sm:g} updates/clk/SM x {sm_max:.0f} MHz (max SM clock, "
                                 f"{peaks_src}); DESIGN.md section 5"}
-    if variant == "uniform":
-        # plain FFMA issues at 84-87 thread-instr/clk/SM on B200 (BASELINE.md note vii), not the nominal 128
-        roofline["frac_of_measured_ffma_rate"] = achieved / (n_sm * 87.0 / 8.0 * sm_max * 1e6 / 1e9)
-    roofline.update({"kernel": f"rad_accum_{variant}", "kernel_ms": kernel_ms,
-                     "algorithmic_bytes": int(bytes_per_step), "updates_per_launch": int(updates_per_step),
-                     "gupdates_per_s": achieved, "hbm_gbs_achieved": hbm_achieved, "hbm_gbs_peak": hbm_peak})
-    if clocks.get("sm_mhz"):
-        if roofline["bound"] == "alu":
+        if measured:
+            peak_m = n_sm * measured * sm_max * 1e6 / 1e9
+            roofline.update({"peak_measured_pipe": peak_m, "frac_of_measured_pipe": achieved / peak_m,
+                             "peak_measured_how": f"{n_sm} SMs x {measured:.3f} updates/clk/SM (alu_peaks) x {sm_max:.0f} MHz"})
+        if clocks.get("sm_mhz"):
             roofline["frac_at_sampled_clock"] = roofline["frac"] * sm_max / clocks["sm_mhz"]
+    roofline.update({"kernel": f"rad_accum_{variant}", "kernel_ms": kernel_ms,
+                     "algorithmic_bytes": int(algorithmic_bytes), "state_bytes": int(bytes_per_step),
+                     "fold_bytes": int(fold_bytes), "updates_per_launch": int(updates_per_step),
+                     "gupdates_per_s": achieved, "hbm_gbs_achieved": hbm_achieved, "hbm_gbs_peak": hbm_peak})
+    if traffic:
+        roofline["traffic_over_algorithmic"] = traffic / algorithmic_bytes
 
-    # rad_accumulate_steps: T resident steps in one launch (ramp/tail/launch latency paid once)
-    multi_step = None
-    T = int(min(16, ring, (2 << 30) // max(bytes_per_step, 1)))
-    if T >= 2 and world == 1:
-        stacked = [torch.stack([dev_states[i][c] for i in range(T)]).contiguous() for c in range(10)]
-        det.accumulate_steps(0, stacked, region_offsets=off)
-        torch.cuda.synchronize()
-        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        reps = max(1, min(10, K // T))
-        m0.record()
-        for r_ in range(reps):
-            det.accumulate_steps(r_ * T, stacked, region_offsets=off)
-        m1.record()
-        torch.cuda.synchronize()
-        ms_ms = m0.elapsed_time(m1) / reps
-        multi_step = {"steps_per_launch": T, "ms_per_launch": ms_ms,
-                      "value": updates_per_step * T / (ms_ms * 1e-3) / 1e9, "unit": UNIT,
-                      "note": "rad_accumulate_steps (kernel only, inputs resident); not the headline"}
-        del stacked
+    out = {"value": value, "unit": UNIT, "steps": K, "warmup": W, "ms_per_step": ms_total / K,
+           "kernel": f"rad_accum_{variant}", "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
+           "config": workload_config(w, n, world, "none" if args.no_overlap else "RAD_FLAG_OVERLAP_STEPS",
+                                     f"ring of {ring} distinct step inputs ({ring * bytes_per_step / 2**20:.0f} MiB) + "
+                                     f"L2 flush before the timed region")}
 
-    # end to end through the public API with HOST buffers: H2D of the step's state and D2H of
-    # the step's spectrum inside the timed region, every step
-    e2e = None
-    if not args.no_e2e:
-        det.reset()
-        # every step's spectrum lands in pinned host memory (RAD_OUT_HOST_ASYNC); the host waits
-        # for step i-1's result while step i's copies and kernels are already queued
-        spec_pinned = [torch.empty(R * w.n_dir, w.n_omega, dtype=torch.float64).pin_memory() for _ in range(2)]
-        arrived = [torch.cuda.Event(), torch.cuda.Event()]
-        ke = max(1, min(K, 50))
-        for i in range(min(W, 3)):
-            accumulate(i, host=True)
-        barrier()
-        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e2e_check = 0.0
-        a0.record()
-        for i in range(W, W + ke):
-            accumulate(i, host=True)
-            b = i & 1
+    # parity of what the timed region computed (outside the timed region; rank 0's own shard)
+    if world == 1 and not args.no_cpu_baseline:
+        out["parity"] = parity_vs_oracle(w, n, states_np, ring, W + K, S_after,
+                                         budget_updates=2.0e9 if headline else 5.0e8)
+
+    if headline:
+        # rad_accumulate_steps: T resident steps in one launch (ramp/tail/launch latency paid once)
+        T = int(min(16, ring, (2 << 30) // max(bytes_per_step, 1)))
+        if T >= 2 and world == 1:
+            stacked = [torch.stack([dev_states[i][c] for i in range(T)]).contiguous() for c in range(10)]
+            det.accumulate_steps(0, stacked, region_offsets=off)
+            torch.cuda.synchronize()
+            m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            reps = max(1, min(10, K // T))
+            m0.record()
+            for r_ in range(reps):
+                det.accumulate_steps(r_ * T, stacked, region_offsets=off)
+            m1.record()
+            torch.cuda.synchronize()
+            ms_ms = m0.elapsed_time(m1) / reps
+            out["multi_step"] = {"steps_per_launch": T, "ms_per_launch": ms_ms,
+                                 "value": updates_per_step * T / (ms_ms * 1e-3) / 1e9, "unit": UNIT,
+                                 "note": "rad_accumulate_steps (kernel only, inputs resident); not the headline"}
+            del stacked
+
+        # end to end through the public API with HOST buffers: H2D of the step's state and D2H of
+        # the step's spectrum inside the timed region, every step
+        if not args.no_e2e:
+            det.reset()
+            # every step's spectrum lands in pinned host memory (RAD_OUT_HOST_ASYNC); the host waits
+            # for step i-1's result while step i's copies and kernels are already queued
+            spec_pinned = [torch.empty(R * w.n_dir, w.n_omega, dtype=torch.float64).pin_memory() for _ in range(2)]
+            arrived = [torch.cuda.Event(), torch.cuda.Event()]
+            ke = max(1, min(K, 50))
+            we = min(W, 3)
+            for i in range(we):
+                accumulate(i, host=True)
+            barrier()
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record()
+            for i in range(we, we + ke):
+                accumulate(i, host=True)
+                b = i & 1
+                if world > 1:
+                    reducer.global_spectrum(out=spec_dev)
+                    reducer.wait()
+                    spec_pinned[b].copy_(spec_dev, non_blocking=True)
+                else:
+                    det.spectrum(out=spec_pinned[b])
+                arrived[b].record()
+                if i > we:
+                    arrived[b ^ 1].synchronize()
+            arrived[(we + ke - 1) & 1].synchronize()
+            a1.record()
+            barrier()
+            S_e2e = spec_pinned[(we + ke - 1) & 1].numpy().copy()
+            ms_e = torch.tensor([a0.elapsed_time(a1)], dtype=torch.float64, device="cuda")
             if world > 1:
-                multi.global_spectrum(det, det_glob, amp_buf, out=spec_dev)
-                spec_pinned[b].copy_(spec_dev, non_blocking=True)
-            else:
-                det.spectrum(out=spec_pinned[b])
-            arrived[b].record()
-            if i > W:
-                arrived[b ^ 1].synchronize()
-                e2e_check += float(spec_pinned[b ^ 1][0, 0])
-        arrived[(W + ke - 1) & 1].synchronize()
-        e2e_check += float(spec_pinned[(W + ke - 1) & 1][0, 0])
-        a1.record()
-        barrier()
-        ms_e = torch.tensor([a0.elapsed_time(a1)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(ms_e, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * updates_per_step * ke / (float(ms_e.item()) * 1e-3) / 1e9, "unit": UNIT,
-               "h2d_bytes_per_step": int(bytes_per_step), "d2h_bytes_per_step": int(spec_pinned[0].numel() * 8),
-               "steps": ke}
+                dist.all_reduce(ms_e, op=dist.ReduceOp.MAX)
+            out["e2e"] = {"value": world * updates_per_step * ke / (float(ms_e.item()) * 1e-3) / 1e9, "unit": UNIT,
+                          "h2d_bytes_per_step": int(bytes_per_step),
+                          "d2h_bytes_per_step": int(spec_pinned[0].numel() * 8), "steps": ke}
+            if world == 1 and not args.no_cpu_baseline:   # the last host-side spectrum of the e2e leg, checked too
+                out["e2e"]["parity"] = parity_vs_oracle(w, n, states_np, ring, we + ke, S_e2e, budget_updates=1.0e9)
 
-    cpu_baseline = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        from oracle import oracle
-        st0 = [a.numpy() for a in host_states[0]]
-        rate, secs, nb = time_oracle(w, st0, budget_s=15.0)
-        cpu_baseline = {"value": rate / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                        "sample": f"{nb} of {w.n_dir * w.n_omega} bins (stratified) x all {n} particles of one "
-                                  f"PIC step of {w.name}; {secs:.1f} s"}
-    if rank == 0:
-        print(json.dumps({
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32 phase/amplitude, f64 set-up and accumulators", "data": "synthetic",
-            "config": {"workload": w.name, "n_particles_per_gpu": n, "n_regions": R, "n_dir": w.n_dir,
-                       "n_omega": w.n_omega,
-                       "state_dtype": np.dtype(w.state_dtype).name, "parallelism": f"particle-shard x{world}",
-                       "flags": "none" if args.no_overlap else "RAD_FLAG_OVERLAP_STEPS",
-                       "l2": f"ring of {ring} distinct step inputs ({ring * bytes_per_step / 2**20:.0f} MiB) + "
-                             f"L2 flush before the timed region"},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-            "cpu_baseline": cpu_baseline, "multi_step": multi_step, "spectrum_checksum": spectrum_check,
-        }))
+        if rank == 0 and world == 1 and not args.no_cpu_baseline:
+            from oracle import oracle
+            rate, secs, nb = time_oracle(w, states_np[0], budget_s=12.0)
+            out["cpu_baseline"] = {"value": rate / 1e9, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                                   "sample": f"{nb} of {w.n_dir * w.n_omega} bins (stratified) x all {n} particles of "
+                                             f"one PIC step of {w.name}; {secs:.1f} s"}
     det.close()
+    if reducer:
+        reducer.close()
+    del dev_states, host_states
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2501_03383_b200 import build as rad_build
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference)")
+    torch.cuda.set_device(local)
     if world > 1:
-        det_glob.close()
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    rad_build.build()
+    peaks, peaks_src = measured_peaks()
+    ctx = {"rank": rank, "world": world, "local": local, "peaks": peaks, "peaks_src": peaks_src,
+           "flush": torch.empty(2 * L2_BYTES // 4, dtype=torch.float32, device="cuda"), "alu_peaks": None}
+    t_start = time.perf_counter()
+    try:
+        ctx["alu_peaks"] = alu_peaks(local, float(peaks.get("sm_max_mhz", 1965.0)))
+    except Exception as exc:       # the microbenchmarks are evidence, not the product: report, go on
+        ctx["alu_peaks"] = None
+        ctx["alu_peaks_error"] = repr(exc)
+
+    head = measure(args.config, args.steps, args.warmup, args, ctx, headline=True)
+    legs = {}
+    if world == 1 and not args.no_legs and args.config == HEADLINE and args.particles is None:
+        for cfg, k, wu in LEGS:
+            try:
+                leg = measure(cfg, k, wu, args, ctx, headline=False)
+                legs[leg["config"]["workload"]] = leg
+            except Exception as exc:
+                legs[f"cfg {cfg}"] = {"error": repr(exc)}
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32 phase/amplitude, f64 set-up and accumulators", "data": "synthetic",
+            "config": head["config"], "clocks": head["clocks"], "e2e": head.get("e2e"),
+            "gpu_launches": head["gpu_launches"], "roofline": head["roofline"],
+            "cpu_baseline": head.get("cpu_baseline"), "parity": head.get("parity"),
+            "multi_step": head.get("multi_step"), "alu_peaks": ctx["alu_peaks"], "configs": legs,
+            "bench_wall_s": time.perf_counter() - t_start,
+        }
+        if "alu_peaks_error" in ctx:
+            line["alu_peaks_error"] = ctx["alu_peaks_error"]
+        print(json.dumps(line))
+    if world > 1:
         dist.destroy_process_group()
 
 

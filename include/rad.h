@@ -40,7 +40,11 @@
  *     cross-stream dependency between calls).
  *   - No exception crosses the ABI.  Every function returns a rad_status; details via
  *     rad_last_error().  Particle values are not scanned: NaN/Inf or 1 - beta.n = 0 in the
- *     state give NaN/Inf in the result (documented, caller's responsibility).
+ *     state give NaN/Inf in every bin the particle contributes to, for fp32 and fp64 state
+ *     alike (documented, caller's responsibility; tests/test_gpu_parity.py
+ *     test_non_finite_particle_state_propagates).
+ *   - An entry point makes the handle's device current while it runs and restores the calling
+ *     thread's current device before it returns.
  *   - There is no CPU fallback: without a CUDA device rad_create fails with RAD_ERR_CUDA.
  */
 #ifndef RAD_H_
@@ -97,7 +101,9 @@ typedef struct {
     double dt;             /* s, > 0: the quadrature weight of every term                  */
     double t0;             /* s: time of step_index 0                                      */
     double scale;          /* S = scale*|A|^2; 0 -> SI e^2/(16 pi^3 eps0 c) J s            */
-    int32_t state_dtype;   /* rad_dtype of the 10 particle arrays                          */
+    int32_t state_dtype;   /* a rad_dtype value (RAD_F32 / RAD_F64) for the 10 particle arrays;
+                              declared int32_t, not the enum, so the struct layout does not
+                              depend on the compiler's enum size                            */
     uint32_t flags;        /* RAD_FLAG_*                                                   */
     int32_t n_regions;     /* 0 or 1: one detector; R > 1: R per-region detectors          */
     int32_t window_type;   /* RAD_WINDOW_*: spatial window on the macro weights (below)    */
@@ -125,11 +131,15 @@ typedef struct {
 #define RAD_WINDOW_TRIANGLE 1
 #define RAD_WINDOW_HAMMING 2
 
-/* Create a detector: copies dirs/omega, builds the device tables, zeroes A.
- * *out is set to NULL on failure. */
+/* Create a detector for a grid of observation directions n and frequencies w_j (BASELINE.json
+ * north_star "on a grid of observation directions n and frequencies w"; the
+ * plugin records "for each wavelength and direction"): copies dirs/omega, builds the device
+ * tables, zeroes A.  *out is set to NULL on failure. */
 RAD_API rad_status rad_create(const rad_config *cfg, rad_handle **out);
 
-/* A += contributions of n_particles particles at time t0 + step_index*dt.
+/* A += contributions of n_particles particles at time t0 + step_index*dt: one PIC step of the
+ * sum ("at each PIConGPU time step ... the sum of the contributions from all
+ * radiating particles"; the summand is north_star's, stated at the top of this header).
  * All 10 arrays DEVICE, `state_dtype` elements, 16-byte aligned not required.
  * n_particles == 0 is a no-op.  Calls are additive: several calls with the same
  * step_index superpose (particle subsets), any order of steps gives the same A up to
@@ -236,7 +246,31 @@ RAD_API rad_status rad_amplitude(rad_handle *h, double *out, int out_on_device, 
  * radiating particles in the simulation"), rad_reset(), then add the reduced buffer. */
 RAD_API rad_status rad_add_amplitude(rad_handle *h, const double *amp_device, void *cuda_stream);
 
-/* A := 0 (start a new accumulation window). */
+/* The accumulator itself, for the multi-GPU sum and for checkpoints.  A is perpendicular to n
+ * (it is n x something), so the library keeps its two components on a fixed orthonormal pair
+ * e1, e2 _|_ n chosen at rad_create from n alone (e1 = normalise(z^ x n), x^ x n if |n_z| > 0.9;
+ * e2 = n x e1): handles created with the same dirs share the basis, whatever the device.
+ *   out_device[(R)][n_dir][n_omega][4] fp64 = (Re A1, Im A1, Re A2, Im A2), A = A1 e1 + A2 e2.
+ * PAPER.md line 80 ("the sum of the contributions from all radiating particles in the
+ * simulation") with particles sharded over GPUs (line 138) means: every rank exports, ONE sum
+ * all-reduce over these n_dir*n_omega*4 doubles (two thirds of the Cartesian rad_amplitude
+ * buffer), then rad_spectrum_of() on the sum -- amplitudes, never intensities, are added.
+ * A device-to-device copy on cuda_stream; asynchronous. */
+RAD_API rad_status rad_export_accumulator(rad_handle *h, double *out_device, void *cuda_stream);
+
+/* A := A + amp4, amp4_device in the rad_export_accumulator layout (restart from a checkpoint,
+ * or fold another rank's amplitude into this handle).  Asynchronous on cuda_stream. */
+RAD_API rad_status rad_import_accumulator(rad_handle *h, const double *amp4_device, void *cuda_stream);
+
+/* out[(R)][n_dir][n_omega] = scale * (|A1|^2 + |A2|^2) of an amplitude buffer in the
+ * rad_export_accumulator layout (DEVICE) instead of the handle's own accumulator, which is not
+ * touched: the |A|^2 step after the all-reduce.  out_on_device as in rad_spectrum. */
+RAD_API rad_status rad_spectrum_of(rad_handle *h, const double *amp4_device, double *out, int out_on_device,
+                                   void *cuda_stream);
+
+/* A := 0: start a new accumulation window.  PAPER.md line 74 "the observed intensity at each
+ * wavelength and direction varies between time steps", line 80 "calculate the radiation spectrum
+ * ... at each time step": a caller that wants per-step or per-window spectra resets between them. */
 RAD_API rad_status rad_reset(rad_handle *h, void *cuda_stream);
 
 /* Frees everything the handle owns after synchronising the device.  NULL-safe. */

@@ -47,6 +47,9 @@ def _load():
         lib.oracle_accumulate_step_w.restype = ctypes.c_int
         lib.oracle_accumulate_step_w.argtypes = (lib.oracle_accumulate_step.argtypes
                                                  + [ctypes.c_int, ctypes.c_void_p, ctypes.c_double])
+        lib.oracle_accumulate_step_ff.restype = ctypes.c_int
+        lib.oracle_accumulate_step_ff.argtypes = (lib.oracle_accumulate_step_w.argtypes
+                                                  + [ctypes.c_int, ctypes.c_void_p])
         lib.oracle_accumulate_step_regions.restype = ctypes.c_int
         lib.oracle_accumulate_step_regions.argtypes = (
             [ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p,
@@ -57,6 +60,12 @@ def _load():
         lib.oracle_accumulate_step_regions_w.restype = ctypes.c_int
         lib.oracle_accumulate_step_regions_w.argtypes = (lib.oracle_accumulate_step_regions.argtypes
                                                          + [ctypes.c_int, ctypes.c_void_p, ctypes.c_double])
+        lib.oracle_accumulate_step_regions_ff.restype = ctypes.c_int
+        lib.oracle_accumulate_step_regions_ff.argtypes = (lib.oracle_accumulate_step_regions_w.argtypes
+                                                          + [ctypes.c_int, ctypes.c_void_p])
+        lib.oracle_spectrum_total.restype = ctypes.c_int
+        lib.oracle_spectrum_total.argtypes = [ctypes.c_longlong, ctypes.c_longlong, ctypes.c_void_p,
+                                              ctypes.c_double, ctypes.c_void_p]
         lib.oracle_spectrum.restype = ctypes.c_int
         lib.oracle_spectrum.argtypes = [ctypes.c_longlong, ctypes.c_void_p, ctypes.c_double,
                                         ctypes.c_void_p]
@@ -83,6 +92,17 @@ def _window_args(window):
     return WINDOW_TYPES[name], np.ascontiguousarray(list(origin) + list(extent), dtype=np.float64)
 
 
+FORM_FACTOR_TYPES = {"none": 0, "gaussian": 1, "cic": 2, "incoherent": 3}
+
+
+def _form_factor_args(form_factor):
+    """form_factor = None or (type name, size[3] in metres) -> (type code, fp64 array of 3)."""
+    if form_factor is None:
+        return 0, np.zeros(3)
+    name, size = form_factor
+    return FORM_FACTOR_TYPES[name], np.ascontiguousarray(list(size), dtype=np.float64)
+
+
 class Oracle:
     """Same call sequence as the C ABI (create / accumulate_step / spectrum / amplitude).
 
@@ -90,8 +110,10 @@ class Oracle:
     dir*W + j) restricts the computation to a subset of bins; other bins stay zero.
     """
 
-    def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, bins=None, window=None, nyquist=0.0):
+    def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, bins=None, window=None, nyquist=0.0,
+                 form_factor=None):
         self.nyquist = float(nyquist)
+        self.ff_type, self.ff_size = _form_factor_args(form_factor)
         self.dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
         self.omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
         self.dt, self.t0, self.scale = float(dt), float(t0), float(scale)
@@ -114,11 +136,12 @@ class Oracle:
             raise ValueError("state arrays must be 1-D and of equal length")
         nb = 0 if self.bins is None else self.bins.shape[0]
         bp = None if self.bins is None else self.bins.ctypes.data
-        rc = _load().oracle_accumulate_step_w(
+        rc = _load().oracle_accumulate_step_ff(
             self.D, self.dirs.ctypes.data, self.W, self.omega.ctypes.data, self.dt, self.t0,
             int(step_index), n, int(dt0 == np.dtype(np.float32)),
             *[a.ctypes.data for a in arrs], nb, bp, self.A.ctypes.data,
-            self.win_type, None if self.win is None else self.win.ctypes.data, self.nyquist)
+            self.win_type, None if self.win is None else self.win.ctypes.data, self.nyquist,
+            self.ff_type, self.ff_size.ctypes.data)
         if rc != 0:
             raise ValueError("oracle_accumulate_step: bad argument")
 
@@ -139,8 +162,10 @@ class RegionOracle:
     only.  Particles are sorted by region; ``offsets`` [R+1] (non-decreasing) are passed with
     every step.  Same (optional) bin subset in every region."""
 
-    def __init__(self, n_regions, dirs, omega, dt, t0=0.0, scale=0.0, bins=None, window=None, nyquist=0.0):
+    def __init__(self, n_regions, dirs, omega, dt, t0=0.0, scale=0.0, bins=None, window=None, nyquist=0.0,
+                 form_factor=None):
         self.win_type, self.win = _window_args(window)
+        self.ff_type, self.ff_size = _form_factor_args(form_factor)
         self.nyquist = float(nyquist)
         self.dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
         self.omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
@@ -166,11 +191,12 @@ class RegionOracle:
             raise ValueError("state arrays must be 1-D, of equal length >= offsets[-1]")
         nb = 0 if self.bins is None else self.bins.shape[0]
         bp = None if self.bins is None else self.bins.ctypes.data
-        rc = _load().oracle_accumulate_step_regions_w(
+        rc = _load().oracle_accumulate_step_regions_ff(
             self.D, self.dirs.ctypes.data, self.W, self.omega.ctypes.data, self.dt, self.t0,
             int(step_index), self.R, offsets.ctypes.data, int(dt0 == np.dtype(np.float32)),
             *[a.ctypes.data for a in arrs], nb, bp, self.A.ctypes.data,
-            self.win_type, None if self.win is None else self.win.ctypes.data, self.nyquist)
+            self.win_type, None if self.win is None else self.win.ctypes.data, self.nyquist,
+            self.ff_type, self.ff_size.ctypes.data)
         if rc != 0:
             raise ValueError("oracle_accumulate_step_regions: bad argument")
 
@@ -189,9 +215,8 @@ class RegionOracle:
 
     def spectrum_total(self):
         """[D, W]: |sum_r A_r|^2 -- amplitudes, not intensities, add up."""
-        tot = np.ascontiguousarray(self.A.sum(axis=0))
         S = np.empty((self.D, self.W), dtype=np.float64)
-        rc = _load().oracle_spectrum(self.D * self.W, tot.ctypes.data, self.scale, S.ctypes.data)
+        rc = _load().oracle_spectrum_total(self.R, self.D * self.W, self.A.ctypes.data, self.scale, S.ctypes.data)
         if rc != 0:
-            raise ValueError("oracle_spectrum: bad argument")
+            raise ValueError("oracle_spectrum_total: bad argument")
         return S

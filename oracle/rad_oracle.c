@@ -60,6 +60,25 @@
  * nothing; a static particle loses exactly the bins w_j dt >= pi nu; the cut-off of a moving
  * particle is Doppler shifted by direction; kept bins equal the closed forms.
  * (nu is the last argument of the _w entry points; 0 = off.)
+ *
+ * Macro-particle form factor (NEXT-3, reading FF1 of DESIGN.md; the plugin
+ * "correctly quantif[ies] coherent and incoherent radiation [39]", ref [39] "a general form
+ * factor formalism for macro-particles", formula not printed in the paper): a macro-particle of
+ * weight w stands for w real particles distributed with a shape whose Fourier transform at the
+ * emitted wave vector k = w_j n / c is F(n, w_j), 0 <= F <= 1.  Their fields add coherently for
+ * the fraction F^2 and incoherently for the rest, intensity factor w^2 F^2 + w (1 - F^2), so the
+ * weight of a term in the amplitude sum becomes
+ *     g_k(n, w_j) = sqrt( w_k + (w_k^2 - w_k) F^2(n, w_j) )        instead of w_k
+ * (the spatial window, if any, still multiplies it).  Shapes (ff_size = s_x, s_y, s_z in metres):
+ *     1 GAUSSIAN    F = exp( -1/2 sum_c (w_j n_c s_c / c)^2 )             (s_c = standard deviations)
+ *     2 CIC         F = prod_c sinc^2( w_j n_c s_c / (2 c) ), sinc x = sin x / x   (s_c = cell sizes)
+ *     3 INCOHERENT  F = 0   (g = sqrt w)
+ *     0 none        g = w   (the detector as BASELINE.json states it; F = 1 gives the same)
+ * Pins (test_p14_*): w = 1 is the identity bit for bit; F = 1 (zero size) reproduces the plain
+ * sum; F = 0 makes the intensity of one macro-particle proportional to w, not w^2; closed forms
+ * g^2 x Dirichlet kernel for the Gaussian (anisotropic, direction dependent) and at the first
+ * zero of the CIC shape; numpy brute force.  (ff_type, ff_size are the last arguments of the _ff
+ * entry points.)
  */
 #include <math.h>
 #include <stddef.h>
@@ -121,14 +140,41 @@ static double window_1d(int type, double u)
  *   nyquist nu of the Nyquist limiter (0: off)
  * Returns 0, or 1 on a bad argument.
  */
-int oracle_accumulate_step_w(int n_dir, const double *dirs, int n_omega, const double *omega,
-                             double dt, double t0, long long step_index, long long n_part,
-                             int is_f32, const void *rx, const void *ry, const void *rz,
-                             const void *bx, const void *by, const void *bz, const void *bdx,
-                             const void *bdy, const void *bdz, const void *w,
-                             long long n_bins, const long long *bin_idx, double *A,
-                             int win_type, const double *win, double nyquist)
+/* F(n, w) of the macro-particle shape, see the header (reading FF1). */
+static double form_factor(int type, const double size[3], const double n[3], double om)
 {
+    if (type == 1) {
+        double q = 0.0;
+        for (int c = 0; c < 3; ++c) {
+            const double x = om * n[c] * size[c] / ORACLE_C_LIGHT;
+            q += x * x;
+        }
+        return exp(-0.5 * q);
+    }
+    if (type == 2) {
+        double F = 1.0;
+        for (int c = 0; c < 3; ++c) {
+            const double x = om * n[c] * size[c] / (2.0 * ORACLE_C_LIGHT);
+            const double sinc = (x == 0.0) ? 1.0 : sin(x) / x;
+            F *= sinc * sinc;
+        }
+        return F;
+    }
+    if (type == 3) return 0.0;
+    return 1.0;
+}
+
+/*   ff_type 0 none / 1 Gaussian / 2 CIC / 3 incoherent; ff_size = {s_x, s_y, s_z} (NULL with type 0) */
+int oracle_accumulate_step_ff(int n_dir, const double *dirs, int n_omega, const double *omega,
+                              double dt, double t0, long long step_index, long long n_part,
+                              int is_f32, const void *rx, const void *ry, const void *rz,
+                              const void *bx, const void *by, const void *bz, const void *bdx,
+                              const void *bdy, const void *bdz, const void *w,
+                              long long n_bins, const long long *bin_idx, double *A,
+                              int win_type, const double *win, double nyquist,
+                              int ff_type, const double *ff_size)
+{
+    if (ff_type != 0 && !ff_size) return 1;
     if (n_dir <= 0 || n_omega <= 0 || !dirs || !omega || !A || n_part < 0) return 1;
     const long long total = bin_idx ? n_bins : (long long)n_dir * n_omega;
     const double t_step = t0 + (double)step_index * dt;
@@ -145,12 +191,14 @@ int oracle_accumulate_step_w(int n_dir, const double *dirs, int n_omega, const d
         const double nn = sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
         n[0] /= nn; n[1] /= nn; n[2] /= nn;
         const double om = omega[j];
+        const double F = ff_type != 0 ? form_factor(ff_type, ff_size, n, om) : 1.0;
         double acc[6] = {0, 0, 0, 0, 0, 0};
         for (long long k = 0; k < n_part; ++k) {
             const double r[3] = {LOAD(rx, k), LOAD(ry, k), LOAD(rz, k)};
             const double be[3] = {LOAD(bx, k), LOAD(by, k), LOAD(bz, k)};
             const double bd[3] = {LOAD(bdx, k), LOAD(bdy, k), LOAD(bdz, k)};
             double wk = LOAD(w, k);
+            if (ff_type != 0) wk = sqrt(wk + (wk * wk - wk) * F * F); /* g_k(n, w_j), reading FF1 */
             if (win_type != 0 && win)
                 for (int c = 0; c < 3; ++c)
                     if (win[3 + c] > 0.0) wk *= window_1d(win_type, (r[c] - win[c]) / win[3 + c]);
@@ -177,6 +225,20 @@ int oracle_accumulate_step_w(int n_dir, const double *dirs, int n_omega, const d
     return 0;
 }
 
+/* No form factor. */
+int oracle_accumulate_step_w(int n_dir, const double *dirs, int n_omega, const double *omega,
+                             double dt, double t0, long long step_index, long long n_part,
+                             int is_f32, const void *rx, const void *ry, const void *rz,
+                             const void *bx, const void *by, const void *bz, const void *bdx,
+                             const void *bdy, const void *bdz, const void *w,
+                             long long n_bins, const long long *bin_idx, double *A,
+                             int win_type, const double *win, double nyquist)
+{
+    return oracle_accumulate_step_ff(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_part, is_f32, rx, ry,
+                                     rz, bx, by, bz, bdx, bdy, bdz, w, n_bins, bin_idx, A, win_type, win,
+                                     nyquist, 0, NULL);
+}
+
 /* The plain detector: no window. */
 int oracle_accumulate_step(int n_dir, const double *dirs, int n_omega, const double *omega,
                            double dt, double t0, long long step_index, long long n_part,
@@ -197,14 +259,14 @@ int oracle_accumulate_step(int n_dir, const double *dirs, int n_omega, const dou
  * every region.  Written as the definition: one plain oracle_accumulate_step per region
  * on that region's slice of the state arrays.
  */
-int oracle_accumulate_step_regions_w(int n_dir, const double *dirs, int n_omega, const double *omega,
-                                     double dt, double t0, long long step_index, long long n_regions,
-                                     const long long *offsets, int is_f32, const void *rx,
-                                     const void *ry, const void *rz, const void *bx, const void *by,
-                                     const void *bz, const void *bdx, const void *bdy,
-                                     const void *bdz, const void *w, long long n_bins,
-                                     const long long *bin_idx, double *A, int win_type, const double *win,
-                                     double nyquist)
+int oracle_accumulate_step_regions_ff(int n_dir, const double *dirs, int n_omega, const double *omega,
+                                      double dt, double t0, long long step_index, long long n_regions,
+                                      const long long *offsets, int is_f32, const void *rx,
+                                      const void *ry, const void *rz, const void *bx, const void *by,
+                                      const void *bz, const void *bdx, const void *bdy,
+                                      const void *bdz, const void *w, long long n_bins,
+                                      const long long *bin_idx, double *A, int win_type, const double *win,
+                                      double nyquist, int ff_type, const double *ff_size)
 {
     if (n_regions <= 0 || !offsets || offsets[0] < 0) return 1;
     for (long long r = 0; r < n_regions; ++r)
@@ -214,14 +276,29 @@ int oracle_accumulate_step_regions_w(int n_dir, const double *dirs, int n_omega,
     for (long long r = 0; r < n_regions; ++r) {
         const long long k0 = offsets[r], n_r = offsets[r + 1] - offsets[r];
         double *A_r = A + (size_t)r * n_dir * n_omega * 6;
-        const int rc = oracle_accumulate_step_w(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_r,
-                                                is_f32, AT(rx, k0), AT(ry, k0), AT(rz, k0), AT(bx, k0),
-                                                AT(by, k0), AT(bz, k0), AT(bdx, k0), AT(bdy, k0),
-                                                AT(bdz, k0), AT(w, k0), n_bins, bin_idx, A_r, win_type, win, nyquist);
+        const int rc = oracle_accumulate_step_ff(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_r,
+                                                 is_f32, AT(rx, k0), AT(ry, k0), AT(rz, k0), AT(bx, k0),
+                                                 AT(by, k0), AT(bz, k0), AT(bdx, k0), AT(bdy, k0),
+                                                 AT(bdz, k0), AT(w, k0), n_bins, bin_idx, A_r, win_type, win, nyquist,
+                                                 ff_type, ff_size);
         if (rc != 0) return rc;
     }
 #undef AT
     return 0;
+}
+
+int oracle_accumulate_step_regions_w(int n_dir, const double *dirs, int n_omega, const double *omega,
+                                     double dt, double t0, long long step_index, long long n_regions,
+                                     const long long *offsets, int is_f32, const void *rx,
+                                     const void *ry, const void *rz, const void *bx, const void *by,
+                                     const void *bz, const void *bdx, const void *bdy,
+                                     const void *bdz, const void *w, long long n_bins,
+                                     const long long *bin_idx, double *A, int win_type, const double *win,
+                                     double nyquist)
+{
+    return oracle_accumulate_step_regions_ff(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_regions, offsets,
+                                             is_f32, rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w, n_bins, bin_idx, A,
+                                             win_type, win, nyquist, 0, NULL);
 }
 
 int oracle_accumulate_step_regions(int n_dir, const double *dirs, int n_omega, const double *omega,
@@ -235,6 +312,23 @@ int oracle_accumulate_step_regions(int n_dir, const double *dirs, int n_omega, c
     return oracle_accumulate_step_regions_w(n_dir, dirs, n_omega, omega, dt, t0, step_index, n_regions, offsets,
                                             is_f32, rx, ry, rz, bx, by, bz, bdx, bdy, bdz, w, n_bins, bin_idx, A,
                                             0, NULL, 0.0);
+}
+
+/* Per-region detectors, detector of all particles: S_total[n][j] = scale * sum_c |sum_r A_r,c|^2
+ * (amplitudes, not intensities, add up: PAPER.md line 80).  A is [n_regions][n_bins][3][2]. */
+int oracle_spectrum_total(long long n_regions, long long n_bins, const double *A, double scale, double *S)
+{
+    if (!A || !S || n_bins < 0 || n_regions <= 0) return 1;
+    const double sc = (scale == 0.0) ? oracle_default_scale() : scale;
+    for (long long b = 0; b < n_bins; ++b) {
+        double tot[6] = {0, 0, 0, 0, 0, 0};
+        for (long long r = 0; r < n_regions; ++r)
+            for (int c = 0; c < 6; ++c) tot[c] += A[((size_t)r * n_bins + b) * 6 + c];
+        double s = 0.0;
+        for (int c = 0; c < 6; ++c) s += tot[c] * tot[c];
+        S[b] = sc * s;
+    }
+    return 0;
 }
 
 /* S[n][j] = scale * sum_c |A_c|^2 ; scale == 0 -> SI default (Q4). */

@@ -27,7 +27,8 @@ ABI_SYMBOLS = (
     "rad_create", "rad_accumulate_step", "rad_accumulate_steps", "rad_accumulate_steps_regions",
     "rad_accumulate_step_host",
     "rad_accumulate_step_regions", "rad_accumulate_step_regions_host", "rad_spectrum",
-    "rad_spectrum_total", "rad_amplitude", "rad_add_amplitude", "rad_reset", "rad_destroy", "rad_launch_count",
+    "rad_spectrum_total", "rad_amplitude", "rad_add_amplitude", "rad_export_accumulator",
+    "rad_import_accumulator", "rad_spectrum_of", "rad_reset", "rad_destroy", "rad_launch_count",
     "rad_kernel_variant", "rad_status_string", "rad_last_error", "rad_version",
 )
 
@@ -88,6 +89,12 @@ def load(path: Optional[Path] = None) -> ctypes.CDLL:
     lib.rad_add_amplitude.argtypes = [vp, vp, vp]
     lib.rad_reset.restype = ctypes.c_int
     lib.rad_reset.argtypes = [vp, vp]
+    for name in ("rad_export_accumulator", "rad_import_accumulator"):
+        f = getattr(lib, name)
+        f.restype = ctypes.c_int
+        f.argtypes = [vp, vp, vp]
+    lib.rad_spectrum_of.restype = ctypes.c_int
+    lib.rad_spectrum_of.argtypes = [vp, vp, vp, ctypes.c_int, vp]
     lib.rad_destroy.restype = None
     lib.rad_destroy.argtypes = [vp]
     lib.rad_launch_count.restype = i64
@@ -200,6 +207,19 @@ def rad_add_amplitude(handle: int, amp_device_ptr: int, stream: int = 0) -> None
     _check(load().rad_add_amplitude(handle, amp_device_ptr, stream), handle)
 
 
+def rad_export_accumulator(handle: int, out_device_ptr: int, stream: int = 0) -> None:
+    """out: DEVICE [(R,) D, W, 4] fp64 = (Re A1, Im A1, Re A2, Im A2) on the handle's transverse basis."""
+    _check(load().rad_export_accumulator(handle, out_device_ptr, stream), handle)
+
+
+def rad_import_accumulator(handle: int, amp4_device_ptr: int, stream: int = 0) -> None:
+    _check(load().rad_import_accumulator(handle, amp4_device_ptr, stream), handle)
+
+
+def rad_spectrum_of(handle: int, amp4_device_ptr: int, out_ptr: int, out_on_device: int, stream: int = 0) -> None:
+    _check(load().rad_spectrum_of(handle, amp4_device_ptr, out_ptr, int(out_on_device), stream), handle)
+
+
 def rad_reset(handle: int, stream: int = 0) -> None:
     _check(load().rad_reset(handle, stream), handle)
 
@@ -235,10 +255,9 @@ class Detector:
         return ((self.R,) if self.R > 1 else ()) + (self.D, self.W) + tail
 
     # -- helpers
-    @staticmethod
-    def _stream() -> int:
+    def _stream(self) -> int:
         import torch
-        return int(torch.cuda.current_stream().cuda_stream)
+        return int(torch.cuda.current_stream(self.device).cuda_stream)
 
     def _ptrs(self, state, want_cuda: bool):
         import torch
@@ -334,6 +353,23 @@ class Detector:
 
     def add_amplitude(self, amp) -> None:
         rad_add_amplitude(self.handle, amp.data_ptr(), self._stream())
+
+    def export_accumulator(self, out) -> None:
+        """out: torch CUDA fp64 tensor [(R,) D, W, 4] (contiguous)."""
+        rad_export_accumulator(self.handle, out.data_ptr(), self._stream())
+
+    def import_accumulator(self, amp4) -> None:
+        rad_import_accumulator(self.handle, amp4.data_ptr(), self._stream())
+
+    def spectrum_of(self, amp4, out=None):
+        """|A|^2 of an exported / all-reduced amplitude buffer; out as in spectrum()."""
+        if out is not None:
+            mode = RAD_OUT_DEVICE if out.is_cuda else RAD_OUT_HOST_ASYNC
+            rad_spectrum_of(self.handle, amp4.data_ptr(), out.data_ptr(), mode, self._stream())
+            return out
+        res = np.empty(self._shape(), dtype=np.float64)
+        rad_spectrum_of(self.handle, amp4.data_ptr(), res.ctypes.data, RAD_OUT_HOST, self._stream())
+        return res
 
     def reset(self) -> None:
         rad_reset(self.handle, self._stream())

@@ -125,6 +125,9 @@ rad_status ensure_chunk_capacity(Handle &h, size_t need)
         cudaFree(h.chunks_d); h.chunks_d = nullptr;
         if (h.chunks_h) cudaFreeHost(h.chunks_h);
         h.chunks_h = nullptr; h.reg_cap = 0;
+        // whatever table was cached lived in these buffers: forget it, so that a failed
+        // allocation below can never be followed by a cache hit on freed memory
+        h.reg_chunk = 0; h.reg_offsets.clear(); h.tap_n = -1; h.tap_chunk = 0; h.reg_n_chunks = 0;
         const size_t cap = std::max<size_t>(need + need / 4, 64);
         bool ok = cudaMallocHost(&h.chunks_h, cap * sizeof(ChunkRec)) == cudaSuccess &&
                   cudaMalloc(&h.chunks_d, cap * sizeof(ChunkRec)) == cudaSuccess;
@@ -199,11 +202,31 @@ rad_status ensure_out(Handle &h, size_t bytes)
     return RAD_OK;
 }
 
-rad_status check_handle(rad_handle *hh)
+// Makes the handle's device current for the duration of an entry point and restores the
+// caller's device afterwards (a call must not change the calling thread's current device).
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    cudaError_t enter(int device)
+    {
+        cudaError_t e = cudaGetDevice(&prev);
+        if (e != cudaSuccess) return e;
+        if (prev == device) return cudaSuccess;
+        e = cudaSetDevice(device);
+        switched = e == cudaSuccess;
+        return e;
+    }
+    ~DeviceGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
+};
+
+rad_status check_handle(rad_handle *hh, DeviceGuard &g)
 {
     if (!hh) return RAD_ERR_INVALID_ARG;
     if (hh->h.broken) return fail(&hh->h, RAD_ERR_STATE, "handle unusable after CUDA error: " + hh->h.err);
-    RAD_CUDA(&hh->h, cudaSetDevice(hh->h.device));
+    RAD_CUDA(&hh->h, g.enter(hh->h.device));
     return RAD_OK;
 }
 
@@ -236,9 +259,10 @@ rad_status build_tapered_table(Handle &h, long long n, int chunk, cudaStream_t s
     if (h.tap_n == n && h.tap_chunk == chunk && h.reg_chunk == -1) return RAD_OK;
     const long long gx = (h.n_wtiles + kWarpsPerBlock - 1) / kWarpsPerBlock;   // blocks per chunk
     const double chunks_per_wave = (double)h.sm_count * kMinBlocks / (double)gx;
-    const double tk = getenv("RAD_TAPER_K") ? atof(getenv("RAD_TAPER_K")) : 1.0;
-    const long long tmin = getenv("RAD_TAPER_MIN") ? atoll(getenv("RAD_TAPER_MIN")) : 128;
-    const double taper = std::max(2.0, tk * chunks_per_wave);
+    // taper factor 1-4 x chunks-per-wave and a floor of 64-256 particles measured within 0.4 % of
+    // each other; frozen at 1 x and 128
+    const long long tmin = 4 * kBatch;
+    const double taper = std::max(2.0, chunks_per_wave);
     std::vector<ChunkRec> recs;
     long long k = 0;
     while (k < n) {
@@ -283,10 +307,6 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.n_particles = n;
     // per-region calls: every region rounds its own chunk count up -> leave room for that
     p.chunk = choose_chunk(h, (region_off ? n + (long long)h.R * 64 : n) * n_steps);
-    if (const char *e = getenv("RAD_CHUNK")) {  // tuning/debug override (particles per block)
-        const int c = atoi(e);
-        if (c >= kBatch) p.chunk = c / kBatch * kBatch;
-    }
     p.n_dir = h.D; p.n_omega = h.W; p.w_pad = h.w_pad;
     p.n_ftiles = h.n_ftiles; p.n_wtiles = h.n_wtiles;
     p.dirs = h.dirs_d; p.F = h.F_d; p.Ff = h.Ff_d; p.fl = h.fl_d;
@@ -311,7 +331,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
         if (st_ != RAD_OK) return st_;
         n_chunks = h.reg_n_chunks;
         p.chunks = h.chunks_d;
-    } else if (!h.stream_nb && !h.deterministic && !getenv("RAD_NO_TAPER") &&
+    } else if (!h.stream_nb && !h.deterministic &&
                (long long)n_chunks * h.n_wtiles >= 4LL * h.sm_count * kMinBlocks * kWarpsPerBlock) {
         rad_status st_ = build_tapered_table(h, n, p.chunk, s);
         if (st_ != RAD_OK) return st_;
@@ -452,6 +472,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     h.stream_nb = (h.R > 1 || h.nyq_lim > 0.0) ? 0 : stream_shape(h.D, h.W, &h.stream_nd);
     // uniform grid?  w_j = w_0 + j dw to fp64 rounding -> rotation-recurrence kernel (a2')
     h.uniform = false;
+    double uni_dw = 0.0;
     if (h.W >= 2 * h.strip && !(cfg->flags & RAD_FLAG_FORCE_GENERAL) && h.nyq_lim == 0.0) {
         const double dw = (h.omega_h.back() - h.omega_h.front()) / (h.W - 1);
         bool uni = true;
@@ -461,18 +482,26 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
             const double step = dw / (2.0 * kPi) / h.f_unit * h.lw;  // rotator frequency, f_unit units
             const double G = std::nearbyint(step);
             h.uniform = true;
-            h.rot_G = (uint32_t)G; h.rot_Gf = (float)G; h.rot_gl = (float)(step - G);
+            // step can exceed 2^32 (lw > W - 1): the integer phase only needs G mod 2^32 (exact,
+            // F*T wraps mod one turn anyway); the fp32 copy multiplies the residual and stays unwrapped
+            h.rot_G = (uint32_t)((uint64_t)G & 0xffffffffull); h.rot_Gf = (float)G; h.rot_gl = (float)(step - G);
+            uni_dw = dw;
         }
     }
+    // Frequency tables.  Padded bins [W, w_pad) are never folded, but on a uniform grid a thread's
+    // rotation chain is anchored at its MIDDLE bin, which may be a padded one while lower bins of
+    // the strip are valid: there the tables continue the grid, w_j = w_0 + j dw (F mod 2^32 for the
+    // integer phase, the fp32 copy unwrapped); on a general grid padded bins stay 0.
     std::vector<uint32_t> F(h.w_pad, 0u);
     std::vector<float> Ff(h.w_pad, 0.0f), fl(h.w_pad, 0.0f);
-    for (int j = 0; j < h.W; ++j) {
-        const double fu = h.omega_h[j] / (2.0 * kPi) / h.f_unit;
+    for (int j = 0; j < (h.uniform ? h.w_pad : h.W); ++j) {
+        const double om = j < h.W ? h.omega_h[j] : h.omega_h[0] + j * uni_dw;
+        const double fu = om / (2.0 * kPi) / h.f_unit;
         const double Fi = std::nearbyint(fu);
-        F[j] = (uint32_t)Fi;
+        F[j] = (uint32_t)((uint64_t)Fi & 0xffffffffull);
         Ff[j] = (float)Fi;
         fl[j] = (float)(fu - Fi);
-        if (j < 16) { h.sF[j] = F[j]; h.sFf[j] = Ff[j]; h.sfl[j] = fl[j]; }
+        if (j < 16 && j < h.W) { h.sF[j] = F[j]; h.sFf[j] = Ff[j]; h.sfl[j] = fl[j]; }
     }
 
     cudaError_t e = cudaSetDevice(h.device);
@@ -517,7 +546,8 @@ rad_status rad_accumulate_step(rad_handle *hh, int64_t step_index, int64_t n_par
                                const void *by, const void *bz, const void *bdx, const void *bdy,
                                const void *bdz, const void *w, void *cuda_stream)
 {
-    rad_status st = check_handle(hh);
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     Handle &h = hh->h;
     if (h.R > 1) return fail(&h, RAD_ERR_INVALID_ARG, "per-region handle: use rad_accumulate_step_regions");
@@ -535,7 +565,8 @@ rad_status rad_accumulate_steps(rad_handle *hh, int64_t first_step_index, int32_
                                 const void *bdx, const void *bdy, const void *bdz, const void *w,
                                 void *cuda_stream)
 {
-    rad_status st = check_handle(hh);
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     Handle &h = hh->h;
     if (h.R > 1) return fail(&h, RAD_ERR_UNSUPPORTED, "rad_accumulate_steps on a per-region handle");
@@ -559,7 +590,8 @@ rad_status rad_accumulate_steps_regions(rad_handle *hh, int64_t first_step_index
                                         const void *bdx, const void *bdy, const void *bdz, const void *w,
                                         void *cuda_stream)
 {
-    rad_status st = check_handle(hh);
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     Handle &h = hh->h;
     st = check_regions(h, n_regions, region_offsets);
@@ -599,7 +631,8 @@ rad_status rad_accumulate_step_regions(rad_handle *hh, int64_t step_index, int32
                                        const void *bdx, const void *bdy, const void *bdz, const void *w,
                                        void *cuda_stream)
 {
-    rad_status st = check_handle(hh);
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     Handle &h = hh->h;
     st = check_regions(h, n_regions, region_offsets);
@@ -663,7 +696,8 @@ rad_status rad_accumulate_step_host(rad_handle *hh, int64_t step_index, int64_t 
                                     const void *by, const void *bz, const void *bdx, const void *bdy,
                                     const void *bdz, const void *w, void *cuda_stream)
 {
-    rad_status st = check_handle(hh);
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     Handle &h = hh->h;
     if (h.R > 1) return fail(&h, RAD_ERR_INVALID_ARG, "per-region handle: use rad_accumulate_step_regions_host");
@@ -682,7 +716,8 @@ rad_status rad_accumulate_step_regions_host(rad_handle *hh, int64_t step_index, 
                                             const void *bdy, const void *bdz, const void *w,
                                             void *cuda_stream)
 {
-    rad_status st = check_handle(hh);
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     Handle &h = hh->h;
     st = check_regions(h, n_regions, region_offsets);
@@ -696,8 +731,10 @@ rad_status rad_accumulate_step_regions_host(rad_handle *hh, int64_t step_index, 
                            (cudaStream_t)cuda_stream);
 }
 
-static rad_status deliver(Handle &h, double *out, int out_on_device, size_t bytes, cudaStream_t s,
-                          cudaError_t (*launch)(const Handle &, double *, cudaStream_t))
+}  // extern "C" (a template cannot have C linkage)
+
+template <typename Launch>
+static rad_status deliver(Handle &h, double *out, int out_on_device, size_t bytes, cudaStream_t s, Launch launch)
 {
     if (!out) return fail(&h, RAD_ERR_INVALID_ARG, "out is NULL");
     if (out_on_device < RAD_OUT_HOST || out_on_device > RAD_OUT_HOST_ASYNC)
@@ -716,9 +753,12 @@ static rad_status deliver(Handle &h, double *out, int out_on_device, size_t byte
     return RAD_OK;
 }
 
+extern "C" {
+
 rad_status rad_spectrum(rad_handle *hh, double *out, int out_on_device, void *cuda_stream)
 {
-    rad_status st = check_handle(hh);
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     return deliver(hh->h, out, out_on_device, (size_t)hh->h.R * hh->h.D * hh->h.W * sizeof(double),
                    (cudaStream_t)cuda_stream, launch_spectrum);
@@ -726,7 +766,8 @@ rad_status rad_spectrum(rad_handle *hh, double *out, int out_on_device, void *cu
 
 rad_status rad_spectrum_total(rad_handle *hh, double *out, int out_on_device, void *cuda_stream)
 {
-    rad_status st = check_handle(hh);
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     return deliver(hh->h, out, out_on_device, (size_t)hh->h.D * hh->h.W * sizeof(double),
                    (cudaStream_t)cuda_stream, launch_spectrum_total);
@@ -734,7 +775,8 @@ rad_status rad_spectrum_total(rad_handle *hh, double *out, int out_on_device, vo
 
 rad_status rad_amplitude(rad_handle *hh, double *out, int out_on_device, void *cuda_stream)
 {
-    rad_status st = check_handle(hh);
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     return deliver(hh->h, out, out_on_device, (size_t)hh->h.R * hh->h.D * hh->h.W * 6 * sizeof(double),
                    (cudaStream_t)cuda_stream, launch_amplitude);
@@ -742,7 +784,8 @@ rad_status rad_amplitude(rad_handle *hh, double *out, int out_on_device, void *c
 
 rad_status rad_add_amplitude(rad_handle *hh, const double *amp_device, void *cuda_stream)
 {
-    rad_status st = check_handle(hh);
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     if (!amp_device) return fail(&hh->h, RAD_ERR_INVALID_ARG, "amp_device is NULL");
     RAD_CUDA(&hh->h, launch_add_amplitude(hh->h, amp_device, (cudaStream_t)cuda_stream));
@@ -750,9 +793,49 @@ rad_status rad_add_amplitude(rad_handle *hh, const double *amp_device, void *cud
     return RAD_OK;
 }
 
+rad_status rad_export_accumulator(rad_handle *hh, double *out_device, void *cuda_stream)
+{
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
+    if (st != RAD_OK) return st;
+    Handle &h = hh->h;
+    if (!out_device) return fail(&h, RAD_ERR_INVALID_ARG, "out_device is NULL");
+    // rows of W*4 doubles out of the padded [R*D][w_pad][4] accumulator; a memcpy keeps its full
+    // stream dependencies under RAD_FLAG_OVERLAP_STEPS (it runs after every fold queued before)
+    const size_t row = (size_t)h.W * 4 * sizeof(double);
+    RAD_CUDA(&h, cudaMemcpy2DAsync(out_device, row, h.acc_d, (size_t)h.w_pad * 4 * sizeof(double), row,
+                                   (size_t)h.R * h.D, cudaMemcpyDeviceToDevice, (cudaStream_t)cuda_stream));
+    return RAD_OK;
+}
+
+rad_status rad_import_accumulator(rad_handle *hh, const double *amp4_device, void *cuda_stream)
+{
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
+    if (st != RAD_OK) return st;
+    if (!amp4_device) return fail(&hh->h, RAD_ERR_INVALID_ARG, "amp4_device is NULL");
+    RAD_CUDA(&hh->h, launch_import_accumulator(hh->h, amp4_device, (cudaStream_t)cuda_stream));
+    hh->h.launches += 1;
+    return RAD_OK;
+}
+
+rad_status rad_spectrum_of(rad_handle *hh, const double *amp4_device, double *out, int out_on_device,
+                           void *cuda_stream)
+{
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
+    if (st != RAD_OK) return st;
+    if (!amp4_device) return fail(&hh->h, RAD_ERR_INVALID_ARG, "amp4_device is NULL");
+    return deliver(hh->h, out, out_on_device, (size_t)hh->h.R * hh->h.D * hh->h.W * sizeof(double),
+                   (cudaStream_t)cuda_stream, [amp4_device](const Handle &h, double *o, cudaStream_t s) {
+                       return launch_spectrum_of(h, amp4_device, o, s);
+                   });
+}
+
 rad_status rad_reset(rad_handle *hh, void *cuda_stream)
 {
-    rad_status st = check_handle(hh);
+    DeviceGuard guard;
+    rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     Handle &h = hh->h;
     RAD_CUDA(&h, cudaMemsetAsync(h.acc_d, 0, (size_t)h.R * h.D * h.w_pad * 4 * sizeof(double),
@@ -763,11 +846,14 @@ rad_status rad_reset(rad_handle *hh, void *cuda_stream)
 void rad_destroy(rad_handle *hh)
 {
     if (!hh) return;
-    if (cudaSetDevice(hh->h.device) == cudaSuccess) {
-        cudaDeviceSynchronize();
-        free_all(hh->h);
+    {
+        DeviceGuard guard;
+        if (guard.enter(hh->h.device) == cudaSuccess) {
+            cudaDeviceSynchronize();
+            free_all(hh->h);
+        }
+        cudaGetLastError();
     }
-    cudaGetLastError();
     delete hh;
 }
 

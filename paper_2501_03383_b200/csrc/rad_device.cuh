@@ -17,22 +17,13 @@ constexpr float kUnitToRad = 1.4629180792671596e-09f;  // 2 pi / 2^32
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
-// state element -> fp64.  fp32 -> fp64 by integer ops (exponent re-bias) instead of F2F.F64.F32:
-// the conversion unit shares the XU pipe with MUFU.SIN/COS, the bound of the whole path, while
-// the integer pipe idles.  Exact for normal numbers; 0 maps to 2^-127 (5.9e-39, harmless: the
-// value only enters sums with terms >= 1e-30 larger); denormals/Inf/NaN are not meaningful
-// particle state.
+// state element -> fp64: exact for every fp32 value (zero, subnormals, Inf and NaN included, so
+// non-finite particle state propagates into the result as include/rad.h documents).
+// F2F.F64.F32 is not an XU-rate instruction (>= 61 results/clk/SM, bench.py alu_peaks), unlike the
+// opposite direction; round 1's integer-pipe version mapped 0 to 2^-127 and Inf/NaN to finite
+// values for no measurable gain.
 __device__ __forceinline__ double to_f64(double x) { return x; }
-__device__ __forceinline__ double to_f64(float x)
-{
-#ifdef RAD_F2D_XU
-    return (double)x;
-#else
-    const uint32_t u = __float_as_uint(x);
-    const uint32_t hi = (u & 0x80000000u) | (((u & 0x7fffffffu) >> 3) + 0x38000000u);
-    return __hiloint2double((int)hi, (int)(u << 29));
-#endif
-}
+__device__ __forceinline__ double to_f64(float x) { return (double)x; }
 
 // fp64 -> fp32 as ONE F2F: with -ftz the plain cast also emits a DSETP + select per conversion
 // to flush fp32 subnormals, which these values (|x| >= 1e-30 or exactly 0) never are.
@@ -90,6 +81,7 @@ __device__ __forceinline__ void stage_record(const Particle &p, const DirRec &dr
 __device__ __forceinline__ int nyquist_count(const AccumParams &P, double d)
 {
     int lo = 0, hi = P.n_omega;
+    if (d != d) return hi;  // NaN state: the comparison is false for every bin, nothing is dropped (NaN propagates)
     while (lo < hi) {
         const int mid = (lo + hi) >> 1;
         if (__dmul_rn(__dmul_rn(__ldg(P.omega64 + mid), P.dt64), d) < P.nyq_lim) lo = mid + 1;
@@ -103,11 +95,7 @@ __device__ __forceinline__ void phase_sincos(uint32_t F, float Ff, float fl, uin
                                              float sf, float &sn, float &cs)
 {
     const uint32_t u = F * T;
-#ifdef RAD_CENTER
-    const float v = __uint_as_float(0x3f800000u | (u >> 9)) - 1.5f;  // frac - 1/2 in turns (exact)
-#else
     const float v = __uint_as_float(0x3f800000u | (u >> 9));  // 1 + frac, in turns
-#endif
     const float q = fmaf(fl, sf, Ff * ql);
     __sincosf(fmaf(v, kTwoPi, q), &sn, &cs);
 }

@@ -101,6 +101,21 @@ __global__ void rad_spectrum_total_kernel(const double *__restrict__ acc, double
     out[b] = scale * (s0 * s0 + s1 * s1 + s2 * s2 + s3 * s3);
 }
 
+// A += amp4 (compact [rows][W][4] -> padded [rows][w_pad][4])
+__global__ void rad_import_accumulator_kernel(double *__restrict__ acc, const double *__restrict__ amp4,
+                                              int rows, int W, int w_pad)
+{
+    const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= (long long)rows * W) return;
+    const int d = (int)(b / W), j = (int)(b - (long long)d * W);
+    const double2 *in = reinterpret_cast<const double2 *>(amp4 + (size_t)b * 4);
+    double2 *a = reinterpret_cast<double2 *>(acc + ((size_t)d * w_pad + j) * 4);
+    const double2 i0 = in[0], i1 = in[1];
+    double2 a0 = a[0], a1 = a[1];
+    a0.x += i0.x; a0.y += i0.y; a1.x += i1.x; a1.y += i1.y;
+    a[0] = a0; a[1] = a1;
+}
+
 inline unsigned blocks_for(long long n, int t) { return (unsigned)((n + t - 1) / t); }
 
 }  // namespace
@@ -134,6 +149,21 @@ cudaError_t launch_reduce_partials(const Handle &h, const double *partial, int n
     const int R = region_chunk_start ? h.R : 1;
     rad_reduce_partials_kernel<<<blocks_for(n * R, 256), 256, 0, s>>>(h.acc_d, partial, n, n_chunks, R,
                                                                      region_chunk_start);
+    return cudaGetLastError();
+}
+
+// |A|^2 of a compact amplitude buffer (rad_export_accumulator layout: row pitch W, not w_pad)
+cudaError_t launch_spectrum_of(const Handle &h, const double *amp4_dev, double *out_dev, cudaStream_t s)
+{
+    const long long n = (long long)h.R * h.D * h.W;
+    return launch_kernel(rad_spectrum_kernel, dim3(blocks_for(n, 256)), dim3(256), 0, s, h.overlap, amp4_dev, out_dev,
+                         h.R * h.D, h.W, h.W, h.scale);
+}
+
+cudaError_t launch_import_accumulator(const Handle &h, const double *amp4_dev, cudaStream_t s)
+{
+    const long long n = (long long)h.R * h.D * h.W;
+    rad_import_accumulator_kernel<<<blocks_for(n, 256), 256, 0, s>>>(h.acc_d, amp4_dev, h.R * h.D, h.W, h.w_pad);
     return cudaGetLastError();
 }
 

@@ -18,30 +18,14 @@ constexpr double kTwo32 = 4294967296.0;        // 2^32
 constexpr int kWarpsPerBlock = 4;              // one warp per SM sub-partition
 constexpr int kThreads = 32 * kWarpsPerBlock;
 constexpr int kBatch = 32;                     // particles staged per warp batch (one per lane)
-#ifndef RAD_STRIP
-#define RAD_STRIP 8
-#endif
-#ifndef RAD_MINB
-#define RAD_MINB 4
-#endif
-#ifndef RAD_POLY_EVEN
-#define RAD_POLY_EVEN 0
-#endif
-#ifndef RAD_POLY_ODD
-#define RAD_POLY_ODD 1
-#endif
 // general kernel, hybrid sincos: bins (of the 8-bin strip) per even / odd particle of a batch
 // that take the FMA-pipe polynomial instead of the XU pipe (0 = pure MUFU).  Measured on B200
 // (cfg 1 / cfg 2, % of R_gen): (0,0) 85.4 / 88.6, (0,1) 88.3 / 91.3, (0,2) 87.1 / 89.6,
 // (1,1) 84.7 / 87.5, (1,2) 88.4 / 90.8, (0,3) 84.0 / 86.6, (2,2) 81.6 / 84.0; cfg 3d (8 lanes
-// along frequency): 82.5 -> 84.6.  RAD_POLY_MINLW: narrowest tile shape that uses it.
-constexpr int kPolyEven = RAD_POLY_EVEN, kPolyOdd = RAD_POLY_ODD;
-#ifndef RAD_POLY_MINLW
-#define RAD_POLY_MINLW 4
-#endif
-constexpr int kPolyMinLW = RAD_POLY_MINLW;
-constexpr int kStrip = RAD_STRIP;              // frequency bins per thread (register strip)
-constexpr int kMinBlocks = RAD_MINB;           // resident blocks per SM the kernels are bounded for
+// along frequency): 82.5 -> 84.6.  Frozen at (0,1) for every tile shape.
+constexpr int kPolyEven = 0, kPolyOdd = 1;
+constexpr int kStrip = 8;                      // frequency bins per thread (register strip)
+constexpr int kMinBlocks = 4;                  // resident blocks per SM the kernels are bounded for
 
 // Per direction (device table).  k = n * (f_unit 2^32 / c): the dot product k.r is the
 // light-travel delay n.r/c measured in units of 2^-32 "unit turns" (phase).
@@ -134,6 +118,8 @@ cudaError_t launch_add_amplitude(const Handle &h, const double *amp_dev, cudaStr
 cudaError_t launch_reduce_partials(const Handle &h, const double *partial, int n_chunks,
                                    const int *region_chunk_start, cudaStream_t s);
 cudaError_t launch_spectrum_total(const Handle &h, double *out_dev, cudaStream_t s);
+cudaError_t launch_spectrum_of(const Handle &h, const double *amp4_dev, double *out_dev, cudaStream_t s);
+cudaError_t launch_import_accumulator(const Handle &h, const double *amp4_dev, cudaStream_t s);
 
 struct Handle {
     int device = 0;

@@ -226,8 +226,8 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
             };
 #pragma unroll 1
             for (int kk = 0; kk < kBatch; kk += 2) {
-                sweep_one(kk, LW >= kPolyMinLW ? kPolyEven : 0);
-                sweep_one(kk + 1, LW >= kPolyMinLW ? kPolyOdd : 0);
+                sweep_one(kk, kPolyEven);
+                sweep_one(kk + 1, kPolyOdd);
             }
         }
         __syncwarp();

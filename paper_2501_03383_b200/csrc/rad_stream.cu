@@ -12,8 +12,6 @@
 // last tile fall back to coalesced ld.global.nc.  At the end the partials go through
 // warp-shuffle reductions, a shared-memory cross-warp sum and one fp64 atomic per value
 // per block (or the deterministic workspace).
-#include <cstdlib>
-
 #include "rad_device.cuh"
 #include "rad_internal.h"
 
@@ -23,22 +21,12 @@ namespace {
 
 using namespace dev;
 
-#ifndef RAD_S_STAGES
-#define RAD_S_STAGES 2
-#endif
-#ifndef RAD_S_TILEBYTES
-#define RAD_S_TILEBYTES 4096
-#endif
-#ifndef RAD_S_UNROLL
-#define RAD_S_UNROLL 4
-#endif
-#ifndef RAD_S_MINB
-#define RAD_S_MINB 2
-#endif
+// Shape of the ring, frozen from the round-1 sweeps.
 constexpr int kSThreads = 256;
-constexpr int kSStages = RAD_S_STAGES;
-constexpr int kSUnroll = RAD_S_UNROLL;
-constexpr int kSTileBytes = RAD_S_TILEBYTES;  // per array per stage -> 1024 fp32 / 512 fp64 particles
+constexpr int kSStages = 2;
+constexpr int kSUnroll = 4;
+constexpr int kSMinBlocks = 2;
+constexpr int kSTileBytes = 4096;  // per array per stage -> 1024 fp32 / 512 fp64 particles
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -96,7 +84,7 @@ __device__ __forceinline__ Particle make_particle(ST rx, ST ry, ST rz, ST bx, ST
 // WIN: spatial window compiled in (kept out of the default instantiation: the streaming kernel
 // is latency bound and loses 3 % to the extra per-particle code even when the window is off)
 template <typename ST, int NB, int ND, bool WIN>
-__global__ void __launch_bounds__(kSThreads, NB <= 8 ? RAD_S_MINB : 1) rad_accum_stream(const AccumParams P, const int use_bulk)
+__global__ void __launch_bounds__(kSThreads, NB <= 8 ? kSMinBlocks : 1) rad_accum_stream(const AccumParams P, const int use_bulk)
 {
     constexpr int TILE = kSTileBytes / (int)sizeof(ST);  // particles per tile
     constexpr int PPT = TILE / kSThreads;                 // particles per thread per tile
@@ -223,7 +211,7 @@ cudaError_t launch_stream_w(const AccumParams &p, int grid, cudaStream_t s, bool
     cudaError_t e = cudaFuncSetAttribute(rad_accum_stream<ST, NB, ND, WIN>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    int use_bulk = getenv("RAD_STREAM_PLAIN") ? 0 : 1;  // debug: force the plain-load path
+    int use_bulk = 1;
     for (int a = 0; a < 10; ++a)
         if (reinterpret_cast<uintptr_t>(p.st[a]) & 15) use_bulk = 0;
     return launch_kernel(rad_accum_stream<ST, NB, ND, WIN>, dim3(grid), dim3(kSThreads), smem, s, overlap, p, use_bulk);
@@ -246,7 +234,7 @@ cudaError_t dispatch_stream(const Handle &h, const AccumParams &p, int grid, cud
 }  // namespace
 
 int stream_tile_particles(bool state_f64) { return kSTileBytes / (state_f64 ? 8 : 4); }
-int stream_blocks_per_sm(int nb) { return nb <= 8 ? RAD_S_MINB : 1; }
+int stream_blocks_per_sm(int nb) { return nb <= 8 ? kSMinBlocks : 1; }
 
 // Shapes served: ND in {1, 2} directions x WB = NB/ND frequencies, NB in {8, 16}.
 // Returns NB (and *nd), or 0 if this detector shape is not a streaming shape.

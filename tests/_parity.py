@@ -67,3 +67,21 @@ def stratified_bins(D, W, n_dir=4, n_om=8, extra=()):
     js = np.unique(np.linspace(0, W - 1, min(n_om, W)).round().astype(int))
     flat = (ds[:, None] * W + js[None, :]).ravel()
     return np.unique(np.concatenate([flat, np.asarray(extra, dtype=np.int64)])).astype(np.int64)
+
+
+def tile_cover_bins(D, W, block=32, n_random=0, seed=1, extra=()):
+    """Flat indices of a bin sample that reaches every warp tile of the accumulate kernels: in
+    EVERY direction, one bin (seeded random position) in every block of `block` consecutive
+    frequencies -- a warp tile is 32/lw directions x lw*8 frequencies with lw in {4, 8, 16, 32},
+    i.e. >= 1 direction x >= 32 frequencies, so block = 32 puts a sample into every (direction
+    group, frequency tile) pair whatever tile shape rad_create picked (block = 64 does for
+    lw >= 8).  Plus `n_random` bins drawn uniformly, the first and last frequency of the first
+    and last direction, and `extra` (e.g. the GPU arg-max bin)."""
+    rng = np.random.default_rng(seed)
+    starts = np.arange(0, W, block)
+    width = np.minimum(block, W - starts)
+    pos = starts[None, :] + (rng.random((D, starts.shape[0])) * width[None, :]).astype(np.int64)
+    flat = (np.arange(D, dtype=np.int64)[:, None] * W + pos).ravel()
+    rnd = rng.integers(0, D * W, size=n_random, dtype=np.int64)
+    corners = np.array([0, W - 1, (D - 1) * W, D * W - 1], dtype=np.int64)
+    return np.unique(np.concatenate([flat, rnd, corners, np.asarray(extra, dtype=np.int64)])).astype(np.int64)

@@ -50,6 +50,55 @@ def test_uniform_grid_recurrence_kernel(oracle_mod, D, W, dtype):
     print(f"uniform {D}x{W} relL2={l2:.2e} maxrel={mr:.2e}")
 
 
+@pytest.mark.parametrize("D,W", [(1, 40), (3, 16), (2, 20), (4, 24), (1, 100), (8, 70), (1, 17), (1, 31), (5, 257)])
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_uniform_grid_padded_anchor_shapes(oracle_mod, D, W, dtype):
+    """Linear grids whose width is not a multiple of the frequency tile: a thread's chain anchor
+    (its middle bin) is then a PADDED bin while lower bins of its strip are valid, so the padded
+    part of the frequency tables must continue the grid (round-1 bug: every bin of 1x40, 3x16,
+    2x20, 4x24 was wrong).  W = 17, 31 with one direction also make the rotator step exceed
+    2^32 f_unit (32 lanes along frequency, lw > W - 1)."""
+    w = wl.Workload("lin_pad", 700, 2, 1e-17, wl.dirs_fibonacci(max(D, 2))[:D], np.linspace(3e14, 3e17, W), dtype,
+                    wl.BASE_SEED + 21, "khi")
+    steps = [(t * 300 + 1, st) for t, st in w.steps(n_steps=2)]
+    S, variant = P.run_gpu(w, steps)
+    assert variant == "uniform"
+    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    l2, mr = P.assert_parity(S, ref, what=f"uniform padded {D}x{W}")
+    for d in range(D):
+        P.assert_parity(S[d], ref[d], what=f"uniform padded {D}x{W} dir {d}")
+    from paper_2501_03383_b200 import binding
+    Sg, vg = P.run_gpu(w, steps, flags=binding.RAD_FLAG_FORCE_GENERAL)
+    assert vg == "general" and P.rel_l2(S, Sg) < 1e-5
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("shape", ["general", "uniform", "stream"])
+def test_non_finite_particle_state_propagates(dtype, shape):
+    """include/rad.h: particle values are not scanned; NaN/Inf in the state give NaN/Inf in the
+    result.  One NaN (or Inf) particle among 500 must poison every bin it contributes to, on every
+    kernel, for fp32 and fp64 state alike (round 1 mapped fp32 Inf/NaN positions to finite numbers)."""
+    from paper_2501_03383_b200 import binding
+    if shape == "stream":
+        dirs, omega = wl.dirs_fibonacci(2)[:1], wl.omega_log(8)
+    elif shape == "uniform":
+        dirs, omega = wl.dirs_fibonacci(3), np.linspace(2e14, 4e16, 48)
+    else:
+        dirs, omega = wl.dirs_fibonacci(3), wl.omega_log(40)
+    w = wl.Workload("nonfinite", 500, 1, 1e-17, dirs, omega, dtype, wl.BASE_SEED + 60, "khi")
+    (t, st), = list(w.steps())
+    for col, bad in ((0, np.nan), (1, np.inf), (4, np.nan), (7, np.nan), (9, np.inf)):
+        st2 = [a.copy() for a in st]
+        st2[col][123] = bad
+        with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, state_dtype=dtype) as det:
+            det.accumulate_step(0, P.to_device(st2))
+            S, variant = det.spectrum(), det.kernel_variant
+        assert variant == shape
+        assert not np.isfinite(S).any(), f"column {col} = {bad}: finite bins remain"
+    S_ok, _ = P.run_gpu(w, [(0, st)])
+    assert np.isfinite(S_ok).all()
+
+
 @pytest.mark.parametrize("cfg", ["1", "2", "3a", "3b", "3c", "3d", "4"])
 def test_reduced_particles_all_bins(oracle_mod, cfg):
     """Every bin / tile path of configs 1-4 on a reduced workload (first 1000 particles --
@@ -181,48 +230,95 @@ def test_edge_cases(oracle_mod):
 
 
 # ------------------------------------------------------------------ full sizes, sampled bins
-def _full_size_sampled(oracle_mod, cfg, n_steps, n_dir=3, n_om=6):
-    """BASELINE.json's full particle count in the launch configuration bench.py times
-    (same handle set-up, same per-step call); the oracle computes a stratified sample of
-    bins plus the GPU arg-max bin one by one (bins are independent sums)."""
+def _full_size_sampled(oracle_mod, cfg, n_steps, bins, flag_sets=None, check_argmax=True):
+    """BASELINE.json's full particle count in the launch configurations bench.py times: the same
+    handle set-up and per-step call, once with flags = 0 and once with RAD_FLAG_OVERLAP_STEPS
+    (bench.py's default).  The oracle computes the sampled `bins` one by one (bins are independent
+    sums) ONCE; both GPU runs are compared with it, and the GPU arg-max bin (the S_peak of the
+    maxrel criterion) is verified by a second, one-bin oracle pass."""
     import torch
     from paper_2501_03383_b200 import binding
     w = wl.make_workload(cfg)
-    bins = P.stratified_bins(w.n_dir, w.n_omega, n_dir, n_om)
+    flag_sets = (0, binding.RAD_FLAG_OVERLAP_STEPS) if flag_sets is None else flag_sets
     o = oracle_mod.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=bins)
-    first = None
-    with binding.Detector(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, state_dtype=w.state_dtype) as det:
+    dets = [binding.Detector(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, state_dtype=w.state_dtype, flags=f)
+            for f in flag_sets]
+    kept = []
+    try:
+        block = []                              # steps are queued in blocks, back to back, so that the
+        def flush():                            # kernels of consecutive steps really overlap under the flag
+            devs = [P.to_device(st) for _, st in block]
+            torch.cuda.synchronize()            # the flag's input contract: inputs complete before the calls
+            for det in dets:
+                for (t, _), dev in zip(block, devs):
+                    det.accumulate_step(t, dev)
+            for t, st in block:                 # the oracle works while the GPU does
+                o.accumulate_step(t, *st)
+            torch.cuda.synchronize()            # inputs stay alive until the kernels are done
+            block.clear()
         for t, st in w.steps(n_steps=n_steps):
-            det.accumulate_step(t, P.to_device(st))
-            o.accumulate_step(t, *st)
-            first = first or st
-        torch.cuda.synchronize()
-        S = det.spectrum()
-    jmax = int(np.argmax(S))
+            block.append((t, st))
+            if check_argmax and n_steps <= 4:
+                kept.append((t, st))
+            if len(block) == 50:
+                flush()
+        if block:
+            flush()
+        spectra = [det.spectrum() for det in dets]
+    finally:
+        for det in dets:
+            det.close()
     Sref = o.spectrum().ravel()[bins]
-    l2, mr = P.assert_parity(S.ravel()[bins], Sref, peak=S.max(), what=f"cfg{cfg} full-size sample")
-    if n_steps == 1:  # the arg-max bin itself, verified separately (cheap for one step)
+    for f, S in zip(flag_sets, spectra):
+        l2, mr = P.assert_parity(S.ravel()[bins], Sref, peak=S.max(), what=f"cfg{cfg} full-size sample flags={f}")
+        print(f"cfg{cfg} full-size flags={f}: {len(bins)} bins relL2={l2:.2e} maxrel={mr:.2e}")
+    if kept:       # the arg-max bin itself
+        jmax = int(np.argmax(spectra[0]))
         om = oracle_mod.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=np.array([jmax]))
-        om.accumulate_step(0, *first)
-        assert S.ravel()[jmax] == pytest.approx(om.spectrum().ravel()[jmax], rel=1e-4)
-    print(f"cfg{cfg} full-size: {len(bins)} bins relL2={l2:.2e} maxrel={mr:.2e}")
+        for t, st in kept:
+            om.accumulate_step(t, *st)
+        for S in spectra:
+            assert int(np.argmax(S)) == jmax
+            assert S.ravel()[jmax] == pytest.approx(om.spectrum().ravel()[jmax], rel=1e-4)
 
 
 def test_cfg1_full_workload_all_1000_steps(oracle_mod):
-    _full_size_sampled(oracle_mod, "1", 1000, n_dir=3, n_om=5)
+    """All 1000 steps of config 1 (late step indices, t up to 1e-14 s) on 64 + 4 sampled bins."""
+    w = wl.make_workload("1")
+    bins = P.tile_cover_bins(w.n_dir, w.n_omega, block=512, n_random=0, seed=11)[::2]
+    _full_size_sampled(oracle_mod, "1", 1000, bins, check_argmax=False)
+
+
+def test_cfg1_full_particles_every_tile(oracle_mod):
+    """Config 1 at its full particle count x 4 steps: >= 2048 oracle-checked bins, one in every
+    (direction, 32-frequency block) -> every warp tile, every chunk of the tapered schedule."""
+    w = wl.make_workload("1")
+    bins = P.tile_cover_bins(w.n_dir, w.n_omega, block=32, n_random=2048, seed=12)
+    assert len(bins) >= 2048
+    _full_size_sampled(oracle_mod, "1", 4, bins)
 
 
 @pytest.mark.parametrize("cfg", ["3a", "3b", "3c", "3d"])
 def test_cfg3_full_particles(oracle_mod, cfg):
-    _full_size_sampled(oracle_mod, cfg, 4, n_dir=3, n_om=6)
+    w = wl.make_workload(cfg)
+    bins = P.tile_cover_bins(w.n_dir, w.n_omega, block=32, n_random=64, seed=13)
+    assert len(bins) >= 2048
+    _full_size_sampled(oracle_mod, cfg, 4, bins)
 
 
 def test_cfg2_full_particles(oracle_mod):
-    _full_size_sampled(oracle_mod, "2", 2, n_dir=3, n_om=6)
+    """The headline configuration: 1 048 576 particles, 256 x 1024 bins (lw = 32: warp tile = one
+    direction x 256 frequencies, so a 64-frequency block puts 4 samples into every tile)."""
+    w = wl.make_workload("2")
+    bins = P.tile_cover_bins(w.n_dir, w.n_omega, block=64, n_random=64, seed=14)
+    assert len(bins) >= 4096
+    _full_size_sampled(oracle_mod, "2", 2, bins)
 
 
 def test_cfg4_full_particles(oracle_mod):
-    _full_size_sampled(oracle_mod, "4", 1, n_dir=3, n_om=6)
+    w = wl.make_workload("4")
+    bins = P.tile_cover_bins(w.n_dir, w.n_omega, block=32, n_random=64, seed=15)
+    _full_size_sampled(oracle_mod, "4", 1, bins)
 
 
 # --------------------------------------------------------------- particle-streaming kernel
@@ -268,7 +364,7 @@ def test_stream_kernel_unaligned_arrays_use_plain_loads(oracle_mod):
 
 
 def test_cfg4b_full_particles(oracle_mod):
-    _full_size_sampled(oracle_mod, "4b", 1, n_dir=1, n_om=8)
+    _full_size_sampled(oracle_mod, "4b", 1, np.arange(8, dtype=np.int64))
 
 
 # ------------------------------------------------------------------ multi-step calls
@@ -356,30 +452,55 @@ def test_spectrum_to_pinned_host_async():
 
 
 def test_multi_gpu_plumbing_on_one_device(oracle_mod):
-    """multi.global_spectrum (export A, all-reduce, import into a second handle, |A|^2) is the
-    path bench.py --gpus N takes; with no process group the all-reduce is the identity, so the
-    result must equal the local spectrum, and two 'ranks' emulated by two handles on particle
-    shards must sum to the oracle of all particles."""
+    """The path bench.py --gpus N takes (multi.AmplitudeAllReduce: rad_export_accumulator -> all-reduce
+    -> rad_spectrum_of on a side stream), emulated on one device: with no process group the
+    all-reduce is the identity, so every queued global spectrum must equal the local spectrum of
+    that step; and two 'ranks' = two handles on particle shards, whose exported accumulators are
+    added (what the all-reduce delivers), must give the oracle's spectrum of all particles.
+    rad_import_accumulator folds one rank's amplitude into the other's handle (same result)."""
     import torch
     from paper_2501_03383_b200 import binding, multi
     w = wl.make_workload("3b")
-    steps = list(w.steps(n_steps=2, n_particles=1500))
-    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
-    dets = [binding.Detector(w.dirs, w.omega, w.dt, scale=1.0) for _ in range(3)]
+    T = 5
+    steps = list(w.steps(n_steps=T, n_particles=1500))
+    o = oracle_mod.Oracle(w.dirs, w.omega, w.dt, scale=1.0)
+    dets = [binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, flags=binding.RAD_FLAG_OVERLAP_STEPS)
+            for _ in range(2)]
     try:
-        amp = [torch.empty(w.n_dir, w.n_omega, 3, 2, dtype=torch.float64, device="cuda") for _ in range(2)]
-        for r in range(2):
-            b, e = multi.shard_range(1500, r, 2)
-            for t, st in steps:
-                dets[r].accumulate_step(t, P.to_device([a[b:e] for a in st]))
-            dets[r].amplitude(out=amp[r])
-        out = torch.empty(w.n_dir, w.n_omega, dtype=torch.float64, device="cuda")
-        multi.global_spectrum(dets[0], dets[2], amp[0], out=out)      # world size 1: identity
+        dev = [[P.to_device([a[slice(*multi.shard_range(1500, r, 2))] for a in st]) for _, st in steps]
+               for r in range(2)]
         torch.cuda.synchronize()
-        assert np.allclose(out.cpu().numpy(), dets[0].spectrum(), rtol=1e-12, atol=0)   # xyz round trip
-        dets[2].reset()
-        dets[2].add_amplitude(amp[0] + amp[1])                       # what the all-reduce delivers
-        P.assert_parity(dets[2].spectrum(), ref, what="two shards summed")
+        red = multi.AmplitudeAllReduce(dets[0])
+        outs = [torch.empty(w.n_dir, w.n_omega, dtype=torch.float64, device="cuda") for _ in range(T)]
+        plain = []
+        for i, (t, _) in enumerate(steps):          # every step: accumulate, queue the exchange, go on
+            dets[0].accumulate_step(t, dev[0][i])
+            red.global_spectrum(out=outs[i])
+        red.wait()
+        torch.cuda.synchronize()
+        with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0) as chk:   # rank 0's running spectrum, step by step
+            for i, (t, _) in enumerate(steps):
+                chk.accumulate_step(t, dev[0][i])
+                plain.append(chk.spectrum())
+        for i in range(T):
+            assert np.allclose(outs[i].cpu().numpy(), plain[i], rtol=1e-9, atol=1e-12 * plain[-1].max()), f"step {i}"
+        red.close()
+        for t, st in steps:
+            o.accumulate_step(t, *st)
+        for i, (t, _) in enumerate(steps):
+            dets[1].accumulate_step(t, dev[1][i])
+        amp = [torch.empty(w.n_dir, w.n_omega, 4, dtype=torch.float64, device="cuda") for _ in range(2)]
+        for r in range(2):
+            dets[r].export_accumulator(amp[r])
+        total = amp[0] + amp[1]                                  # what the all-reduce delivers
+        ref = o.spectrum()
+        P.assert_parity(dets[0].spectrum_of(total), ref, what="two shards summed")
+        P.assert_parity(dets[1].spectrum_of(total), ref, what="two shards summed (other rank's handle)")
+        dets[0].import_accumulator(amp[1])
+        P.assert_parity(dets[0].spectrum(), ref, what="import_accumulator")
+        # the 4-component export carries the whole amplitude: A1 e1 + A2 e2 == rad_amplitude
+        A = dets[0].amplitude()
+        assert np.abs(A - o.amplitude()).max() <= 2e-5 * np.abs(o.amplitude()).max()
     finally:
         for d in dets:
             d.close()
@@ -584,7 +705,9 @@ def test_checkpoint_resume_through_amplitude_export(oracle_mod):
 def test_cfg2_full_workload_all_2000_steps(oracle_mod):
     """BASELINE.json configs[2] in full (1 048 576 particles x 2000 steps x 256 x 1024 bins =
     5.5e14 updates on the GPU); the oracle follows on 12 stratified bins (2.5e10 updates)."""
-    _full_size_sampled(oracle_mod, "2", 2000, n_dir=3, n_om=4)
+    w = wl.make_workload("2")
+    _full_size_sampled(oracle_mod, "2", 2000, P.stratified_bins(w.n_dir, w.n_omega, 3, 4), flag_sets=(0,),
+                       check_argmax=False)
 
 
 @pytest.mark.parametrize("cfg,n", [("5r", 40000), ("3c", 9000), ("4b", 50000), ("0", 256), ("3d", 3000)])
@@ -631,3 +754,104 @@ def test_overlap_steps_flag_keeps_every_intermediate_spectrum(oracle_mod, cfg, n
     for r in range(R):
         sl = slice(r * w.n_dir, (r + 1) * w.n_dir)
         P.assert_parity(over[-1][sl], ref[sl], what=f"overlap cfg{cfg} region {r}")
+
+
+@pytest.mark.parametrize("shape", ["general", "uniform", "stream", "regions"])
+def test_overlap_plus_deterministic_is_bit_identical_to_deterministic(oracle_mod, shape):
+    """include/rad.h: RAD_FLAG_OVERLAP_STEPS "combines with RAD_FLAG_DETERMINISTIC (results stay
+    bit-identical)".  12 short steps back to back, a spectrum after every step, on the general,
+    uniform, streaming and per-region handles: every intermediate spectrum of the
+    OVERLAP|DETERMINISTIC run equals the DETERMINISTIC run's bit for bit (the workspace of step
+    i+1 must not be written before step i's reduction has read it), the last one meets the oracle."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    R, n, T = 1, 20000, 12
+    if shape == "general":
+        dirs, omega = wl.dirs_fibonacci(6), wl.omega_log(96)
+    elif shape == "uniform":
+        dirs, omega = wl.dirs_fibonacci(6), np.linspace(2e14, 6e16, 96)
+    elif shape == "stream":
+        dirs, omega, n = wl.dirs_fibonacci(2)[:1], wl.omega_log(8), 60000
+    else:
+        dirs, omega, R = wl.dirs_fibonacci(3), wl.omega_log(64), 4
+    w = wl.Workload("detov", n, T, 1e-17, dirs, omega, np.float32, wl.BASE_SEED + 70, "khi")
+    steps = list(w.steps())
+    dev = [P.to_device(st) for _, st in steps]
+    off = np.array([0, n // 7, n // 7, n // 2, n], dtype=np.int64) if R > 1 else None
+
+    def run(flags):
+        outs = [torch.zeros(R * w.n_dir, w.n_omega, dtype=torch.float64, device="cuda") for _ in range(T)]
+        with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, flags=flags, n_regions=R if R > 1 else 0) as det:
+            for rep in range(2):
+                det.reset()
+                torch.cuda.synchronize()
+                for i, (t, _) in enumerate(steps):
+                    if R > 1:
+                        det.accumulate_step_regions(t, off, dev[i])
+                    else:
+                        det.accumulate_step(t, dev[i])
+                    det.spectrum(out=outs[i])
+            torch.cuda.synchronize()
+            variant = det.kernel_variant
+        return [o.cpu().numpy() for o in outs], variant
+
+    det_only, v0 = run(binding.RAD_FLAG_DETERMINISTIC)
+    both, v1 = run(binding.RAD_FLAG_DETERMINISTIC | binding.RAD_FLAG_OVERLAP_STEPS)
+    assert v0 == v1 == ("general" if shape == "regions" else shape)
+    for i in range(T):
+        assert np.array_equal(both[i], det_only[i]), f"step {i} differs"
+    if R > 1:
+        o = oracle_mod.RegionOracle(R, w.dirs, w.omega, w.dt, scale=1.0)
+        for t, st in steps:
+            o.accumulate_step(t, off, *st)
+        ref = o.spectrum().reshape(R * w.n_dir, w.n_omega)
+    else:
+        ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    for r in range(R):
+        sl = slice(r * w.n_dir, (r + 1) * w.n_dir)
+        if ref[sl].max() > 0:
+            P.assert_parity(both[-1][sl], ref[sl], what=f"overlap+deterministic {shape} region {r}")
+
+
+@pytest.mark.parametrize("regions", [False, True])
+def test_e2e_call_sequence_every_step_spectrum_matches_oracle(oracle_mod, regions):
+    """bench.py's `e2e` leg, call for call: RAD_FLAG_OVERLAP_STEPS handle, state in pinned HOST
+    memory through rad_accumulate_step(_regions)_host, every step's spectrum delivered to one of
+    two pinned host buffers with RAD_OUT_HOST_ASYNC, the host one step behind on an event.  EVERY
+    step's host spectrum (the running sum up to that step) is compared with the oracle's."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    R = 3 if regions else 1
+    n, T = 30000, 8
+    w = wl.Workload("e2e", n, T, 1e-17, wl.dirs_fibonacci(16), wl.omega_log(128), np.float32, wl.BASE_SEED + 71, "khi")
+    steps = list(w.steps())
+    host = [[torch.from_numpy(a).pin_memory() for a in st] for _, st in steps]
+    off = np.array([0, 9000, 9001, n], dtype=np.int64) if regions else None
+    o = (oracle_mod.RegionOracle(R, w.dirs, w.omega, w.dt, scale=1.0) if regions
+         else oracle_mod.Oracle(w.dirs, w.omega, w.dt, scale=1.0))
+    refs = []
+    for t, st in steps:
+        o.accumulate_step(t, *([off] if regions else []), *st)
+        refs.append(o.spectrum().reshape(R * w.n_dir, w.n_omega).copy())
+    got = [None] * T
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, flags=binding.RAD_FLAG_OVERLAP_STEPS,
+                          n_regions=R if regions else 0) as det:
+        pinned = [torch.empty(R * w.n_dir, w.n_omega, dtype=torch.float64).pin_memory() for _ in range(2)]
+        arrived = [torch.cuda.Event(), torch.cuda.Event()]
+        for i, (t, _) in enumerate(steps):
+            if regions:
+                det.accumulate_step_regions_host(t, off, host[i])
+            else:
+                det.accumulate_step_host(t, host[i])
+            b = i & 1
+            det.spectrum(out=pinned[b])          # RAD_OUT_HOST_ASYNC
+            arrived[b].record()
+            if i > 0:
+                arrived[b ^ 1].synchronize()
+                got[i - 1] = pinned[b ^ 1].numpy().copy()
+        arrived[(T - 1) & 1].synchronize()
+        got[T - 1] = pinned[(T - 1) & 1].numpy().copy()
+    for i in range(T):
+        for r in range(R):
+            sl = slice(r * w.n_dir, (r + 1) * w.n_dir)
+            P.assert_parity(got[i][sl], refs[i][sl], what=f"e2e sequence step {i} region {r}")

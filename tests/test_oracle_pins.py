@@ -533,3 +533,141 @@ def test_p13_nyquist_cutoff_is_doppler_shifted_by_direction(oracle_mod):
         os_.accumulate_step(t, *s1)
     cut_mov = OMEGA * DT * 1.9 >= np.pi * nu                     # direction -x
     assert np.allclose(ob.spectrum()[1, cut_mov], os_.spectrum()[1, cut_mov], rtol=1e-12)
+
+
+# ---------------------------------------------- P14 macro-particle form factor (reading FF1)
+# g_k(n, w) = sqrt(w_k + (w_k^2 - w_k) F^2(n, w)); the pins below fix everything the
+# mathematics fixes about it: both limits, the interpolation between them in closed form for two
+# shapes, the direction dependence, and the order "form factor first, window after".
+def _ff_run(oracle_mod, dirs, omega, dt, steps, form_factor, **kw):
+    o = oracle_mod.Oracle(dirs, omega, dt, scale=1.0, form_factor=form_factor, **kw)
+    for t, st in steps:
+        o.accumulate_step(t, *st)
+    return o
+
+
+def _ff_steps(rng, n, T, wmax=None):
+    steps = []
+    w = np.ones(n) if wmax is None else 10.0 ** rng.uniform(0, np.log10(wmax), n)
+    for t in range(T):
+        st = [rng.uniform(0, 2e-6, n) for _ in range(3)] + [rng.uniform(-0.4, 0.4, n) for _ in range(3)] \
+            + [rng.normal(0, 1e13, n) for _ in range(3)] + [w]
+        steps.append((t, st))
+    return steps
+
+
+@pytest.mark.parametrize("ff", [("gaussian", (3e-8, 1e-8, 2e-8)), ("cic", (5e-8, 5e-8, 5e-8)),
+                                ("incoherent", (0, 0, 0))])
+def test_p14_unit_weight_is_the_identity_bit_for_bit(oracle_mod, ff):
+    """w = 1: g = sqrt(1 + 0 * F^2) = 1 exactly, whatever the shape."""
+    steps = _ff_steps(np.random.default_rng(141), 40, 3)
+    a = _ff_run(oracle_mod, DIRS, OMEGA, DT, steps, ff)
+    b = _run(oracle_mod, DIRS, OMEGA, DT, steps)
+    assert np.array_equal(a.A, b.A)
+
+
+@pytest.mark.parametrize("ff", [("gaussian", (0, 0, 0)), ("cic", (0, 0, 0))])
+def test_p14_point_particle_limit_is_the_coherent_sum(oracle_mod, ff):
+    """Zero size: F = 1, g = sqrt(w^2) = w -> today's fully coherent sum (amplitude linear in w)."""
+    steps = _ff_steps(np.random.default_rng(142), 30, 2, wmax=1e4)
+    a = _ff_run(oracle_mod, DIRS, OMEGA, DT, steps, ff)
+    b = _run(oracle_mod, DIRS, OMEGA, DT, steps)
+    assert np.abs(a.A - b.A).max() <= 1e-13 * np.abs(b.A).max()
+
+
+def test_p14_incoherent_limit_intensity_is_linear_in_the_weight(oracle_mod):
+    """F = 0: one macro-particle of weight w radiates w times (not w^2 times) one particle; the
+    same at huge size for the Gaussian shape (F underflows to 0)."""
+    rng = np.random.default_rng(143)
+    (t, st), = _ff_steps(rng, 1, 1)
+    S1 = _run(oracle_mod, DIRS, OMEGA, DT, [(0, st)]).spectrum()
+    for wgt in (4.0, 1234.5):
+        stw = st[:9] + [np.array([wgt])]
+        Sw = _ff_run(oracle_mod, DIRS, OMEGA, DT, [(0, stw)], ("incoherent", (0, 0, 0))).spectrum()
+        assert np.allclose(Sw, wgt * S1, rtol=1e-13)
+        Sg = _ff_run(oracle_mod, DIRS, OMEGA, DT, [(0, stw)], ("gaussian", (1.0, 1.0, 1.0))).spectrum()
+        assert np.allclose(Sg, wgt * S1, rtol=1e-13)
+        Sc = _run(oracle_mod, DIRS, OMEGA, DT, [(0, stw)]).spectrum()      # coherent, for contrast
+        assert np.allclose(Sc, wgt ** 2 * S1, rtol=1e-13)
+
+
+def test_p14_gaussian_shape_times_dirichlet_closed_form(oracle_mod):
+    """Static macro-particle, constant betadot b, T steps (pin P2's set-up):
+    S = g^2 (|b|^2 - (n.b)^2) dt^2 sin^2(wT dt/2)/sin^2(w dt/2), g^2 = w + (w^2 - w) exp(-sum_c (w n_c s_c/c)^2)
+    with an ANISOTROPIC Gaussian, so the value depends on the direction through n_c s_c."""
+    T, wgt = 17, 250.0
+    b = np.array([2.0e12, -1.0e12, 3.0e12])
+    sig = np.array([4.0e-8, 1.0e-8, 2.5e-8])
+    st = _const_state([1e-7, 2e-7, -1e-7], [0, 0, 0], b, w=wgt)
+    o = _ff_run(oracle_mod, DIRS, OMEGA, DT, [(t, st) for t in range(T)], ("gaussian", sig))
+    S = o.spectrum()
+    saw_intermediate = False
+    for i, n in enumerate(UNIT):
+        for j, om in enumerate(OMEGA):
+            F2 = np.exp(-np.sum((om * n * sig / C) ** 2))
+            g2 = wgt + (wgt ** 2 - wgt) * F2
+            expect = g2 * (b @ b - (n @ b) ** 2) * DT ** 2 * _dirichlet(om * DT, T) ** 2
+            assert S[i, j] == pytest.approx(expect, rel=1e-11)
+            saw_intermediate |= 0.05 < F2 < 0.95
+    assert saw_intermediate           # the grid really samples the transition, not only the two limits
+
+
+def test_p14_cic_shape_first_zero_and_textbook_values(oracle_mod):
+    """CIC (triangular) shape of cell size D along x, observed along x: F = sinc^2(w D / 2c).
+    At w D / 2c = pi the shape factor vanishes (fully incoherent, g^2 = w); at pi/2 it is
+    (2/pi)^2, F^2 = (2/pi)^4; at 0+ it is 1."""
+    wgt, D = 100.0, 6.0e-8
+    n = np.array([[1.0, 0.0, 0.0]])
+    om = np.array([2e-6 * C / D, np.pi * C / D, 2 * np.pi * C / D])               # x = w D/2c = 1e-6, pi/2, pi
+    b = np.array([0.0, 1.0e12, 0.0])
+    st = _const_state([0, 0, 0], [0, 0, 0], b, w=wgt)
+    dt = 1e-19
+    S = _ff_run(oracle_mod, n, om, dt, [(0, st)], ("cic", (D, 7 * D, 9 * D))).spectrum()[0]   # y, z sizes: n_y = n_z = 0
+    base = (b @ b) * dt ** 2
+    assert S[0] == pytest.approx(wgt ** 2 * base, rel=1e-10)
+    assert S[1] == pytest.approx((wgt + (wgt ** 2 - wgt) * (2 / np.pi) ** 4) * base, rel=1e-12)
+    assert S[2] == pytest.approx(wgt * base, rel=1e-9)      # sin(pi) ~ 1e-16: F^2 ~ 1e-64
+
+
+def test_p14_bruteforce_numpy_with_window(oracle_mod):
+    """Independent numpy complex128 evaluation of the whole sum with g_k(n, w) and a window:
+    the form factor acts on the macro weight, the window multiplies afterwards."""
+    rng = np.random.default_rng(145)
+    n_p, T = 12, 3
+    steps = _ff_steps(rng, n_p, T, wmax=1e3)
+    size = np.array([2e-8, 3e-8, 1e-8])
+    win = ("triangle", (0.0, 0.0, 0.0), (2e-6, 0.0, 2e-6))
+    for kind in ("gaussian", "cic"):
+        o = _ff_run(oracle_mod, DIRS, OMEGA, DT, steps, (kind, size), window=win)
+        A = np.zeros((len(UNIT), len(OMEGA), 3), dtype=np.complex128)
+        for t, st in steps:
+            r, be, bd, w = np.stack(st[0:3], 1), np.stack(st[3:6], 1), np.stack(st[6:9], 1), st[9]
+            u = r / np.array([2e-6, 1.0, 2e-6])
+            Wn = (1 - np.abs(2 * u[:, 0] - 1)) * (1 - np.abs(2 * u[:, 2] - 1))
+            for i, n in enumerate(UNIT):
+                d = 1 - be @ n
+                vec = np.cross(n, np.cross(n - be, bd))
+                tau = t * DT - r @ n / C
+                for j, om in enumerate(OMEGA):
+                    if kind == "gaussian":
+                        F = np.exp(-0.5 * np.sum((om * n * size / C) ** 2))
+                    else:
+                        F = np.prod(np.sinc(om * n * size / (2 * C) / np.pi) ** 2)
+                    g = np.sqrt(w + (w * w - w) * F * F)
+                    A[i, j] += ((g * Wn * DT / d ** 2 * np.exp(1j * om * tau))[:, None] * vec).sum(0)
+        assert np.abs(o.amplitude() - A).max() <= 1e-12 * np.abs(A).max()
+
+
+def test_p14_regions_and_bad_arguments(oracle_mod):
+    rng = np.random.default_rng(146)
+    steps = _ff_steps(rng, 20, 2, wmax=50)
+    ff = ("gaussian", (2e-8, 2e-8, 2e-8))
+    off = np.array([0, 7, 7, 20])
+    ro = oracle_mod.RegionOracle(3, DIRS, OMEGA, DT, scale=1.0, form_factor=ff)
+    for t, st in steps:
+        ro.accumulate_step(t, off, *st)
+    whole = _ff_run(oracle_mod, DIRS, OMEGA, DT, steps, ff)
+    assert np.abs(ro.A.sum(axis=0) - whole.A).max() <= 1e-13 * np.abs(whole.A).max()
+    assert np.allclose(ro.spectrum_total(), whole.spectrum(), rtol=1e-12)
+    with pytest.raises(KeyError):
+        oracle_mod.Oracle(DIRS, OMEGA, DT, form_factor=("box", (1, 1, 1)))
