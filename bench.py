@@ -46,8 +46,8 @@ MUFU_PER_UPDATE = 2         # sin + cos: no recurrence exists on a non-uniform g
 FP32_PER_UPDATE_UNIFORM = 8  # 4 (complex rotation) + 4 (accumulate) FMA-pipe instructions
 L2_BYTES = 126 * 2 ** 20
 # short legs run after the headline: (config, timed steps, warm-up steps)
-LEGS = (("1", 20, 3), ("3a", 10, 3), ("3b", 10, 3), ("3c", 10, 3), ("3d", 10, 3), ("4", 3, 1), ("4b", 20, 3),
-        ("5r", 30, 5), ("0", 50, 5), ("1u", 20, 3))
+LEGS = (("1", 50, 3), ("3a", 10, 3), ("3b", 10, 3), ("3c", 10, 3), ("3d", 10, 3), ("4", 3, 1), ("4b", 200, 3),
+        ("5r", 200, 5), ("0", 500, 5), ("1u", 50, 3))
 
 
 def parse_args():
@@ -126,8 +126,8 @@ class ClockSampler(threading.Thread):
 def oracle_for(w, bins):
     from oracle import oracle
     if w.n_regions > 1:
-        return oracle.RegionOracle(w.n_regions, w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=bins)
-    return oracle.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=1.0, bins=bins)
+        return oracle.RegionOracle(w.n_regions, w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0, bins=bins)
+    return oracle.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0, bins=bins)   # scale 0 = SI default, as the detector
 
 
 def oracle_step(o, w, step_index, state, n):

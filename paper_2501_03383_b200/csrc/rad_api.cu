@@ -51,6 +51,7 @@ void free_all(Handle &h)
     cudaFree(h.dirs_d); cudaFree(h.basis_d); cudaFree(h.F_d); cudaFree(h.Ff_d); cudaFree(h.fl_d);
     cudaFree(h.acc_d); cudaFree(h.partial_d); cudaFree(h.stage_d[0]); cudaFree(h.stage_d[1]);
     cudaFree(h.out_d); cudaFree(h.chunks_d); cudaFree(h.reg_cstart_d); cudaFree(h.omega_d);
+
     if (h.chunks_h) cudaFreeHost(h.chunks_h);
     if (h.reg_cstart_h) cudaFreeHost(h.reg_cstart_h);
     if (h.reg_uploaded) cudaEventDestroy(h.reg_uploaded);
@@ -341,7 +342,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.n_chunks = n_chunks;
     int stream_grid = 0;
     if (h.stream_nb) {  // few bins: persistent particle-streaming kernel, one partial slot per block
-        const int tile = stream_tile_particles(h.state_f64);
+        const int tile = stream_tile_particles(h.stream_nb, h.state_f64);
         const long long n_tiles = (n + tile - 1) / tile;
         stream_grid = (int)std::min<long long>(n_tiles, (long long)stream_blocks_per_sm(h.stream_nb) * h.sm_count);
         for (int j = 0; j < 16; ++j) { p.sF[j] = h.sF[j]; p.sFf[j] = h.sFf[j]; p.sfl[j] = h.sfl[j]; }

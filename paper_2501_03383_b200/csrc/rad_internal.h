@@ -109,7 +109,7 @@ cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_
                               cudaStream_t s, int *n_launches, const char **variant);
 cudaError_t launch_accumulate_stream(const Handle &h, const AccumParams &p, bool state_f64, int grid,
                                      cudaStream_t s);
-int stream_tile_particles(bool state_f64);
+int stream_tile_particles(int nb, bool state_f64);
 int stream_blocks_per_sm(int nb);
 int stream_shape(int D, int W, int *nd);
 cudaError_t launch_spectrum(const Handle &h, double *out_dev, cudaStream_t s);

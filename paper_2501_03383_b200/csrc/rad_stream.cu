@@ -3,15 +3,31 @@
 // of state per particle feed only a handful of updates and HBM bandwidth binds
 // (BASELINE.json configs[4] "streamed from HBM each step").
 //
-// Mapping: a thread owns particles (4 per 1024-particle tile) and keeps ALL bins' fp32 partial
-// amplitudes in registers; blocks are persistent and walk the tiles with stride gridDim.x.
-// Staging (the "per-step particle-staging kernel ... staged via TMA", BASELINE.json north_star):
-// one elected thread issues ten 1-D bulk async copies (cp.async.bulk, SASS UBLKCP) per tile
-// into a two-stage shared-memory ring, completion signalled on an mbarrier (expect_tx), so
-// the copy of tile i+1 runs under the arithmetic of tile i.  Unaligned arrays or a ragged
-// last tile fall back to coalesced ld.global.nc.  At the end the partials go through
-// warp-shuffle reductions, a shared-memory cross-warp sum and one fp64 atomic per value
-// per block (or the deterministic workspace).
+// Mapping: a lane owns particles and keeps ALL bins' fp32 partial amplitudes in registers.
+// Every WARP runs its own copy pipeline -- no block-level barrier anywhere in the loop (round 1's
+// per-tile __syncthreads cost 0.75 stall cycles per issued instruction at 16 warps per SM):
+//   * one persistent block of 20 warps per SM; the warps work through "warp tiles" of 32 x PPT
+//     particles (PPT = 16 B / sizeof(state element): 4 fp32 or 2 fp64 particles per lane) drawn
+//     from the block's tile counter in shared memory (work stealing within the SM; static
+//     round-robin shares in deterministic mode);
+//   * staging (the "per-step particle-staging kernel ... staged via TMA" of BASELINE.json
+//     north_star): lane 0 issues ten 512-byte 1-D bulk async copies (cp.async.bulk, SASS UBLKCP)
+//     per warp tile into the warp's own two-stage shared-memory ring (2 x 5 KB), completion
+//     signalled on the warp's own mbarrier (expect_tx);
+//   * a lane reads its PPT consecutive particles of each array with ONE 16-byte shared-memory
+//     load (10 LDS.128 per warp tile instead of 40 LDS.32); at the top of a turn -- after a
+//     __syncwarp -- lane 0 refills the stage read in the previous turn with the next tile, which
+//     arrives under this turn's arithmetic (20 warps x 5 KB in flight per SM, ~3x the 35 KB that
+//     latency x bandwidth asks for).
+// The ragged tail (N mod 32*PPT particles) and arrays that are not 16-byte aligned go through
+// coalesced ld.global.nc, one particle per lane.  At the end the partials go through warp-shuffle
+// reductions, a shared-memory cross-warp sum and one fp64 atomic per value per block (or the
+// deterministic workspace).
+//
+// Per update the four accumulate FMAs are two packed fma.rn.f32x2 (A1 and A2 each times the
+// (cos, sin) pair): the kernel is co-limited by instruction issue (~200 instructions per particle
+// against 40 B of HBM traffic), so halving the accumulate instructions matters more than the
+// lower per-instruction rate of the packed form.
 #include "rad_device.cuh"
 #include "rad_internal.h"
 
@@ -21,12 +37,14 @@ namespace {
 
 using namespace dev;
 
-// Shape of the ring, frozen from the round-1 sweeps.
-constexpr int kSThreads = 256;
+// Shape of the pipeline: ONE block per SM, so that the warps of an SM can
+// share a tile counter in shared memory.
 constexpr int kSStages = 2;
-constexpr int kSUnroll = 4;
-constexpr int kSMinBlocks = 2;
-constexpr int kSTileBytes = 4096;  // per array per stage -> 1024 fp32 / 512 fp64 particles
+constexpr int kSArrayBytes = 512;           // per array per stage per warp: 32 lanes x 16 B
+constexpr int kSStageBytes = 10 * kSArrayBytes;
+// warps per block, each with its own 10 KB ring: 20 (200 KB of rings, <= 102 registers) for <= 8
+// bins per thread, 12 for 16 bins per thread (168 registers)
+__host__ __device__ constexpr int stream_warps(int nb) { return nb <= 8 ? 20 : 12; }
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
@@ -64,6 +82,31 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
         : "memory");
 }
 
+// one lane of the (converged) warp; with warp-uniform operands the copy instructions that follow
+// are issued from the uniform datapath without a per-lane address loop
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile("{\n.reg .pred P;\nelect.sync _|P, 0xffffffff;\nselp.u32 %0, 1, 0, P;\n}" : "=r"(pred));
+    return pred != 0;
+}
+
+// two fp32 in one 64-bit register pair, for fma.rn.f32x2
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(unsigned long long v, float &lo, float &hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ void fma2(unsigned long long &acc, unsigned long long a, unsigned long long b)
+{
+    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
+}
+
 template <typename ST, bool WIN>
 __device__ __forceinline__ Particle make_particle(ST rx, ST ry, ST rz, ST bx, ST by, ST bz, ST dx,
                                                   ST dy, ST dz, ST w, const AccumParams &P)
@@ -78,113 +121,157 @@ __device__ __forceinline__ Particle make_particle(ST rx, ST ry, ST rz, ST bx, ST
     return p;
 }
 
+// 16 bytes of state = PPT consecutive particles of one array
+template <typename ST> struct Vec16;
+template <> struct Vec16<float> {
+    float4 v;
+    __device__ __forceinline__ float get(int i) const { return i == 0 ? v.x : i == 1 ? v.y : i == 2 ? v.z : v.w; }
+};
+template <> struct Vec16<double> {
+    double2 v;
+    __device__ __forceinline__ double get(int i) const { return i == 0 ? v.x : v.y; }
+};
+
+// a1 + a2 for one particle: all bins of all (<= 2) directions
+template <int NB, int ND>
+__device__ __forceinline__ void accumulate_particle(const AccumParams &P, const Particle &p,
+                                                    unsigned long long (&acc01)[NB], unsigned long long (&acc23)[NB])
+{
+    constexpr int WB = NB / ND;
+#pragma unroll
+    for (int d = 0; d < ND; ++d) {
+        float4 r4;
+        float sf;
+        stage_record(p, P.sdir[d], P.ts32, r4, sf);  // a1 (direction record: constant bank)
+        const unsigned long long a1 = pack2(r4.z, r4.z), a2 = pack2(r4.w, r4.w);
+#pragma unroll
+        for (int j = 0; j < WB; ++j) {  // a2
+            float sn, cs;
+            phase_sincos(P.sF[j], P.sFf[j], P.sfl[j], __float_as_uint(r4.x), r4.y, sf, sn, cs);
+            const unsigned long long z = pack2(cs, sn);
+            fma2(acc01[d * WB + j], a1, z);  // (Re, Im) A1 += a1 (cos, sin)
+            fma2(acc23[d * WB + j], a2, z);  // (Re, Im) A2 += a2 (cos, sin)
+        }
+    }
+}
+
 // NB bins per thread = ND directions x WB frequencies (compile time; W is padded to WB with
 // zero-frequency bins that are discarded).  Per-bin frequency constants come straight from the
 // kernel-parameter constant bank (P.sF/sFf/sfl), not from registers.
 // WIN: spatial window compiled in (kept out of the default instantiation: the streaming kernel
 // is latency bound and loses 3 % to the extra per-particle code even when the window is off)
 template <typename ST, int NB, int ND, bool WIN>
-__global__ void __launch_bounds__(kSThreads, NB <= 8 ? kSMinBlocks : 1) rad_accum_stream(const AccumParams P, const int use_bulk)
+__global__ void __launch_bounds__(32 * stream_warps(NB), 1) rad_accum_stream(const AccumParams P, const int use_bulk)
 {
-    constexpr int TILE = kSTileBytes / (int)sizeof(ST);  // particles per tile
-    constexpr int PPT = TILE / kSThreads;                 // particles per thread per tile
+    constexpr int kSWarps = stream_warps(NB);
+    constexpr int PPT = 16 / (int)sizeof(ST);  // particles per lane per warp tile
+    constexpr int WTILE = 32 * PPT;            // particles per warp tile
     constexpr int WB = NB / ND;
-    static_assert(PPT >= 1 && WB * ND == NB, "tile/bin shape");
-    extern __shared__ __align__(128) unsigned char s_raw[];
-    __shared__ __align__(8) uint64_t s_full[kSStages];
-    __shared__ float s_red[kSThreads / 32][NB * 4];
+    static_assert(WB * ND == NB && kSStages == 2, "bin shape / two-stage ring");
+    extern __shared__ __align__(128) unsigned char s_raw[];  // [kSWarps][kSStages][10][512 B]
+    __shared__ __align__(8) uint64_t s_full[kSWarps][kSStages];
+    __shared__ float s_red[kSWarps][NB * 4];
+    __shared__ int s_next;  // dynamic schedule: next tile of this block
 
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);  // warp-uniform to the compiler: uniform-datapath addresses
     pdl_trigger();
-    float acc[NB][4];
+    unsigned long long acc01[NB], acc23[NB];
 #pragma unroll
-    for (int b = 0; b < NB; ++b) acc[b][0] = acc[b][1] = acc[b][2] = acc[b][3] = 0.0f;
+    for (int b = 0; b < NB; ++b) acc01[b] = acc23[b] = 0ull;
 
     const long long N = P.n_particles;
-    const long long n_tiles = (N + TILE - 1) / TILE;
-    if (tid == 0) {
-        for (int s = 0; s < kSStages; ++s) mbar_init(&s_full[s], 1);
+    const long long n_full = use_bulk ? N / WTILE : 0;  // warp tiles that go through the bulk-copy ring
+    const long long gw = (long long)blockIdx.x * kSWarps + warp, GW = (long long)gridDim.x * kSWarps;
+    unsigned char *ring = s_raw + (size_t)warp * kSStages * kSStageBytes;
+    uint64_t *full = s_full[warp];
+
+    if (tid == 0) s_next = 0;
+    if (elect_one()) {
+#pragma unroll
+        for (int s = 0; s < kSStages; ++s) mbar_init(&full[s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    __syncthreads();
+    __syncthreads();  // the one block barrier before the loop (tile counter, barriers)
 
-    auto tile_bulk = [&](long long t) -> bool {  // full tile (16-B multiple) and aligned arrays
-        return use_bulk && (t + 1) * TILE <= N;
-    };
-    auto issue = [&](long long t, int stage) {  // thread 0 only
-        mbar_expect_tx(&s_full[stage], 10u * kSTileBytes);
+    auto issue = [&](long long t, int stage) {  // one elected lane: ten 512-byte copies, one barrier
+        mbar_expect_tx(&full[stage], (uint32_t)kSStageBytes);
 #pragma unroll
         for (int a = 0; a < 10; ++a)
-            bulk_g2s(s_raw + ((size_t)stage * 10 + a) * kSTileBytes,
-                     reinterpret_cast<const ST *>(P.st[a]) + t * TILE, kSTileBytes, &s_full[stage]);
+            bulk_g2s(ring + (size_t)stage * kSStageBytes + a * kSArrayBytes,
+                     reinterpret_cast<const ST *>(P.st[a]) + t * WTILE, kSArrayBytes, &full[stage]);
     };
 
-    // prologue: fill kSStages-1 stages ahead
-    const long long t0 = blockIdx.x, dtile = gridDim.x;
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < kSStages - 1; ++s) {
-            const long long tp = t0 + s * dtile;
-            if (tp < n_tiles && tile_bulk(tp)) issue(tp, s);
-        }
+    // Which tiles a warp works on.  The tiles are dealt to the blocks round robin (block b owns
+    // tiles b, b + gridDim.x, ...); within the block (= within the SM) the warps DRAW the block's
+    // tiles from a shared-memory counter, one draw ahead of the copy it feeds.  The warp schedulers
+    // are not fair (measured: with equal static shares the favoured warps of an SM finish early and
+    // the rest crawl on alone -- 14.5 of 20 resident warps active on average); with a counter the
+    // fast warps simply take more tiles and all end together.  (A single global counter serialises
+    // in L2: 131 072 draws took 0.3 ms.)  Deterministic mode (P.partial != NULL) keeps static
+    // round-robin shares, whose partial sums do not depend on timing.
+    const bool dynamic = P.partial == nullptr;
+    const long long n_mine = n_full > blockIdx.x ? (n_full - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;  // tiles of this block
+    int n_drawn = 0;  // static schedule: tiles this warp has drawn so far
+    constexpr long long kNoTile = 0x7fffffffffffffffLL;
+    auto draw = [&]() -> long long {  // lane 0 only -> block-local tile index
+        if (dynamic) return (long long)atomicAdd(&s_next, 1);
+        return warp + (long long)(n_drawn++) * kSWarps;
+    };
+    auto tile_of = [&](long long k) { return (long long)blockIdx.x + k * (long long)gridDim.x; };
+    long long t_a = kNoTile, t_b = kNoTile;
+    if (lane == 0) {
+        t_a = draw();
+        if (t_a < n_mine) t_b = draw();
     }
-    uint32_t phase_bits = 0;  // bit s: parity the next wait on stage s expects
+    long long cur = __shfl_sync(0xffffffffu, t_a, 0);
+    if (cur < n_mine && elect_one()) issue(tile_of(cur), 0);  // prologue: the first tile
+    uint32_t parity = 0;  // bit s: parity the next wait on stage s expects
     int stage = 0;
-    for (long long t = t0; t < n_tiles; t += dtile) {
-        // stage (stage-1) mod kSStages was read in the previous iteration; its barrier is behind us
-        const long long tn = t + (kSStages - 1) * dtile;
-        const int sn = stage == 0 ? kSStages - 1 : stage - 1;
-        if (tid == 0 && tn < n_tiles && tile_bulk(tn)) issue(tn, sn);
-        const bool bulk = tile_bulk(t);
-        if (bulk) {
-            mbar_wait(&s_full[stage], (phase_bits >> stage) & 1u);
-            phase_bits ^= 1u << stage;
-        }
-        const ST *sm = reinterpret_cast<const ST *>(s_raw + (size_t)stage * 10 * kSTileBytes);
-#pragma unroll kSUnroll
+    while (cur < n_mine) {
+        // the other stage was read in the previous turn (its values are consumed): refill it with
+        // the next tile, which then arrives under this turn's arithmetic
+        __syncwarp();
+        const int other = stage ^ 1;
+        const long long nxt = __shfl_sync(0xffffffffu, t_b, 0);  // drawn one turn ago
+        if (lane == 0) t_b = nxt < n_mine ? draw() : kNoTile;     // for the turn after the next
+        if (nxt < n_mine && elect_one()) issue(tile_of(nxt), other);
+        mbar_wait(&full[stage], (parity >> stage) & 1u);
+        parity ^= 1u << stage;
+        const unsigned char *src = ring + (size_t)stage * kSStageBytes + lane * 16;
+        Vec16<ST> v[10];
+#pragma unroll
+        for (int a = 0; a < 10; ++a) v[a].v = *reinterpret_cast<const decltype(v[a].v) *>(src + a * kSArrayBytes);
+#pragma unroll
         for (int pp = 0; pp < PPT; ++pp) {
-            const int kl = tid + pp * kSThreads;
-            const long long k = t * TILE + kl;
-            Particle p;
-            if (bulk) {
-                p = make_particle<ST, WIN>(sm[0 * TILE + kl], sm[1 * TILE + kl], sm[2 * TILE + kl],
-                                      sm[3 * TILE + kl], sm[4 * TILE + kl], sm[5 * TILE + kl],
-                                      sm[6 * TILE + kl], sm[7 * TILE + kl], sm[8 * TILE + kl],
-                                      sm[9 * TILE + kl], P);
-            } else {
-                p = load_particle<ST, WIN>(P, k, k < N);
-            }
-#pragma unroll
-            for (int d = 0; d < ND; ++d) {
-                float4 r4;
-                float sf;
-                stage_record(p, P.sdir[d], P.ts32, r4, sf);  // a1 (direction record: constant bank)
-#pragma unroll
-                for (int j = 0; j < WB; ++j) {  // a2
-                    const int b = d * WB + j;
-                    float sn2, cs2;
-                    phase_sincos(P.sF[j], P.sFf[j], P.sfl[j], __float_as_uint(r4.x), r4.y, sf, sn2, cs2);
-                    acc[b][0] = fmaf(r4.z, cs2, acc[b][0]);
-                    acc[b][1] = fmaf(r4.z, sn2, acc[b][1]);
-                    acc[b][2] = fmaf(r4.w, cs2, acc[b][2]);
-                    acc[b][3] = fmaf(r4.w, sn2, acc[b][3]);
-                }
-            }
+            const Particle p = make_particle<ST, WIN>(v[0].get(pp), v[1].get(pp), v[2].get(pp), v[3].get(pp),
+                                                      v[4].get(pp), v[5].get(pp), v[6].get(pp), v[7].get(pp),
+                                                      v[8].get(pp), v[9].get(pp), P);
+            accumulate_particle<NB, ND>(P, p, acc01, acc23);
         }
-        __syncthreads();  // this stage may be refilled by the next iteration's issue
-        stage = stage + 1 == kSStages ? 0 : stage + 1;
+        cur = nxt;
+        stage = other;
+    }
+    // ragged tail / unaligned arrays: plain coalesced loads, one particle per lane
+    for (long long k = n_full * WTILE + gw * 32 + lane; k < N; k += GW * 32) {
+        const Particle p = load_particle<ST, WIN>(P, k, true);
+        accumulate_particle<NB, ND>(P, p, acc01, acc23);
     }
 
     // a3: warp-shuffle reduction, cross-warp sum in shared memory, one fp64 add per value
 #pragma unroll
-    for (int b = 0; b < NB; ++b)
+    for (int b = 0; b < NB; ++b) {
+        float v4[4];
+        unpack2(acc01[b], v4[0], v4[1]);
+        unpack2(acc23[b], v4[2], v4[3]);
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
-            float v = acc[b][c];
+            float v = v4[c];
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
             if (lane == 0) s_red[warp][b * 4 + c] = v;
         }
+    }
     __syncthreads();
     pdl_wait();  // the accumulator belongs to earlier work until here
     if (tid < NB * 4) {
@@ -193,7 +280,7 @@ __global__ void __launch_bounds__(kSThreads, NB <= 8 ? kSMinBlocks : 1) rad_accu
         if (d < P.n_dir && j < P.n_omega) {
             double v = 0.0;
 #pragma unroll
-            for (int wp = 0; wp < kSThreads / 32; ++wp) v += (double)s_red[wp][tid];
+            for (int wp = 0; wp < kSWarps; ++wp) v += (double)s_red[wp][tid];
             const size_t off = ((size_t)d * P.w_pad + j) * 4 + c;
             if (P.partial)
                 P.partial[(size_t)blockIdx.x * P.n_dir * P.w_pad * 4 + off] = v;
@@ -206,15 +293,15 @@ __global__ void __launch_bounds__(kSThreads, NB <= 8 ? kSMinBlocks : 1) rad_accu
 template <typename ST, int NB, int ND, bool WIN>
 cudaError_t launch_stream_w(const AccumParams &p, int grid, cudaStream_t s, bool overlap)
 {
-    const size_t smem = (size_t)kSStages * 10 * kSTileBytes;
+    const size_t smem = (size_t)stream_warps(NB) * kSStages * kSStageBytes;
     // per device and per template instance; the call is a cheap host-side set, so no caching
     cudaError_t e = cudaFuncSetAttribute(rad_accum_stream<ST, NB, ND, WIN>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    int use_bulk = 1;
+    int use_bulk = 1;  // bulk copies need 16-byte aligned sources
     for (int a = 0; a < 10; ++a)
         if (reinterpret_cast<uintptr_t>(p.st[a]) & 15) use_bulk = 0;
-    return launch_kernel(rad_accum_stream<ST, NB, ND, WIN>, dim3(grid), dim3(kSThreads), smem, s, overlap, p, use_bulk);
+    return launch_kernel(rad_accum_stream<ST, NB, ND, WIN>, dim3(grid), dim3(32 * stream_warps(NB)), smem, s, overlap, p, use_bulk);
 }
 
 template <typename ST, int NB, int ND>
@@ -233,8 +320,9 @@ cudaError_t dispatch_stream(const Handle &h, const AccumParams &p, int grid, cud
 
 }  // namespace
 
-int stream_tile_particles(bool state_f64) { return kSTileBytes / (state_f64 ? 8 : 4); }
-int stream_blocks_per_sm(int nb) { return nb <= 8 ? kSMinBlocks : 1; }
+// particles per block per turn of the persistent loop (host side: grid sizing)
+int stream_tile_particles(int nb, bool state_f64) { return stream_warps(nb) * 32 * (state_f64 ? 2 : 4); }
+int stream_blocks_per_sm(int) { return 1; }
 
 // Shapes served: ND in {1, 2} directions x WB = NB/ND frequencies, NB in {8, 16}.
 // Returns NB (and *nd), or 0 if this detector shape is not a streaming shape.

@@ -5,7 +5,10 @@
 // Every kind runs 8 independent dependency chains per thread (dependent-free at the warp level
 // once >= 4 warps per scheduler are resident), ITERS x 8 operations per thread, and reports
 //   per_clk_sm = thread-level results per SM clock per SM, from clock64() inside the kernel
-//                (independent of the clock frequency), averaged over the blocks, and
+//                (independent of the clock frequency): per SM, the results of all warps that ran
+//                there / (latest end - earliest start over those warps), averaged over the SMs
+//                (a single warp's own duration would overstate the rate: the warp scheduler is
+//                not fair, early warps finish while late ones are still running), and
 //   gops       = 1e-9 x thread-level results per second of the whole GPU, from CUDA events.
 // The roofline denominators derived from them:
 //   general grid   R_gen = sincos pairs/clk/SM (kind SINCOS) x SMs x clock      [nominal 8]
@@ -18,6 +21,7 @@ namespace {
 constexpr int kIters = 2048;
 constexpr int kChains = 8;
 constexpr int kThreads = 256;
+constexpr int kMaxSmid = 1024;  // %smid values are not guaranteed contiguous: generous table
 
 enum Kind {
     K_FFMA = 0,      // fma.rn.f32, three register operands
@@ -36,6 +40,7 @@ enum Kind {
 template <int KIND>
 __global__ void __launch_bounds__(kThreads) pipe_kernel(float *out, float a, float b, long long *clk)
 {
+    // clk: [3][kMaxSmid] = earliest start, latest end, number of warps, per SM (%smid)
     float x[kChains];
     unsigned long long y[kChains];
     double z[kChains];
@@ -87,7 +92,15 @@ __global__ void __launch_bounds__(kThreads) pipe_kernel(float *out, float a, flo
 #pragma unroll
     for (int i = 0; i < kChains; ++i) s += x[i] + c[i] + (float)(y[i] >> 32) + (float)z[i] + (float)w[i];
     out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = s;
-    if (threadIdx.x == 0) clk[blockIdx.x] = t1 - t0;
+    if ((threadIdx.x & 31) == 0) {
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        if (smid < kMaxSmid) {
+            atomicMin(clk + smid, t0);
+            atomicMax(clk + kMaxSmid + smid, t1);
+            atomicAdd(reinterpret_cast<unsigned long long *>(clk + 2 * kMaxSmid + smid), 1ull);
+        }
+    }
 }
 
 template <int KIND>
@@ -97,25 +110,38 @@ int run_kind(int n_sm, int blocks_per_sm, int reps, double *per_clk_sm, double *
     float *out = nullptr;
     long long *clk = nullptr;
     if (cudaMalloc(&out, (size_t)grid * kThreads * sizeof(float)) != cudaSuccess) return 1;
-    if (cudaMalloc(&clk, (size_t)grid * sizeof(long long)) != cudaSuccess) { cudaFree(out); return 1; }
+    const size_t clk_bytes = (size_t)3 * kMaxSmid * sizeof(long long);
+    if (cudaMalloc(&clk, clk_bytes) != cudaSuccess) { cudaFree(out); return 1; }
+    long long *h = new long long[3 * kMaxSmid];
+    auto reset_clk = [&]() {
+        for (int i = 0; i < kMaxSmid; ++i) { h[i] = 0x7fffffffffffffffLL; h[kMaxSmid + i] = 0; h[2 * kMaxSmid + i] = 0; }
+        cudaMemcpy(clk, h, clk_bytes, cudaMemcpyHostToDevice);
+    };
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
+    reset_clk();
     for (int r = 0; r < 2; ++r) pipe_kernel<KIND><<<grid, kThreads>>>(out, 1.0001f, 0.5f, clk);  // warm-up
+    cudaDeviceSynchronize();
+    reset_clk();
+    pipe_kernel<KIND><<<grid, kThreads>>>(out, 1.0001f, 0.5f, clk);  // the launch the per-SM cycle windows are read from
+    int rc = cudaDeviceSynchronize() == cudaSuccess ? 0 : 2;
+    if (cudaMemcpy(h, clk, clk_bytes, cudaMemcpyDeviceToHost) != cudaSuccess) rc = 2;
     cudaEventRecord(e0);
     for (int r = 0; r < reps; ++r) pipe_kernel<KIND><<<grid, kThreads>>>(out, 1.0001f, 0.5f, clk);
     cudaEventRecord(e1);
-    int rc = cudaDeviceSynchronize() == cudaSuccess ? 0 : 2;
+    if (cudaDeviceSynchronize() != cudaSuccess) rc = 2;
     float ms = 0.0f;
     cudaEventElapsedTime(&ms, e0, e1);
-    long long *h = new long long[grid];
-    if (cudaMemcpy(h, clk, (size_t)grid * sizeof(long long), cudaMemcpyDeviceToHost) != cudaSuccess) rc = 2;
-    double cyc = 0.0;
-    for (int i = 0; i < grid; ++i) cyc += (double)h[i];
-    cyc /= grid;
+    double rate = 0.0;
+    int used = 0;
+    for (int i = 0; i < kMaxSmid; ++i) {
+        const double warps = (double)h[2 * kMaxSmid + i], cyc = (double)(h[kMaxSmid + i] - h[i]);
+        if (warps > 0.0 && cyc > 0.0) { rate += warps * 32.0 * kIters * kChains / cyc; ++used; }
+    }
     delete[] h;
     const double ops_per_sm = (double)kIters * kChains * kThreads * blocks_per_sm;  // thread-level results
-    *per_clk_sm = cyc > 0.0 ? ops_per_sm / cyc : 0.0;
+    *per_clk_sm = used ? rate / used : 0.0;
     *gops = ms > 0.0f ? ops_per_sm * n_sm * reps / (ms * 1e-3) / 1e9 : 0.0;
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);

@@ -742,8 +742,11 @@ def test_overlap_steps_flag_keeps_every_intermediate_spectrum(oracle_mod, cfg, n
         return [o.cpu().numpy() for o in outs]
 
     plain, over = run(0), run(binding.RAD_FLAG_OVERLAP_STEPS)
+    # GPU vs GPU: a step missing from (or leaking into) a spectrum changes it by O(1/T); rounding
+    # differences between two runs are ~1e-7 (fp32 partial sums whose grouping depends on timing:
+    # fp64 atomics everywhere, work-stealing tile shares in the streaming kernel)
     for i in range(T):
-        assert np.allclose(over[i], plain[i], rtol=1e-9, atol=1e-12 * plain[-1].max()), f"step {i}"
+        assert np.allclose(over[i], plain[i], rtol=2e-5, atol=1e-9 * plain[-1].max()), f"step {i}"
     if R > 1:
         o = oracle_mod.RegionOracle(R, w.dirs, w.omega, w.dt, scale=1.0)
         for t, st in steps:
