@@ -9,7 +9,7 @@ rad_spectrum (a4).  Metric (BASELINE.json): particle*direction*frequency updates
 in G/s, whole job.  Headline workload = BASELINE.json configs[2] ("production-like": 1 048 576
 electrons x 256 directions x 1024 log-spaced frequencies, fp32 state), the largest single-GPU
 configuration.  The same invocation also runs short legs of every other configuration (1, 3a-d,
-4, 4b, 5r, 0, 1u) and reports them under "configs", runs the pipe microbenchmarks
+4, 4b, 5r, 0, 1u, 1f) and reports them under "configs", runs the pipe microbenchmarks
 (librad_ubench.so) and reports the measured ALU peaks under "alu_peaks", and compares the
 spectrum left by the timed region with the fp64 oracle on sampled bins ("parity").
 
@@ -47,7 +47,7 @@ FP32_PER_UPDATE_UNIFORM = 8  # 4 (complex rotation) + 4 (accumulate) FMA-pipe in
 L2_BYTES = 126 * 2 ** 20
 # short legs run after the headline: (config, timed steps, warm-up steps)
 LEGS = (("1", 50, 3), ("3a", 10, 3), ("3b", 10, 3), ("3c", 10, 3), ("3d", 10, 3), ("4", 3, 1), ("4b", 200, 3),
-        ("5r", 200, 5), ("0", 500, 5), ("1u", 50, 3))
+        ("5r", 200, 5), ("0", 500, 5), ("1u", 50, 3), ("1f", 50, 3))
 
 
 def parse_args():
@@ -126,8 +126,10 @@ class ClockSampler(threading.Thread):
 def oracle_for(w, bins):
     from oracle import oracle
     if w.n_regions > 1:
-        return oracle.RegionOracle(w.n_regions, w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0, bins=bins)
-    return oracle.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0, bins=bins)   # scale 0 = SI default, as the detector
+        return oracle.RegionOracle(w.n_regions, w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0, bins=bins,
+                                   form_factor=w.form_factor)
+    return oracle.Oracle(w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0, bins=bins,   # scale 0 = SI default, as the detector
+                         form_factor=w.form_factor)
 
 
 def oracle_step(o, w, step_index, state, n):
@@ -292,7 +294,7 @@ def measure(cfg, K, W, args, ctx, headline):
     # reach the kernels through an event of the library's copy stream.
     flags = 0 if args.no_overlap else binding.RAD_FLAG_OVERLAP_STEPS
     det = binding.Detector(w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0, state_dtype=w.state_dtype,
-                           device=local, n_regions=R if R > 1 else 0, flags=flags)
+                           device=local, n_regions=R if R > 1 else 0, flags=flags, form_factor=w.form_factor)
     spec_dev = torch.empty(R * w.n_dir, w.n_omega, dtype=torch.float64, device="cuda")
     reducer = multi.AmplitudeAllReduce(det) if world > 1 else None
 
@@ -374,6 +376,10 @@ def measure(cfg, K, W, args, ctx, headline):
         if variant == "uniform":  # rotation recurrence: 4 FP32 rotate + 4 FMA accumulate per update
             per_clk_sm, pipe = FP32_LANES_PER_SM / FP32_PER_UPDATE_UNIFORM, "FP32 (8 FMA-pipe instr per update)"
             measured = peaks_alu["ffma_per_clk_sm"] / FP32_PER_UPDATE_UNIFORM if peaks_alu else None
+        elif variant.endswith("+formfactor") and not variant.startswith("uniform"):
+            # general grid with the macro-particle form factor: sin + cos + sqrt per update
+            per_clk_sm, pipe = MUFU_LANES_PER_SM / 3.0, "MUFU (sin+cos+sqrt per update)"
+            measured = peaks_alu["mufu_per_clk_sm"] / 3.0 if peaks_alu else None
         else:                     # general grid: sin + cos per update on the 16-lane MUFU
             per_clk_sm, pipe = MUFU_LANES_PER_SM / MUFU_PER_UPDATE, "MUFU (sin+cos per update)"
             measured = peaks_alu["sincos_pairs_per_clk_sm"] if peaks_alu else None

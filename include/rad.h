@@ -110,7 +110,30 @@ typedef struct {
     double window_origin[3]; /* m: lower corner o of the window box                        */
     double window_extent[3]; /* m: edge lengths L; L_c <= 0: axis c is not windowed        */
     double nyquist_factor; /* nu >= 0; 0: off.  Nyquist limiter (below)                      */
+    int32_t form_factor_type;     /* RAD_FF_*: macro-particle form factor (below); 0: none   */
+    int32_t reserved0;            /* must be 0                                               */
+    double form_factor_size[3];   /* m: s_x, s_y, s_z of the macro-particle shape, >= 0      */
 } rad_config;
+
+/* Macro-particle form factor (the plugin "correctly quantif[ies] coherent and
+ * incoherent radiation [39]"; ref [39], line 338, "a general form factor formalism for
+ * macro-particles"; the formula is not printed in the paper -- reading FF1 of DESIGN.md).  A
+ * macro-particle of weight w stands for w real particles distributed with a shape whose Fourier
+ * transform at the emitted wave vector k = w_j n / c is F(n, w_j), 0 <= F <= 1; their fields add
+ * coherently for the fraction F^2 and incoherently for the rest (intensity w^2 F^2 + w (1 - F^2)),
+ * so with form_factor_type != RAD_FF_NONE the weight of a term in the amplitude sum is
+ *     g_k(n, w_j) = sqrt( w_k + (w_k^2 - w_k) F^2(n, w_j) )         instead of w_k
+ * (the spatial window, if any, still multiplies it; weights must be >= 0).
+ *     RAD_FF_GAUSSIAN    F = exp( -1/2 sum_c (w_j n_c s_c / c)^2 )           s_c: standard deviations
+ *     RAD_FF_CIC         F = prod_c sinc^2( w_j n_c s_c / (2c) )             s_c: cell sizes (cloud in cell)
+ *     RAD_FF_INCOHERENT  F = 0: g = sqrt(w)
+ * w = 1 is the identity for every shape; zero sizes give F = 1, g = w (the detector as
+ * BASELINE.json states it).  F^2 is tabulated per (direction, frequency) at rad_create in fp64;
+ * the square root is taken per update (a third special-function operation per update). */
+#define RAD_FF_NONE 0
+#define RAD_FF_GAUSSIAN 1
+#define RAD_FF_CIC 2
+#define RAD_FF_INCOHERENT 3
 
 /* Nyquist limiter (not in the paper; reading N1 of DESIGN.md): with nyquist_factor = nu > 0 the
  * term of particle k at a step is left out of bin (n, w_j) when

@@ -22,6 +22,9 @@ RAD_FLAG_DETERMINISTIC, RAD_FLAG_FORCE_GENERAL, RAD_FLAG_OVERLAP_STEPS = 1, 2, 4
 RAD_OUT_HOST, RAD_OUT_DEVICE, RAD_OUT_HOST_ASYNC = 0, 1, 2
 RAD_WINDOW_NONE, RAD_WINDOW_TRIANGLE, RAD_WINDOW_HAMMING = 0, 1, 2
 WINDOW_TYPES = {"none": RAD_WINDOW_NONE, "triangle": RAD_WINDOW_TRIANGLE, "hamming": RAD_WINDOW_HAMMING}
+RAD_FF_NONE, RAD_FF_GAUSSIAN, RAD_FF_CIC, RAD_FF_INCOHERENT = 0, 1, 2, 3
+FORM_FACTOR_TYPES = {"none": RAD_FF_NONE, "gaussian": RAD_FF_GAUSSIAN, "cic": RAD_FF_CIC,
+                     "incoherent": RAD_FF_INCOHERENT}
 
 ABI_SYMBOLS = (
     "rad_create", "rad_accumulate_step", "rad_accumulate_steps", "rad_accumulate_steps_regions",
@@ -43,6 +46,8 @@ class rad_config(ctypes.Structure):
         ("n_regions", ctypes.c_int32), ("window_type", ctypes.c_int32),
         ("window_origin", ctypes.c_double * 3), ("window_extent", ctypes.c_double * 3),
         ("nyquist_factor", ctypes.c_double),
+        ("form_factor_type", ctypes.c_int32), ("reserved0", ctypes.c_int32),
+        ("form_factor_size", ctypes.c_double * 3),
     ]
 
 
@@ -128,9 +133,10 @@ def _check(status: int, handle) -> None:
 # ------------------------------------------------------------------ ABI-named functions
 def rad_create(dirs, omega, dt: float, t0: float = 0.0, scale: float = 0.0,
                state_dtype: int = RAD_F32, flags: int = 0, device: int = 0, n_regions: int = 0,
-               window=None, nyquist: float = 0.0) -> int:
+               window=None, nyquist: float = 0.0, form_factor=None) -> int:
     """-> opaque handle (int).  dirs [D,3], omega [W]: HOST fp64 (copied by the library).
-    window: None or (type name | code, origin[3], extent[3])."""
+    window: None or (type name | code, origin[3], extent[3]).
+    form_factor: None or (type name | code, size[3] in metres)."""
     dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
     omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
     cfg = rad_config(ctypes.sizeof(rad_config), device, dirs.shape[0], omega.shape[0],
@@ -142,6 +148,10 @@ def rad_create(dirs, omega, dt: float, t0: float = 0.0, scale: float = 0.0,
         cfg.window_type = WINDOW_TYPES[kind] if isinstance(kind, str) else int(kind)
         cfg.window_origin = (ctypes.c_double * 3)(*[float(x) for x in origin])
         cfg.window_extent = (ctypes.c_double * 3)(*[float(x) for x in extent])
+    if form_factor is not None:
+        kind, size = form_factor
+        cfg.form_factor_type = FORM_FACTOR_TYPES[kind] if isinstance(kind, str) else int(kind)
+        cfg.form_factor_size = (ctypes.c_double * 3)(*[float(x) for x in size])
     h = ctypes.c_void_p()
     _check(load().rad_create(ctypes.byref(cfg), ctypes.byref(h)), None)
     return h.value
@@ -242,14 +252,15 @@ class Detector:
     pinned torch CPU tensors (host path, copies inside the library)."""
 
     def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, state_dtype=np.float32, flags=0, device=0,
-                 n_regions=0, window=None, nyquist=0.0):
+                 n_regions=0, window=None, nyquist=0.0, form_factor=None):
         self.D = int(np.asarray(dirs).reshape(-1, 3).shape[0])
         self.W = int(np.asarray(omega).reshape(-1).shape[0])
         self.R = max(1, int(n_regions))
         self.np_dtype = np.dtype(state_dtype)
         code = {np.dtype(np.float32): RAD_F32, np.dtype(np.float64): RAD_F64}[self.np_dtype]
         self.device = device
-        self.handle = rad_create(dirs, omega, dt, t0, scale, code, flags, device, n_regions, window, nyquist)
+        self.handle = rad_create(dirs, omega, dt, t0, scale, code, flags, device, n_regions, window, nyquist,
+                                 form_factor)
 
     def _shape(self, *tail):
         return ((self.R,) if self.R > 1 else ()) + (self.D, self.W) + tail

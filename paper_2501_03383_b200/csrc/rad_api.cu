@@ -50,7 +50,7 @@ void free_all(Handle &h)
 {
     cudaFree(h.dirs_d); cudaFree(h.basis_d); cudaFree(h.F_d); cudaFree(h.Ff_d); cudaFree(h.fl_d);
     cudaFree(h.acc_d); cudaFree(h.partial_d); cudaFree(h.stage_d[0]); cudaFree(h.stage_d[1]);
-    cudaFree(h.out_d); cudaFree(h.chunks_d); cudaFree(h.reg_cstart_d); cudaFree(h.omega_d);
+    cudaFree(h.out_d); cudaFree(h.chunks_d); cudaFree(h.reg_cstart_d); cudaFree(h.omega_d); cudaFree(h.F2_d);
 
     if (h.chunks_h) cudaFreeHost(h.chunks_h);
     if (h.reg_cstart_h) cudaFreeHost(h.reg_cstart_h);
@@ -310,7 +310,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.chunk = choose_chunk(h, (region_off ? n + (long long)h.R * 64 : n) * n_steps);
     p.n_dir = h.D; p.n_omega = h.W; p.w_pad = h.w_pad;
     p.n_ftiles = h.n_ftiles; p.n_wtiles = h.n_wtiles;
-    p.dirs = h.dirs_d; p.F = h.F_d; p.Ff = h.Ff_d; p.fl = h.fl_d;
+    p.dirs = h.dirs_d; p.F = h.F_d; p.Ff = h.Ff_d; p.fl = h.fl_d; p.F2 = h.F2_d;
     p.ts32 = (h.t0 + (double)step * h.dt) * h.f_unit * kTwo32;
     p.dts32 = h.dt * h.f_unit * kTwo32;
     p.nyq_lim = h.nyq_lim; p.dt64 = h.dt; p.omega64 = h.omega_d;
@@ -347,6 +347,11 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
         stream_grid = (int)std::min<long long>(n_tiles, (long long)stream_blocks_per_sm(h.stream_nb) * h.sm_count);
         for (int j = 0; j < 16; ++j) { p.sF[j] = h.sF[j]; p.sFf[j] = h.sFf[j]; p.sfl[j] = h.sfl[j]; }
         p.sdir[0] = h.sdir[0]; p.sdir[1] = h.sdir[1];
+        if (h.F2_d) {  // bin b = d * WB + j of the streaming kernel
+            const int wb = h.stream_nb / h.stream_nd;
+            for (int d = 0; d < h.stream_nd && d < h.D; ++d)
+                for (int j = 0; j < wb && j < h.W; ++j) p.sF2[d * wb + j] = h.F2_h[(size_t)d * h.w_pad + j];
+        }
         n_chunks = stream_grid;
     }
     if (h.deterministic) {
@@ -408,6 +413,12 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         for (int c = 0; c < 3; ++c)
             if (!std::isfinite(cfg->window_origin[c]) || !std::isfinite(cfg->window_extent[c]))
                 return fail(nullptr, RAD_ERR_INVALID_ARG, "window origin/extent must be finite");
+    if (cfg->form_factor_type < RAD_FF_NONE || cfg->form_factor_type > RAD_FF_INCOHERENT || cfg->reserved0 != 0)
+        return fail(nullptr, RAD_ERR_INVALID_ARG, "unknown form_factor_type (or reserved0 != 0)");
+    if (cfg->form_factor_type != RAD_FF_NONE)
+        for (int c = 0; c < 3; ++c)
+            if (!std::isfinite(cfg->form_factor_size[c]) || cfg->form_factor_size[c] < 0.0)
+                return fail(nullptr, RAD_ERR_INVALID_ARG, "form_factor_size must be finite and >= 0");
     for (int j = 0; j < cfg->n_omega; ++j) {
         const double w = cfg->omega[j];
         if (!std::isfinite(w) || !(w > 0.0) || (j > 0 && !(w > cfg->omega[j - 1])))
@@ -425,6 +436,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         h.win_il[c] = (h.win_type != RAD_WINDOW_NONE && cfg->window_extent[c] > 0.0) ? 1.0 / cfg->window_extent[c] : 0.0;
     }
     if (h.win_il[0] == 0.0 && h.win_il[1] == 0.0 && h.win_il[2] == 0.0) h.win_type = RAD_WINDOW_NONE;
+    h.ff_type = cfg->form_factor_type;
     h.dt = cfg->dt; h.t0 = cfg->t0;
     h.scale = cfg->scale == 0.0 ? default_scale() : cfg->scale;
     h.state_f64 = cfg->state_dtype == RAD_F64;
@@ -505,6 +517,31 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         if (j < 16 && j < h.W) { h.sF[j] = F[j]; h.sFf[j] = Ff[j]; h.sfl[j] = fl[j]; }
     }
 
+    // macro-particle form factor (rad.h, reading FF1): F^2(n, w_j) per (direction, frequency), fp64 -> fp32
+    if (h.ff_type != RAD_FF_NONE) {
+        h.F2_h.assign((size_t)h.D * h.w_pad, 0.0f);
+        const double *sz = cfg->form_factor_size;
+        for (int d = 0; d < h.D; ++d)
+            for (int j = 0; j < h.W; ++j) {
+                const double *n = &h.dirs_h[3 * d];
+                const double om = h.omega_h[j];
+                double Fv = 0.0;
+                if (h.ff_type == RAD_FF_GAUSSIAN) {
+                    double q = 0.0;
+                    for (int c = 0; c < 3; ++c) { const double x = om * n[c] * sz[c] / kC; q += x * x; }
+                    Fv = std::exp(-0.5 * q);
+                } else if (h.ff_type == RAD_FF_CIC) {
+                    Fv = 1.0;
+                    for (int c = 0; c < 3; ++c) {
+                        const double x = om * n[c] * sz[c] / (2.0 * kC);
+                        const double sinc = x == 0.0 ? 1.0 : std::sin(x) / x;
+                        Fv *= sinc * sinc;
+                    }
+                }
+                h.F2_h[(size_t)d * h.w_pad + j] = (float)(Fv * Fv);
+            }
+    }
+
     cudaError_t e = cudaSetDevice(h.device);
     if (e != cudaSuccess) { delete hh; return cuda_fail(nullptr, e, "cudaSetDevice"); }
     cudaDeviceProp prop;
@@ -518,7 +555,8 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
               cudaMalloc(&h.Ff_d, sizeof(float) * h.w_pad) == cudaSuccess &&
               cudaMalloc(&h.fl_d, sizeof(float) * h.w_pad) == cudaSuccess &&
               cudaMalloc(&h.acc_d, acc_bytes) == cudaSuccess &&
-              (h.nyq_lim == 0.0 || cudaMalloc(&h.omega_d, sizeof(double) * h.W) == cudaSuccess);
+              (h.nyq_lim == 0.0 || cudaMalloc(&h.omega_d, sizeof(double) * h.W) == cudaSuccess) &&
+              (h.F2_h.empty() || cudaMalloc(&h.F2_d, sizeof(float) * h.F2_h.size()) == cudaSuccess);
     if (!ok) {
         cudaGetLastError(); free_all(h); delete hh;
         return fail(nullptr, RAD_ERR_ALLOC, "cudaMalloc(tables/accumulator) failed");
@@ -529,6 +567,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
          cudaMemcpy(h.Ff_d, Ff.data(), sizeof(float) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemcpy(h.fl_d, fl.data(), sizeof(float) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemset(h.acc_d, 0, acc_bytes) == cudaSuccess &&
+         (!h.F2_d || cudaMemcpy(h.F2_d, h.F2_h.data(), sizeof(float) * h.F2_h.size(), cudaMemcpyHostToDevice) == cudaSuccess) &&
          (!h.omega_d || cudaMemcpy(h.omega_d, h.omega_h.data(), sizeof(double) * h.W, cudaMemcpyHostToDevice) == cudaSuccess) &&
          cudaStreamCreateWithFlags(&h.copy_stream, cudaStreamNonBlocking) == cudaSuccess;
     for (int i = 0; ok && i < 2; ++i)

@@ -44,7 +44,16 @@ __device__ __forceinline__ ST ld_state(const void *p, long long k)
 struct Particle {
     double rx, ry, rz, bx, by, bz;  // fp64 for the phase and the Doppler factor
     float bfx, bfy, bfz, bdx, bdy, bdz, wdt;
+    float w, ww;  // form factor on: macro weight w and w^2 - w (wdt is then dt [x window] only)
 };
+
+// form-factor weight g = sqrt(w + (w^2 - w) F^2) of one update (rad.h, reading FF1): FFMA + MUFU.SQRT
+__device__ __forceinline__ float ff_weight(float w, float ww, float F2)
+{
+    float g;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(g) : "f"(fmaf(ww, F2, w)));
+    return g;
+}
 
 __device__ __forceinline__ void stage_record(const Particle &p, const DirRec &dr, double ts32,
                                              float4 &rec, float &sf, uint32_t *T_out = nullptr,
@@ -149,8 +158,10 @@ __device__ __forceinline__ float window_weight(const AccumParams &P, double rx, 
     return W;
 }
 
+// ff: form factor on -- the macro weight stays out of the amplitude record (it enters per update
+// through ff_weight); the record then carries dt [x window] only
 template <typename ST, bool WIN = true>
-__device__ __forceinline__ Particle load_particle(const AccumParams &P, long long k, bool valid)
+__device__ __forceinline__ Particle load_particle(const AccumParams &P, long long k, bool valid, const bool ff = false)
 {
     Particle p;
     if (valid) {
@@ -165,11 +176,13 @@ __device__ __forceinline__ Particle load_particle(const AccumParams &P, long lon
         p.bx = to_f64(bx); p.by = to_f64(by); p.bz = to_f64(bz);
         p.bfx = (float)bx; p.bfy = (float)by; p.bfz = (float)bz;
         p.bdx = (float)dx; p.bdy = (float)dy; p.bdz = (float)dz;
-        p.wdt = (float)w * P.dt;
+        p.w = (float)w;
+        p.ww = fmaf(p.w, p.w, -p.w);
+        p.wdt = ff ? P.dt : p.w * P.dt;
         if (WIN) p.wdt *= window_weight(P, p.rx, p.ry, p.rz);
     } else {  // padding lane: zero amplitude, harmless phase
         p.rx = p.ry = p.rz = p.bx = p.by = p.bz = 0.0;
-        p.bfx = p.bfy = p.bfz = p.bdx = p.bdy = p.bdz = p.wdt = 0.0f;
+        p.bfx = p.bfy = p.bfz = p.bdx = p.bdy = p.bdz = p.wdt = p.w = p.ww = 0.0f;
     }
     return p;
 }

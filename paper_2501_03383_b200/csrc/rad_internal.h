@@ -65,6 +65,7 @@ struct AccumParams {
     const uint32_t *F;     // [w_pad] integer part of f_j / f_unit
     const float *Ff;       // [w_pad] (float)F_j
     const float *fl;       // [w_pad] f_j / f_unit - F_j  in [-0.5, 0.5]
+    const float *F2;       // form factor: [D][w_pad] F^2(n, w_j) (rad.h, reading FF1), NULL: off
     double ts32;           // (t0 + step dt) f_unit 2^32
     double dts32;          // dt f_unit 2^32: multi-step calls, chunk time = ts32 + chunk.step * dts32
     float dt;              // quadrature weight
@@ -80,6 +81,7 @@ struct AccumParams {
     // parameter constant bank (operands come straight from c[0][..]: no loads, no registers)
     uint32_t sF[16];
     float sFf[16], sfl[16];
+    float sF2[16];         // form factor: F^2 of bin b = d * WB + j
     DirRec sdir[2];
     // uniform-grid variant only: LW*(f_1 - f_0)/f_unit = rot_G + rot_gl (integer + fraction)
     uint32_t rot_G;
@@ -148,6 +150,9 @@ struct Handle {
     double *basis_d = nullptr;       // [D][6] fp64 e1, e2 (amplitude export/import)
     uint32_t *F_d = nullptr;
     float *Ff_d = nullptr, *fl_d = nullptr;
+    int ff_type = 0;                 // RAD_FF_*
+    float *F2_d = nullptr;           // form factor on: [D][w_pad] F^2(n, w_j)
+    std::vector<float> F2_h;         // host copy (streaming shapes pass it in the parameter bank)
     double *acc_d = nullptr;         // [D][w_pad][4]
     double *partial_d = nullptr;     // deterministic workspace
     size_t partial_bytes = 0;

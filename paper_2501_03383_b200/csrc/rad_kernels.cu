@@ -95,7 +95,10 @@ __device__ __forceinline__ bool decode_task(const AccumParams &P, int warp, int 
 // NYQ (general grid only): Nyquist limiter -- the staging lane also finds, per (particle,
 // direction), how many bins lie below the cut-off (nyquist_count); the sweep accumulates bin j
 // only if j < that count (one ISETP per update, the four FFMAs are predicated).
-template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ>
+// FF: macro-particle form factor (rad.h, reading FF1) -- every update's (cos, sin) is scaled by
+// g = sqrt(w + (w^2 - w) F^2): F^2 of the thread's S bins in registers, (w, w^2 - w) of the batch's
+// particles in shared memory; one FFMA + MUFU.SQRT + 2 FMUL more per update.
+template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ, bool FF>
 __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
 {
     static_assert(!(UNI && NYQ), "the limiter runs on the general-grid kernel");
@@ -106,6 +109,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
     __shared__ float s_sf[kWarpsPerBlock][kBatch * DPW];
     __shared__ float2 s_rot[UNI ? kWarpsPerBlock : 1][UNI ? kBatch * DPW : 1];
     __shared__ int s_jc[NYQ ? kWarpsPerBlock : 1][NYQ ? kBatch * DPW : 1];
+    __shared__ float2 s_w[FF ? kWarpsPerBlock : 1][FF ? kBatch : 1];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     int wt, ci, region;
@@ -128,16 +132,24 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
     }
 #pragma unroll
     for (int i = 0; i < S; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.0f;
+    float F2r[FF ? S : 1];
+    if (FF) {
+        const float *row = P.F2 + (size_t)min(dg * DPW + ld, P.n_dir - 1) * P.w_pad + jbase;
+#pragma unroll
+        for (int i = 0; i < S; ++i) F2r[FF ? i : 0] = __ldg(row + i * LW);
+    }
 
     float4 *rec = s_rec[warp];
     float *sfs = s_sf[warp];
     float2 *rots = s_rot[UNI ? warp : 0];
     int *jcs = s_jc[NYQ ? warp : 0];
+    float2 *ws = s_w[FF ? warp : 0];
 
     for (long long kb = k0; kb < k1; kb += kBatch) {
         {  // a1: stage
             const long long k = kb + lane;
-            const Particle p = load_particle<ST>(P, k, k < k1);
+            const Particle p = load_particle<ST, true>(P, k, k < k1, FF);
+            if (FF) ws[lane] = make_float2(p.w, p.ww);
 #pragma unroll(DPW > 2 ? 1 : DPW)  // 4 or 8 directions per warp: keep the staging code out of the register budget
             for (int dd = 0; dd < DPW; ++dd) {
                 const int dir = min(dg * DPW + dd, P.n_dir - 1);
@@ -165,20 +177,23 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 const float2 rot = rots[kk * DPW + ld];
                 float zi0, zr0;
                 phase_sincos(F[0], Ff[0], fl[0], __float_as_uint(r4.x), r4.y, sf, zi0, zr0);
-                acc[MID][0] = fmaf(r4.z, zr0, acc[MID][0]);
-                acc[MID][1] = fmaf(r4.z, zi0, acc[MID][1]);
-                acc[MID][2] = fmaf(r4.w, zr0, acc[MID][2]);
-                acc[MID][3] = fmaf(r4.w, zi0, acc[MID][3]);
+                const float2 wq = FF ? ws[kk] : make_float2(0.0f, 0.0f);
+                auto add = [&](const int i, const float zr_, const float zi_) {  // acc[i] += a (x) z [* g]
+                    const float g = FF ? ff_weight(wq.x, wq.y, F2r[FF ? i : 0]) : 1.0f;
+                    const float cr = FF ? zr_ * g : zr_, ci = FF ? zi_ * g : zi_;
+                    acc[i][0] = fmaf(r4.z, cr, acc[i][0]);
+                    acc[i][1] = fmaf(r4.z, ci, acc[i][1]);
+                    acc[i][2] = fmaf(r4.w, cr, acc[i][2]);
+                    acc[i][3] = fmaf(r4.w, ci, acc[i][3]);
+                };
+                add(MID, zr0, zi0);
                 float zr = zr0, zi = zi0;
 #pragma unroll
                 for (int i = MID + 1; i < S; ++i) {  // forwards: z *= rot
                     const float t = fmaf(zr, rot.x, -zi * rot.y);
                     zi = fmaf(zi, rot.x, zr * rot.y);
                     zr = t;
-                    acc[i][0] = fmaf(r4.z, zr, acc[i][0]);
-                    acc[i][1] = fmaf(r4.z, zi, acc[i][1]);
-                    acc[i][2] = fmaf(r4.w, zr, acc[i][2]);
-                    acc[i][3] = fmaf(r4.w, zi, acc[i][3]);
+                    add(i, zr, zi);
                 }
                 zr = zr0; zi = zi0;
 #pragma unroll
@@ -186,10 +201,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                     const float t = fmaf(zr, rot.x, zi * rot.y);
                     zi = fmaf(zi, rot.x, -zr * rot.y);
                     zr = t;
-                    acc[i][0] = fmaf(r4.z, zr, acc[i][0]);
-                    acc[i][1] = fmaf(r4.z, zi, acc[i][1]);
-                    acc[i][2] = fmaf(r4.w, zr, acc[i][2]);
-                    acc[i][3] = fmaf(r4.w, zi, acc[i][3]);
+                    add(i, zr, zi);
                 }
             }
         } else {
@@ -200,6 +212,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 const float sf = sfs[kk * DPW + ld];
                 const uint32_t T = __float_as_uint(r4.x);
                 const int m = NYQ ? jcs[kk * DPW + ld] - jbase : 0;  // bins jbase + i*LW < count are kept
+                const float2 wq = FF ? ws[kk] : make_float2(0.0f, 0.0f);
 #pragma unroll
                 for (int i = 0; i < S; ++i) {
                     float sn, cs;
@@ -207,6 +220,11 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                         phase_sincos_poly(F[i % NC], Ff[i % NC], fl[i % NC], T, r4.y, sf, sn, cs);
                     else
                         phase_sincos(F[i % NC], Ff[i % NC], fl[i % NC], T, r4.y, sf, sn, cs);
+                    if (FF) {
+                        const float g = ff_weight(wq.x, wq.y, F2r[FF ? i : 0]);
+                        sn *= g;
+                        cs *= g;
+                    }
                     if (NYQ) {
                         // limiter: one SETP + four predicated FFMAs written in PTX, so that the
                         // compiler keeps the bins' instruction streams interleaved (as C++ it
@@ -238,23 +256,33 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
 
 // ------------------------------------------------------------------------------------------
 // Launch logic.
-template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ>
+template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ, bool FF>
 static cudaError_t launch_one(const AccumParams &p, cudaStream_t s, bool overlap)
 {
     const long long n_tasks = (long long)p.n_wtiles * p.n_chunks;
     const unsigned grid = (unsigned)((n_tasks + kWarpsPerBlock - 1) / kWarpsPerBlock);
-    return launch_kernel(rad_accum<ST, LW, S, MINB, UNI, NYQ>, dim3(grid), dim3(kThreads), 0, s, overlap, p);
+    return launch_kernel(rad_accum<ST, LW, S, MINB, UNI, NYQ, FF>, dim3(grid), dim3(kThreads), 0, s, overlap, p);
+}
+
+template <typename ST, bool UNI, bool NYQ, bool FF>
+static cudaError_t dispatch_lw(const Handle &h, const AccumParams &p, cudaStream_t s)
+{
+    // the form-factor variants need 8 more registers (F^2 of the strip): the narrow tile shapes and
+    // the limiter variant would spill at the 128-register cap of 4 blocks per SM -> 3 blocks (168)
+    constexpr int kMB = FF ? kMinBlocks - 1 : kMinBlocks;
+    constexpr int kMBwide = (FF && NYQ) ? kMinBlocks - 1 : kMinBlocks;
+    switch (h.lw) {
+        case 32: return launch_one<ST, 32, kStrip, kMBwide, UNI, NYQ, FF>(p, s, h.overlap);
+        case 16: return launch_one<ST, 16, kStrip, kMBwide, UNI, NYQ, FF>(p, s, h.overlap);
+        case 8: return launch_one<ST, 8, kStrip, kMB, UNI, NYQ, FF>(p, s, h.overlap);
+        default: return launch_one<ST, 4, kStrip, kMB, UNI, NYQ, FF>(p, s, h.overlap);
+    }
 }
 
 template <typename ST, bool UNI, bool NYQ>
 static cudaError_t dispatch(const Handle &h, const AccumParams &p, cudaStream_t s)
 {
-    switch (h.lw) {
-        case 32: return launch_one<ST, 32, kStrip, kMinBlocks, UNI, NYQ>(p, s, h.overlap);
-        case 16: return launch_one<ST, 16, kStrip, kMinBlocks, UNI, NYQ>(p, s, h.overlap);
-        case 8: return launch_one<ST, 8, kStrip, kMinBlocks, UNI, NYQ>(p, s, h.overlap);
-        default: return launch_one<ST, 4, kStrip, kMinBlocks, UNI, NYQ>(p, s, h.overlap);
-    }
+    return p.F2 ? dispatch_lw<ST, UNI, NYQ, true>(h, p, s) : dispatch_lw<ST, UNI, NYQ, false>(h, p, s);
 }
 
 cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_f64,
@@ -262,14 +290,14 @@ cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_
 {
     *n_launches = 1;
     if (h.uniform) {
-        *variant = "uniform";
+        *variant = p.F2 ? "uniform+formfactor" : "uniform";
         return state_f64 ? dispatch<double, true, false>(h, p, s) : dispatch<float, true, false>(h, p, s);
     }
     if (p.nyq_lim > 0.0) {
-        *variant = "general+nyquist";
+        *variant = p.F2 ? "general+nyquist+formfactor" : "general+nyquist";
         return state_f64 ? dispatch<double, false, true>(h, p, s) : dispatch<float, false, true>(h, p, s);
     }
-    *variant = "general";
+    *variant = p.F2 ? "general+formfactor" : "general";
     return state_f64 ? dispatch<double, false, false>(h, p, s) : dispatch<float, false, false>(h, p, s);
 }
 

@@ -116,7 +116,9 @@ __device__ __forceinline__ Particle make_particle(ST rx, ST ry, ST rz, ST bx, ST
     p.bx = to_f64(bx); p.by = to_f64(by); p.bz = to_f64(bz);
     p.bfx = (float)bx; p.bfy = (float)by; p.bfz = (float)bz;
     p.bdx = (float)dx; p.bdy = (float)dy; p.bdz = (float)dz;
-    p.wdt = (float)w * P.dt;
+    p.w = (float)w;
+    p.ww = fmaf(p.w, p.w, -p.w);
+    p.wdt = (WIN && P.F2) ? P.dt : p.w * P.dt;  // form factor on: the weight enters per update (ff_weight)
     if (WIN) p.wdt *= window_weight(P, p.rx, p.ry, p.rz);
     return p;
 }
@@ -133,7 +135,7 @@ template <> struct Vec16<double> {
 };
 
 // a1 + a2 for one particle: all bins of all (<= 2) directions
-template <int NB, int ND>
+template <int NB, int ND, bool WIN>
 __device__ __forceinline__ void accumulate_particle(const AccumParams &P, const Particle &p,
                                                     unsigned long long (&acc01)[NB], unsigned long long (&acc23)[NB])
 {
@@ -148,6 +150,11 @@ __device__ __forceinline__ void accumulate_particle(const AccumParams &P, const 
         for (int j = 0; j < WB; ++j) {  // a2
             float sn, cs;
             phase_sincos(P.sF[j], P.sFf[j], P.sfl[j], __float_as_uint(r4.x), r4.y, sf, sn, cs);
+            if (WIN && P.F2) {  // macro-particle form factor (rad.h, reading FF1)
+                const float g = ff_weight(p.w, p.ww, P.sF2[d * WB + j]);
+                sn *= g;
+                cs *= g;
+            }
             const unsigned long long z = pack2(cs, sn);
             fma2(acc01[d * WB + j], a1, z);  // (Re, Im) A1 += a1 (cos, sin)
             fma2(acc23[d * WB + j], a2, z);  // (Re, Im) A2 += a2 (cos, sin)
@@ -158,8 +165,8 @@ __device__ __forceinline__ void accumulate_particle(const AccumParams &P, const 
 // NB bins per thread = ND directions x WB frequencies (compile time; W is padded to WB with
 // zero-frequency bins that are discarded).  Per-bin frequency constants come straight from the
 // kernel-parameter constant bank (P.sF/sFf/sfl), not from registers.
-// WIN: spatial window compiled in (kept out of the default instantiation: the streaming kernel
-// is latency bound and loses 3 % to the extra per-particle code even when the window is off)
+// WIN: spatial window and macro-particle form factor compiled in (kept out of the default
+// instantiation: the streaming kernel loses 3 % to the extra per-particle code even when both are off)
 template <typename ST, int NB, int ND, bool WIN>
 __global__ void __launch_bounds__(32 * stream_warps(NB), 1) rad_accum_stream(const AccumParams P, const int use_bulk)
 {
@@ -247,15 +254,15 @@ __global__ void __launch_bounds__(32 * stream_warps(NB), 1) rad_accum_stream(con
             const Particle p = make_particle<ST, WIN>(v[0].get(pp), v[1].get(pp), v[2].get(pp), v[3].get(pp),
                                                       v[4].get(pp), v[5].get(pp), v[6].get(pp), v[7].get(pp),
                                                       v[8].get(pp), v[9].get(pp), P);
-            accumulate_particle<NB, ND>(P, p, acc01, acc23);
+            accumulate_particle<NB, ND, WIN>(P, p, acc01, acc23);
         }
         cur = nxt;
         stage = other;
     }
     // ragged tail / unaligned arrays: plain coalesced loads, one particle per lane
     for (long long k = n_full * WTILE + gw * 32 + lane; k < N; k += GW * 32) {
-        const Particle p = load_particle<ST, WIN>(P, k, true);
-        accumulate_particle<NB, ND>(P, p, acc01, acc23);
+        const Particle p = load_particle<ST, WIN>(P, k, true, WIN && P.F2);
+        accumulate_particle<NB, ND, WIN>(P, p, acc01, acc23);
     }
 
     // a3: warp-shuffle reduction, cross-warp sum in shared memory, one fp64 add per value
@@ -307,7 +314,7 @@ cudaError_t launch_stream_w(const AccumParams &p, int grid, cudaStream_t s, bool
 template <typename ST, int NB, int ND>
 cudaError_t launch_stream_t(const AccumParams &p, int grid, cudaStream_t s, bool overlap)
 {
-    return p.win_type != RAD_WINDOW_NONE ? launch_stream_w<ST, NB, ND, true>(p, grid, s, overlap)
+    return (p.win_type != RAD_WINDOW_NONE || p.F2) ? launch_stream_w<ST, NB, ND, true>(p, grid, s, overlap)
                                          : launch_stream_w<ST, NB, ND, false>(p, grid, s, overlap);
 }
 

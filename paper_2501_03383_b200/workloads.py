@@ -109,7 +109,7 @@ class KHISource:
     """
 
     def __init__(self, n: int, seed: int, dt: float, L=10e-6, B0=50.0, stream=0.2,
-                 sigma=0.01, shear=0.5e-6, regions=None):
+                 sigma=0.01, shear=0.5e-6, regions=None, weights=None):
         self.n, self.dt, self.L, self.B0, self.shear = n, dt, L, B0, shear
         self.r = np.stack([L * uniform01(seed, s, n) for s in (0, 1, 2)], axis=0)
         self.b = np.stack([sigma * normal01(seed, 10 + s, n) for s in (0, 1, 2)], axis=0)
@@ -130,7 +130,11 @@ class KHISource:
             self.region_offsets = np.concatenate([[0], np.cumsum(counts)]).astype(np.int64)
         g = 1.0 / np.sqrt(1.0 - np.sum(self.b * self.b, axis=0))
         self.qm = (-E_CHARGE / M_ELECTRON) / g      # q/(gamma m); gamma is conserved (E=0)
-        self.w = np.ones(n)
+        # macro weights: 1 (BASELINE.json configs), or seeded log-uniform in [1, wmax) for the
+        # form-factor workloads (a PIC run with density gradients has weights spanning decades)
+        self.w = np.ones(n) if weights is None else float(weights) ** uniform01(seed, 20, n)
+        if weights is not None and regions is not None:
+            self.w = self.w[order]
 
     def _Bz(self):
         x, y = self.r[0], self.r[1]
@@ -165,6 +169,7 @@ class Workload:
     kind: str                      # "helix" | "khi"
     t0: float = 0.0
     extra: dict = field(default_factory=dict)
+    form_factor: Optional[tuple] = None     # (type name, size[3] in metres) for rad_config / the oracle
 
     @property
     def n_dir(self) -> int:
@@ -241,6 +246,13 @@ def make_workload(cfg: str) -> Workload:
         # uniform-grid rotation-recurrence kernel (a2') is measured
         return Workload("cfg1u_khi_linear_grid", 65536, 1000, 1e-17, dirs_fibonacci(128),
                         omega_linear(512, 1e17), np.float32, BASE_SEED + 1, "khi")
+    if cfg == "1f":
+        # config 1 with macro weights log-uniform in [1, 1e4) and a Gaussian macro-particle shape of
+        # 30 nm (the form factor passes from coherent to incoherent around w = c / 30 nm = 1e16 rad/s,
+        # the middle of the grid): the form-factor leg of bench.py (not a BASELINE.json config)
+        return Workload("cfg1f_khi_form_factor", 65536, 1000, 1e-17, dirs_fibonacci(128),
+                        omega_log(512), np.float32, BASE_SEED + 1, "khi", extra={"weights": 1e4},
+                        form_factor=("gaussian", (3e-8, 3e-8, 3e-8)))
     if cfg == "5r":
         # smallest KHI run = 192 x 256 x 12 cells x 9 particles per cell on 16
         # GPUs -> 331 776 particles per GPU; line 196: one ML sample = the ~3e4 particles of a
@@ -250,4 +262,4 @@ def make_workload(cfg: str) -> Workload:
     raise KeyError(cfg)
 
 
-ALL_CONFIGS = ("0", "1", "1u", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r")
+ALL_CONFIGS = ("0", "1", "1u", "1f", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r")

@@ -48,15 +48,18 @@ def test_struct_layout_matches_header(tmp_path):
     src.write_text('''#include <stdio.h>
 #include <stddef.h>
 #include "rad.h"
-int main(void){ printf("%zu %zu %zu %zu %zu %zu %zu\\n", sizeof(rad_config), offsetof(rad_config, n_dir),
+int main(void){ printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\\n", sizeof(rad_config), offsetof(rad_config, n_dir),
   offsetof(rad_config, dirs), offsetof(rad_config, omega), offsetof(rad_config, dt),
-  offsetof(rad_config, state_dtype), offsetof(rad_config, flags)); return 0; }''')
+  offsetof(rad_config, state_dtype), offsetof(rad_config, flags), offsetof(rad_config, window_origin),
+  offsetof(rad_config, nyquist_factor), offsetof(rad_config, form_factor_type),
+  offsetof(rad_config, form_factor_size)); return 0; }''')
     exe = tmp_path / "layout"
     subprocess.run(["gcc", "-I", str(ROOT / "include"), str(src), "-o", str(exe)], check=True)
     got = [int(x) for x in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()]
     c = binding.rad_config
     assert got == [ctypes.sizeof(c), c.n_dir.offset, c.dirs.offset, c.omega.offset, c.dt.offset,
-                   c.state_dtype.offset, c.flags.offset]
+                   c.state_dtype.offset, c.flags.offset, c.window_origin.offset, c.nyquist_factor.offset,
+                   c.form_factor_type.offset, c.form_factor_size.offset]
 
 
 def test_status_strings_and_version(lib):
@@ -81,6 +84,10 @@ GOOD_OMEGA = np.array([1e15, 2e15, 4e15])
     (dict(scale=-1.0), "scale"),
     (dict(state_dtype=7), "state_dtype"),
     (dict(flags=1 << 9), "flag"),
+    (dict(form_factor=(7, (0, 0, 0))), "form_factor_type"),
+    (dict(form_factor=("gaussian", (1e-8, float("inf"), 0))), "form_factor_size"),
+    (dict(nyquist=-0.5), "nyquist_factor"),
+    (dict(window=(5, (0, 0, 0), (1, 1, 1))), "window_type"),
 ])
 def test_create_rejects_bad_arguments_without_a_device(lib, kw, msg):
     from paper_2501_03383_b200 import binding

@@ -858,3 +858,82 @@ def test_e2e_call_sequence_every_step_spectrum_matches_oracle(oracle_mod, region
         for r in range(R):
             sl = slice(r * w.n_dir, (r + 1) * w.n_dir)
             P.assert_parity(got[i][sl], refs[i][sl], what=f"e2e sequence step {i} region {r}")
+
+
+# ------------------------------------------------- macro-particle form factor (reading FF1)
+@pytest.mark.parametrize("kind,size", [("gaussian", (3e-8, 1e-8, 2e-8)), ("cic", (6e-8, 6e-8, 3e-8)),
+                                        ("incoherent", (0.0, 0.0, 0.0))])
+@pytest.mark.parametrize("shape", ["general", "uniform", "stream", "regions", "nyquist"])
+def test_form_factor(oracle_mod, kind, size, shape):
+    """NEXT-3 macro-particle form factor (rad.h, reading FF1; "correctly quantify
+    coherent and incoherent radiation [39]"): g = sqrt(w + (w^2 - w) F^2(n, w_j)) per update, through
+    every accumulate kernel; macro weights log-uniform in [1, 1e4), shape sizes chosen so that F
+    passes from 1 to 0 inside the frequency grid; fp32 state."""
+    from paper_2501_03383_b200 import binding
+    ff = (kind, size)
+    kw = {}
+    if shape == "uniform":
+        dirs, omega = wl.dirs_fibonacci(6), np.linspace(2e14, 6e16, 128)
+    elif shape == "stream":
+        dirs, omega = wl.dirs_fibonacci(2), wl.omega_log(8, 1e15, 1e17)
+    elif shape == "nyquist":
+        dirs, omega, kw = wl.dirs_fibonacci(5), wl.omega_log(96), {"nyquist": 0.5}
+    else:
+        dirs, omega = wl.dirs_fibonacci(5), wl.omega_log(96)
+    w = wl.Workload("ff", 3000, 2, 1e-17, dirs, omega, np.float32, wl.BASE_SEED + 80, "khi", extra={"weights": 1e4})
+    steps = list(w.steps())
+    assert steps[0][1][9].max() > 1e3
+    if shape == "regions":
+        off = np.array([0, 1000, 1000, 3000], dtype=np.int64)
+        o = oracle_mod.RegionOracle(3, w.dirs, w.omega, w.dt, scale=1.0, form_factor=ff)
+        for t, st in steps:
+            o.accumulate_step(t, off, *st)
+        with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, n_regions=3, form_factor=ff) as det:
+            for t, st in steps:
+                det.accumulate_step_regions(t, off, P.to_device(st))
+            S = det.spectrum()
+        for r in (0, 2):
+            P.assert_parity(S[r], o.spectrum()[r], what=f"form factor regions {r}")
+        assert np.all(S[1] == 0.0)
+        return
+    o = oracle_mod.Oracle(w.dirs, w.omega, w.dt, scale=1.0, form_factor=ff, **kw)
+    for t, st in steps:
+        o.accumulate_step(t, *st)
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, form_factor=ff, **kw) as det:
+        for t, st in steps:
+            det.accumulate_step(t, P.to_device(st))
+        S, variant = det.spectrum(), det.kernel_variant
+    want = {"general": "general+formfactor", "uniform": "uniform+formfactor", "stream": "stream",
+            "nyquist": "general+nyquist+formfactor"}[shape]
+    assert variant == want
+    ref = o.spectrum()
+    l2, mr = P.assert_parity(S, ref, what=f"form factor {kind} {shape}")
+    for d in range(len(dirs)):
+        P.assert_parity(S[d], ref[d], what=f"form factor {kind} {shape} dir {d}")
+    plain = oracle_mod.Oracle(w.dirs, w.omega, w.dt, scale=1.0, **kw)
+    for t, st in steps:
+        plain.accumulate_step(t, *st)
+    Sp = plain.spectrum()                                  # the form factor really changes the result:
+    assert np.max(np.abs(ref - Sp)[Sp > 0] / Sp[Sp > 0]) > 0.5   # incoherent bins drop by up to w (relL2 only sees the coherent peak)
+    print(f"form factor {kind}/{shape}: relL2={l2:.2e} maxrel={mr:.2e}")
+
+
+def test_form_factor_identities_and_argument_errors(oracle_mod):
+    """w = 1: any shape is the identity (same spectrum as a handle without form factor, to fp32
+    rounding of sqrt(1)); zero size = point particle = today's coherent sum; bad arguments."""
+    from paper_2501_03383_b200 import binding
+    w = wl.make_workload("3c")
+    (t, st), = list(w.steps(n_steps=1, n_particles=800))
+    S0, _ = P.run_gpu(w, [(t, st)])
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, form_factor=("gaussian", (3e-8, 3e-8, 3e-8))) as det:
+        det.accumulate_step(t, P.to_device(st))
+        assert P.rel_l2(det.spectrum(), S0) < 1e-6
+    stw = st[:9] + [np.full_like(st[9], 37.0)]
+    Sw, _ = P.run_gpu(w, [(t, stw)])
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, form_factor=("cic", (0.0, 0.0, 0.0))) as det:
+        det.accumulate_step(t, P.to_device(stw))
+        assert P.rel_l2(det.spectrum(), Sw) < 1e-6
+    with pytest.raises(binding.RadError, match="form_factor_type"):
+        binding.Detector(w.dirs, w.omega, w.dt, form_factor=(9, (0, 0, 0)))
+    with pytest.raises(binding.RadError, match="form_factor_size"):
+        binding.Detector(w.dirs, w.omega, w.dt, form_factor=("gaussian", (1e-8, -1e-8, 0)))
