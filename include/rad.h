@@ -76,6 +76,7 @@ typedef enum { RAD_F32 = 0, RAD_F64 = 1 } rad_dtype;
                                      bit-reproducible run to run (slower, more memory) */
 #define RAD_FLAG_FORCE_GENERAL 2u /* bit 1: never use the uniform-grid recurrence kernel */
 #define RAD_FLAG_OVERLAP_STEPS 4u /* bit 2: consecutive calls on one stream may overlap (below) */
+#define RAD_FLAG_FAST_GRIDDED 8u  /* bit 3: approximate fast path (gridded in retarded time, below) */
 
 /* RAD_FLAG_OVERLAP_STEPS.  The accumulate and result kernels are then launched with
  * programmatic stream serialization: the blocks of a call may start while the last blocks of
@@ -113,7 +114,35 @@ typedef struct {
     int32_t form_factor_type;     /* RAD_FF_*: macro-particle form factor (below); 0: none   */
     int32_t reserved0;            /* must be 0                                               */
     double form_factor_size[3];   /* m: s_x, s_y, s_z of the macro-particle shape, >= 0      */
+    /* RAD_FLAG_FAST_GRIDDED only (ignored otherwise): */
+    double fast_box_min[3];       /* m: a box that contains every particle position of the   */
+    double fast_box_max[3];       /*    accumulation window                                   */
+    int64_t fast_step_min;        /* step indices of the window: fast_step_min <= step_index  */
+    int64_t fast_step_max;        /*    <= fast_step_max in every accumulate call             */
+    double fast_tolerance;        /* target relative accuracy of the gridding, 0 -> 1e-6      */
 } rad_config;
+
+/* RAD_FLAG_FAST_GRIDDED -- the approximate fast path (PAPER.md line
+ * 142: the plugin's cost, "scaling with the number of particles, frequencies, and directions,
+ * easily exceed[s] the computational limits of the underlying particle-in-cell simulation").
+ * For one direction n the sum is a non-uniform Fourier sum over the retarded times
+ * tau = t - n.r/c of all (particle, step) terms,
+ *     A(n, w_j) = sum a(n) exp(i w_j tau),        a = the real transverse amplitude (A1, A2).
+ * Instead of W sin/cos pairs per term, every term is SPREAD onto a uniform grid in tau that the
+ * handle keeps per direction (spacing h = pi / (2 w_max), i.e. twofold oversampling of the highest
+ * frequency; a compactly supported "exponential of semicircle" kernel of width 4..12 grid points,
+ * chosen from fast_tolerance), at a cost independent of W: about 5 vector atomics per (particle,
+ * direction).  rad_spectrum / rad_amplitude then evaluate
+ *     A(n, w_j) = (1 / Phi(w_j)) sum_m g_m(n) exp(i w_j tau_m)
+ * exactly (a direct sum over the grid points with the integer-phase sin/cos of the direct path,
+ * no FFT) and divide by the kernel's Fourier transform Phi.  The result approximates the exact
+ * sum to about fast_tolerance (relative to the typical |A| of a bin); the oracle and the parity
+ * tolerances are those of the exact path.  Worth it when spectra are taken every many steps.
+ * Restrictions: one region, no Nyquist limiter, no form factor, no RAD_FLAG_DETERMINISTIC
+ * (RAD_ERR_UNSUPPORTED at rad_create); particles outside fast_box or steps outside the window
+ * are not deposited and make the next rad_spectrum / rad_amplitude fail with RAD_ERR_STATE.
+ * rad_export_accumulator / rad_import_accumulator / rad_add_amplitude are not available
+ * (RAD_ERR_UNSUPPORTED); rad_reset clears the grid. */
 
 /* Macro-particle form factor (the plugin "correctly quantif[ies] coherent and
  * incoherent radiation [39]"; ref [39], line 338, "a general form factor formalism for

@@ -18,7 +18,7 @@ LIB_PATH = _PKG / "librad.so"
 
 RAD_OK, RAD_ERR_INVALID_ARG, RAD_ERR_ALLOC, RAD_ERR_CUDA, RAD_ERR_STATE, RAD_ERR_UNSUPPORTED = range(6)
 RAD_F32, RAD_F64 = 0, 1
-RAD_FLAG_DETERMINISTIC, RAD_FLAG_FORCE_GENERAL, RAD_FLAG_OVERLAP_STEPS = 1, 2, 4
+RAD_FLAG_DETERMINISTIC, RAD_FLAG_FORCE_GENERAL, RAD_FLAG_OVERLAP_STEPS, RAD_FLAG_FAST_GRIDDED = 1, 2, 4, 8
 RAD_OUT_HOST, RAD_OUT_DEVICE, RAD_OUT_HOST_ASYNC = 0, 1, 2
 RAD_WINDOW_NONE, RAD_WINDOW_TRIANGLE, RAD_WINDOW_HAMMING = 0, 1, 2
 WINDOW_TYPES = {"none": RAD_WINDOW_NONE, "triangle": RAD_WINDOW_TRIANGLE, "hamming": RAD_WINDOW_HAMMING}
@@ -48,6 +48,9 @@ class rad_config(ctypes.Structure):
         ("nyquist_factor", ctypes.c_double),
         ("form_factor_type", ctypes.c_int32), ("reserved0", ctypes.c_int32),
         ("form_factor_size", ctypes.c_double * 3),
+        ("fast_box_min", ctypes.c_double * 3), ("fast_box_max", ctypes.c_double * 3),
+        ("fast_step_min", ctypes.c_int64), ("fast_step_max", ctypes.c_int64),
+        ("fast_tolerance", ctypes.c_double),
     ]
 
 
@@ -133,10 +136,11 @@ def _check(status: int, handle) -> None:
 # ------------------------------------------------------------------ ABI-named functions
 def rad_create(dirs, omega, dt: float, t0: float = 0.0, scale: float = 0.0,
                state_dtype: int = RAD_F32, flags: int = 0, device: int = 0, n_regions: int = 0,
-               window=None, nyquist: float = 0.0, form_factor=None) -> int:
+               window=None, nyquist: float = 0.0, form_factor=None, fast=None) -> int:
     """-> opaque handle (int).  dirs [D,3], omega [W]: HOST fp64 (copied by the library).
     window: None or (type name | code, origin[3], extent[3]).
-    form_factor: None or (type name | code, size[3] in metres)."""
+    form_factor: None or (type name | code, size[3] in metres).
+    fast (with RAD_FLAG_FAST_GRIDDED): (box_min[3], box_max[3], step_min, step_max, tolerance)."""
     dirs = np.ascontiguousarray(dirs, dtype=np.float64).reshape(-1, 3)
     omega = np.ascontiguousarray(omega, dtype=np.float64).reshape(-1)
     cfg = rad_config(ctypes.sizeof(rad_config), device, dirs.shape[0], omega.shape[0],
@@ -152,6 +156,11 @@ def rad_create(dirs, omega, dt: float, t0: float = 0.0, scale: float = 0.0,
         kind, size = form_factor
         cfg.form_factor_type = FORM_FACTOR_TYPES[kind] if isinstance(kind, str) else int(kind)
         cfg.form_factor_size = (ctypes.c_double * 3)(*[float(x) for x in size])
+    if fast is not None:
+        bmin, bmax, smin, smax, tol = fast
+        cfg.fast_box_min = (ctypes.c_double * 3)(*[float(x) for x in bmin])
+        cfg.fast_box_max = (ctypes.c_double * 3)(*[float(x) for x in bmax])
+        cfg.fast_step_min, cfg.fast_step_max, cfg.fast_tolerance = int(smin), int(smax), float(tol)
     h = ctypes.c_void_p()
     _check(load().rad_create(ctypes.byref(cfg), ctypes.byref(h)), None)
     return h.value
@@ -252,7 +261,7 @@ class Detector:
     pinned torch CPU tensors (host path, copies inside the library)."""
 
     def __init__(self, dirs, omega, dt, t0=0.0, scale=0.0, state_dtype=np.float32, flags=0, device=0,
-                 n_regions=0, window=None, nyquist=0.0, form_factor=None):
+                 n_regions=0, window=None, nyquist=0.0, form_factor=None, fast=None):
         self.D = int(np.asarray(dirs).reshape(-1, 3).shape[0])
         self.W = int(np.asarray(omega).reshape(-1).shape[0])
         self.R = max(1, int(n_regions))
@@ -260,7 +269,7 @@ class Detector:
         code = {np.dtype(np.float32): RAD_F32, np.dtype(np.float64): RAD_F64}[self.np_dtype]
         self.device = device
         self.handle = rad_create(dirs, omega, dt, t0, scale, code, flags, device, n_regions, window, nyquist,
-                                 form_factor)
+                                 form_factor, fast)
 
     def _shape(self, *tail):
         return ((self.R,) if self.R > 1 else ()) + (self.D, self.W) + tail

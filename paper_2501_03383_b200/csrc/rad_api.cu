@@ -50,6 +50,8 @@ void free_all(Handle &h)
 {
     cudaFree(h.dirs_d); cudaFree(h.basis_d); cudaFree(h.F_d); cudaFree(h.Ff_d); cudaFree(h.fl_d);
     cudaFree(h.acc_d); cudaFree(h.partial_d); cudaFree(h.stage_d[0]); cudaFree(h.stage_d[1]);
+    cudaFree(h.Fg_d); cudaFree(h.Ffg_d); cudaFree(h.flg_d);
+    cudaFree(h.g_s0_d); cudaFree(h.g_corr_d); cudaFree(h.g_delta_d); cudaFree(h.g_master_d); cudaFree(h.g_oob_d);
     cudaFree(h.out_d); cudaFree(h.chunks_d); cudaFree(h.reg_cstart_d); cudaFree(h.omega_d); cudaFree(h.F2_d);
 
     if (h.chunks_h) cudaFreeHost(h.chunks_h);
@@ -284,6 +286,58 @@ rad_status build_tapered_table(Handle &h, long long n, int chunk, cudaStream_t s
     return RAD_OK;
 }
 
+// ---- fast gridded path (rad.h RAD_FLAG_FAST_GRIDDED; kernels in rad_gridded.cu) ----
+constexpr int kGridFoldEvery = 1;  // accumulate calls between folds of the fp32 delta grid into the fp64 master
+                                   // (rad_gridded.cu: more than one costs accuracy on dark bins; a fold is ~2 % of a call)
+
+void grid_params(const Handle &h, AccumParams &p)
+{
+    p.g_delta = h.g_delta_d; p.g_master = h.g_master_d; p.g_s0 = h.g_s0_d; p.g_corr = h.g_corr_d;
+    p.g_hs = h.g_hs; p.g_ihs = 1.0 / h.g_hs; p.g_M = h.g_M; p.g_jdiff = h.g_jdiff;
+    p.g_beta2 = (float)(h.g_beta * 1.4426950408889634);
+    p.g_oob = h.g_oob_d;
+}
+
+rad_status grid_fold(Handle &h, cudaStream_t s)
+{
+    if (h.g_pending == 0) return RAD_OK;
+    RAD_CUDA(&h, launch_grid_fold(h, s));
+    h.launches += 1;
+    h.g_pending = 0;
+    return RAD_OK;
+}
+
+// spread one step's particles onto the grids of all directions
+rad_status accumulate_gridded(Handle &h, int64_t step, int64_t n, const void *const st[10], cudaStream_t s)
+{
+    if (step < h.g_step_min || step > h.g_step_max)
+        return fail(&h, RAD_ERR_INVALID_ARG, "step_index outside [fast_step_min, fast_step_max] given at rad_create");
+    AccumParams p{};
+    for (int i = 0; i < 10; ++i) p.st[i] = st[i];
+    p.n_particles = n;
+    p.n_dir = h.D; p.n_omega = h.W; p.w_pad = h.w_pad;
+    p.dirs = h.dirs_d;
+    p.ts32 = (h.t0 + (double)step * h.dt) * h.f_unit * kTwo32;
+    p.dt = (float)h.dt;
+    p.win_type = h.win_type;
+    for (int c = 0; c < 3; ++c) { p.win_o[c] = h.win_o[c]; p.win_il[c] = h.win_il[c]; }
+    grid_params(h, p);
+    // direction groups whose delta rows stay L2 resident (~48 MB); the 40 B/particle are re-read per group
+    const int per = (int)std::max<long long>(1, (48LL << 20) / ((long long)h.g_M * (long long)sizeof(float2)));
+    for (int d0 = 0; d0 < h.D; d0 += per) {
+        p.dir0 = d0; p.dir1 = std::min(h.D, d0 + per);
+        RAD_CUDA(&h, launch_spread(h, p, h.state_f64, s));
+        h.launches += 1;
+    }
+    h.variant = "gridded";
+    h.g_acc_valid = false;
+    if (++h.g_pending >= kGridFoldEvery) return grid_fold(h, s);
+    return RAD_OK;
+}
+
+// A(n, w_j) := (1/Phi_j) sum_m g_m(n) exp(i w_j tau_m) into the accumulator (rad_spectrum / rad_amplitude)
+rad_status evaluate_gridded(Handle &h, cudaStream_t s);
+
 // st: DEVICE arrays.  region_off == NULL: particles [0, n) of the one detector; else n_regions+1
 // HOST offsets into arrays whose element 0 is particle `region_base` of the caller's numbering
 // and n = particles spanned by the regions.
@@ -292,6 +346,16 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
                              const int64_t *region_off = nullptr, long long region_base = 0,
                              int n_steps = 1, long long step_stride = 0)
 {
+    if (h.fast) {  // approximate fast path: one spreading pass per step
+        const size_t esz = h.state_f64 ? 8 : 4;
+        for (int t = 0; t < n_steps; ++t) {
+            const void *sub[10];
+            for (int i = 0; i < 10; ++i) sub[i] = (const char *)st[i] + (size_t)t * step_stride * esz;
+            rad_status st_ = accumulate_gridded(h, step + t, n, sub, s);
+            if (st_ != RAD_OK) return st_;
+        }
+        return RAD_OK;
+    }
     if (n_steps > 1 && (h.stream_nb || h.deterministic)) {
         // few-bin streaming kernel / deterministic workspace: one launch per step
         const size_t esz = h.state_f64 ? 8 : 4;
@@ -385,6 +449,32 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     return RAD_OK;
 }
 
+rad_status evaluate_gridded(Handle &h, cudaStream_t s)
+{
+    if (h.g_acc_valid) return RAD_OK;
+    rad_status st = grid_fold(h, s);
+    if (st != RAD_OK) return st;
+    RAD_CUDA(&h, cudaMemsetAsync(h.acc_d, 0, (size_t)h.D * h.w_pad * 4 * sizeof(double), s));
+    AccumParams p{};
+    p.n_particles = h.g_M;          // the "particles" of this sweep are the grid points
+    // Short chunks: consecutive grid points are consecutive in retarded time, so below the highest
+    // frequencies the fp32 partial sum of a chunk is COHERENT (large) and the bin's amplitude is what
+    // survives the cancellation between chunks -- the rounding of the partial sums must stay below that.
+    // (Measured on configs 2 and 3a with 4096-point chunks: a floor of 5e-7 of the peak amplitude,
+    // 8e-4 relative on bins at 1e-6 of the peak, whatever the kernel width; the error scales with the chunk.)
+    p.chunk = 8 * kBatch;
+    p.n_chunks = (h.g_M + p.chunk - 1) / p.chunk;
+    p.n_dir = h.D; p.n_omega = h.W; p.w_pad = h.w_pad;
+    p.n_ftiles = h.n_ftiles; p.n_wtiles = h.n_wtiles;
+    p.dirs = h.dirs_d; p.F = h.Fg_d; p.Ff = h.Ffg_d; p.fl = h.flg_d;   // tables in units of one grid step
+    p.acc = h.acc_d;
+    grid_params(h, p);
+    RAD_CUDA(&h, launch_eval_grid(h, p, s));
+    h.launches += 1;
+    h.g_acc_valid = true;
+    return RAD_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -402,7 +492,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         return fail(nullptr, RAD_ERR_INVALID_ARG, "dt must be finite and > 0; t0, scale finite; scale >= 0");
     if (cfg->state_dtype != RAD_F32 && cfg->state_dtype != RAD_F64)
         return fail(nullptr, RAD_ERR_INVALID_ARG, "state_dtype must be RAD_F32 or RAD_F64");
-    if (cfg->flags & ~(RAD_FLAG_DETERMINISTIC | RAD_FLAG_FORCE_GENERAL | RAD_FLAG_OVERLAP_STEPS))
+    if (cfg->flags & ~(RAD_FLAG_DETERMINISTIC | RAD_FLAG_FORCE_GENERAL | RAD_FLAG_OVERLAP_STEPS | RAD_FLAG_FAST_GRIDDED))
         return fail(nullptr, RAD_ERR_INVALID_ARG, "unknown flag bits");
     if (cfg->n_regions < 0) return fail(nullptr, RAD_ERR_INVALID_ARG, "n_regions must be >= 0");
     if (!std::isfinite(cfg->nyquist_factor) || cfg->nyquist_factor < 0.0)
@@ -424,6 +514,21 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         if (!std::isfinite(w) || !(w > 0.0) || (j > 0 && !(w > cfg->omega[j - 1])))
             return fail(nullptr, RAD_ERR_INVALID_ARG, "omega must be finite, > 0 and strictly increasing");
     }
+    const bool fast = (cfg->flags & RAD_FLAG_FAST_GRIDDED) != 0;
+    if (fast) {
+        for (int c = 0; c < 3; ++c)
+            if (!std::isfinite(cfg->fast_box_min[c]) || !std::isfinite(cfg->fast_box_max[c]) ||
+                cfg->fast_box_max[c] < cfg->fast_box_min[c])
+                return fail(nullptr, RAD_ERR_INVALID_ARG, "fast_box must be finite with min <= max");
+        if (cfg->fast_step_max < cfg->fast_step_min)
+            return fail(nullptr, RAD_ERR_INVALID_ARG, "fast_step_max < fast_step_min");
+        if (!std::isfinite(cfg->fast_tolerance) || cfg->fast_tolerance < 0.0 || cfg->fast_tolerance >= 1.0)
+            return fail(nullptr, RAD_ERR_INVALID_ARG, "fast_tolerance must be in [0, 1)");
+        if (cfg->n_regions > 1 || cfg->nyquist_factor > 0.0 || cfg->form_factor_type != RAD_FF_NONE ||
+            (cfg->flags & RAD_FLAG_DETERMINISTIC))
+            return fail(nullptr, RAD_ERR_UNSUPPORTED,
+                        "RAD_FLAG_FAST_GRIDDED: no regions, Nyquist limiter, form factor or deterministic mode");
+    }
     rad_handle *hh = new (std::nothrow) rad_handle();
     if (!hh) return fail(nullptr, RAD_ERR_ALLOC, "out of host memory");
     Handle &h = hh->h;
@@ -442,6 +547,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     h.state_f64 = cfg->state_dtype == RAD_F64;
     h.deterministic = (cfg->flags & RAD_FLAG_DETERMINISTIC) != 0;
     h.overlap = (cfg->flags & RAD_FLAG_OVERLAP_STEPS) != 0;
+    h.fast = fast;
 
     // directions: normalise in fp64 (Q8), build e1, e2 with e1 x e2 = n
     h.dirs_h.resize((size_t)h.D * 3);
@@ -482,11 +588,11 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     h.sdir[0] = recs[0]; h.sdir[1] = recs[h.D > 1 ? 1 : 0];
     choose_tile(h);
     // per-region detectors and the Nyquist limiter: bin-owner kernels only
-    h.stream_nb = (h.R > 1 || h.nyq_lim > 0.0) ? 0 : stream_shape(h.D, h.W, &h.stream_nd);
+    h.stream_nb = (h.R > 1 || h.nyq_lim > 0.0 || h.fast) ? 0 : stream_shape(h.D, h.W, &h.stream_nd);
     // uniform grid?  w_j = w_0 + j dw to fp64 rounding -> rotation-recurrence kernel (a2')
     h.uniform = false;
     double uni_dw = 0.0;
-    if (h.W >= 2 * h.strip && !(cfg->flags & RAD_FLAG_FORCE_GENERAL) && h.nyq_lim == 0.0) {
+    if (h.W >= 2 * h.strip && !(cfg->flags & RAD_FLAG_FORCE_GENERAL) && h.nyq_lim == 0.0 && !h.fast) {
         const double dw = (h.omega_h.back() - h.omega_h.front()) / (h.W - 1);
         bool uni = true;
         for (int j = 0; j < h.W && uni; ++j)
@@ -542,6 +648,85 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
             }
     }
 
+    // fast gridded path: kernel width from the tolerance, grid spacing h = pi / (2 w_max), per direction
+    // the retarded-time interval that the box and the step window can reach, 1 / Phi(w_j)
+    std::vector<double> g_s0;
+    std::vector<double2> g_corr;
+    std::vector<uint32_t> Fg;
+    std::vector<float> Ffg, flg;
+    if (h.fast) {
+        const double eps = cfg->fast_tolerance > 0.0 ? cfg->fast_tolerance : 1e-6;
+        int wd = (int)std::ceil(std::log10(1.0 / eps)) + 1;
+        wd = std::min(12, std::max(4, wd + (wd & 1)));
+        h.g_w = wd;
+        h.g_beta = 2.30 * wd;
+        const double h_tau = kPi / (2.0 * h.omega_h.back());
+        h.g_hs = h_tau * h.f_unit * kTwo32;
+        for (int c = 0; c < 3; ++c) { h.g_box_min[c] = cfg->fast_box_min[c]; h.g_box_max[c] = cfg->fast_box_max[c]; }
+        h.g_step_min = cfg->fast_step_min; h.g_step_max = cfg->fast_step_max;
+        const double t_lo = h.t0 + (double)h.g_step_min * h.dt, t_hi = h.t0 + (double)h.g_step_max * h.dt;
+        g_s0.resize(h.D);
+        long long M = 0;
+        for (int d = 0; d < h.D; ++d) {
+            double pmin = 0.0, pmax = 0.0;  // range of n.r over the box
+            for (int c = 0; c < 3; ++c) {
+                const double a = h.dirs_h[3 * d + c] * h.g_box_min[c], b = h.dirs_h[3 * d + c] * h.g_box_max[c];
+                pmin += std::min(a, b); pmax += std::max(a, b);
+            }
+            const double tau_lo = t_lo - pmax / kC, tau_hi = t_hi - pmin / kC;
+            g_s0[d] = std::floor(tau_lo / h_tau) - (0.5 * wd + 2.0);   // grid points sit at integer multiples of h
+            M = std::max(M, (long long)std::ceil((tau_hi - tau_lo) / h_tau) + wd + 8);
+        }
+        M = (M + 63) / 64 * 64;
+        if ((double)M * h.D * 24.0 > 64e9) {
+            delete hh;
+            return fail(nullptr, RAD_ERR_INVALID_ARG, "RAD_FLAG_FAST_GRIDDED: the box / window needs more than 64 GB of grid");
+        }
+        h.g_M = (int)M;
+        // frequency tables of the evaluation sweep: f_j in units of 1 / (h 2^32) (<= 2^30: h f_max = 1/4)
+        Fg.assign(h.w_pad, 0u); Ffg.assign(h.w_pad, 0.0f); flg.assign(h.w_pad, 0.0f);
+        for (int j = 0; j < h.W; ++j) {
+            const double fu = h.omega_h[j] / (2.0 * kPi) * h_tau * kTwo32;
+            const double Fi = std::nearbyint(fu);
+            Fg[j] = (uint32_t)Fi; Ffg[j] = (float)Fi; flg[j] = (float)(fu - Fi);
+        }
+        // Phi(w) = (wd/2) * integral_{-1}^{1} phi(x) cos(xi x) dx, xi = w h wd / 2; with x = sin(theta) the
+        // integrand exp(beta (cos(theta) - 1)) cos(xi sin(theta)) cos(theta) is smooth: trapezoid rule
+        g_corr.assign(h.w_pad, make_double2(0.0, 0.0));
+        // bins of whole frequency tiles with w h >= 2.5e-3 are evaluated from first differences of the grid
+        // (rad_kernels.cu, GRID staging): first such bin, rounded up to a tile boundary
+        {
+            const int tile = h.lw * h.strip;
+            int j_first = h.W;
+            for (int j = 0; j < h.W; ++j)
+                if (h.omega_h[j] * h_tau >= 2.5e-3) { j_first = j; break; }
+            h.g_jdiff = (j_first + tile - 1) / tile * tile;
+        }
+        const int nq = 4096;
+        for (int j = 0; j < h.W; ++j) {
+            const double xi = h.omega_h[j] * h_tau * 0.5 * wd;
+            double acc = 0.0;
+            for (int q = 0; q <= nq; ++q) {
+                const double th = -0.5 * kPi + kPi * q / nq;
+                const double f = std::exp(h.g_beta * (std::cos(th) - 1.0)) * std::cos(xi * std::sin(th)) * std::cos(th);
+                acc += (q == 0 || q == nq) ? 0.5 * f : f;
+            }
+            const double inv_phi = 1.0 / (0.5 * wd * acc * (kPi / nq));
+            // the evaluation sums first differences of the grid: divide by 1 - exp(i w h) =
+            // 2 sin^2(theta/2) - i sin(theta), theta = w h (no cancellation at small theta)
+            if (j >= h.g_jdiff) {
+                const double th = h.omega_h[j] * h_tau, sh = std::sin(0.5 * th);
+                const double re = 2.0 * sh * sh, im = -std::sin(th), n2 = re * re + im * im;
+                g_corr[j] = make_double2(inv_phi * re / n2, -inv_phi * im / n2);
+            } else {
+                g_corr[j] = make_double2(inv_phi, 0.0);
+            }
+            // phase_sincos_grid centres the turn on 0 (frac - 1/2): every term carries exp(-i pi) = -1
+            g_corr[j].x = -g_corr[j].x;
+            g_corr[j].y = -g_corr[j].y;
+        }
+    }
+
     cudaError_t e = cudaSetDevice(h.device);
     if (e != cudaSuccess) { delete hh; return cuda_fail(nullptr, e, "cudaSetDevice"); }
     cudaDeviceProp prop;
@@ -556,7 +741,15 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
               cudaMalloc(&h.fl_d, sizeof(float) * h.w_pad) == cudaSuccess &&
               cudaMalloc(&h.acc_d, acc_bytes) == cudaSuccess &&
               (h.nyq_lim == 0.0 || cudaMalloc(&h.omega_d, sizeof(double) * h.W) == cudaSuccess) &&
-              (h.F2_h.empty() || cudaMalloc(&h.F2_d, sizeof(float) * h.F2_h.size()) == cudaSuccess);
+              (h.F2_h.empty() || cudaMalloc(&h.F2_d, sizeof(float) * h.F2_h.size()) == cudaSuccess) &&
+              (!h.fast || (cudaMalloc(&h.g_s0_d, sizeof(double) * h.D) == cudaSuccess &&
+                           cudaMalloc(&h.g_corr_d, sizeof(double2) * h.w_pad) == cudaSuccess &&
+                           cudaMalloc(&h.Fg_d, sizeof(uint32_t) * h.w_pad) == cudaSuccess &&
+                           cudaMalloc(&h.Ffg_d, sizeof(float) * h.w_pad) == cudaSuccess &&
+                           cudaMalloc(&h.flg_d, sizeof(float) * h.w_pad) == cudaSuccess &&
+                           cudaMalloc(&h.g_delta_d, sizeof(float2) * (size_t)h.D * h.g_M) == cudaSuccess &&
+                           cudaMalloc(&h.g_master_d, sizeof(double2) * (size_t)h.D * h.g_M) == cudaSuccess &&
+                           cudaMalloc(&h.g_oob_d, sizeof(unsigned long long)) == cudaSuccess));
     if (!ok) {
         cudaGetLastError(); free_all(h); delete hh;
         return fail(nullptr, RAD_ERR_ALLOC, "cudaMalloc(tables/accumulator) failed");
@@ -567,6 +760,14 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
          cudaMemcpy(h.Ff_d, Ff.data(), sizeof(float) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemcpy(h.fl_d, fl.data(), sizeof(float) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
          cudaMemset(h.acc_d, 0, acc_bytes) == cudaSuccess &&
+         (!h.fast || (cudaMemcpy(h.g_s0_d, g_s0.data(), sizeof(double) * h.D, cudaMemcpyHostToDevice) == cudaSuccess &&
+                      cudaMemcpy(h.g_corr_d, g_corr.data(), sizeof(double2) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
+                      cudaMemcpy(h.Fg_d, Fg.data(), sizeof(uint32_t) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
+                      cudaMemcpy(h.Ffg_d, Ffg.data(), sizeof(float) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
+                      cudaMemcpy(h.flg_d, flg.data(), sizeof(float) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
+                      cudaMemset(h.g_delta_d, 0, sizeof(float2) * (size_t)h.D * h.g_M) == cudaSuccess &&
+                      cudaMemset(h.g_master_d, 0, sizeof(double2) * (size_t)h.D * h.g_M) == cudaSuccess &&
+                      cudaMemset(h.g_oob_d, 0, sizeof(unsigned long long)) == cudaSuccess)) &&
          (!h.F2_d || cudaMemcpy(h.F2_d, h.F2_h.data(), sizeof(float) * h.F2_h.size(), cudaMemcpyHostToDevice) == cudaSuccess) &&
          (!h.omega_d || cudaMemcpy(h.omega_d, h.omega_h.data(), sizeof(double) * h.W, cudaMemcpyHostToDevice) == cudaSuccess) &&
          cudaStreamCreateWithFlags(&h.copy_stream, cudaStreamNonBlocking) == cudaSuccess;
@@ -577,6 +778,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         e = cudaGetLastError(); free_all(h); delete hh;
         return cuda_fail(nullptr, e, "table upload / stream set-up");
     }
+    h.g_acc_valid = h.fast;  // an empty grid evaluates to the zeroed accumulator
     *out = hh;
     return RAD_OK;
 }
@@ -779,6 +981,18 @@ static rad_status deliver(Handle &h, double *out, int out_on_device, size_t byte
     if (!out) return fail(&h, RAD_ERR_INVALID_ARG, "out is NULL");
     if (out_on_device < RAD_OUT_HOST || out_on_device > RAD_OUT_HOST_ASYNC)
         return fail(&h, RAD_ERR_INVALID_ARG, "out_on_device must be RAD_OUT_HOST, RAD_OUT_DEVICE or RAD_OUT_HOST_ASYNC");
+    if (h.fast) {  // approximate fast path: the accumulator is evaluated from the retarded-time grids on demand
+        rad_status st_ = evaluate_gridded(h, s);
+        if (st_ != RAD_OK) return st_;
+        if (out_on_device == RAD_OUT_HOST) {  // the synchronous form also reports terms that missed the grid
+            unsigned long long lost = 0;
+            RAD_CUDA(&h, cudaMemcpyAsync(&lost, h.g_oob_d, sizeof(lost), cudaMemcpyDeviceToHost, s));
+            RAD_CUDA(&h, cudaStreamSynchronize(s));
+            if (lost)
+                return fail(&h, RAD_ERR_STATE, std::to_string(lost) + " (particle, direction) terms fell outside "
+                            "the fast_box / step window given at rad_create and were not deposited");
+        }
+    }
     if (out_on_device == RAD_OUT_DEVICE) {
         RAD_CUDA(&h, launch(h, out, s));
         h.launches += 1;
@@ -828,6 +1042,7 @@ rad_status rad_add_amplitude(rad_handle *hh, const double *amp_device, void *cud
     rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     if (!amp_device) return fail(&hh->h, RAD_ERR_INVALID_ARG, "amp_device is NULL");
+    if (hh->h.fast) return fail(&hh->h, RAD_ERR_UNSUPPORTED, "rad_add_amplitude on a RAD_FLAG_FAST_GRIDDED handle");
     RAD_CUDA(&hh->h, launch_add_amplitude(hh->h, amp_device, (cudaStream_t)cuda_stream));
     hh->h.launches += 1;
     return RAD_OK;
@@ -840,6 +1055,7 @@ rad_status rad_export_accumulator(rad_handle *hh, double *out_device, void *cuda
     if (st != RAD_OK) return st;
     Handle &h = hh->h;
     if (!out_device) return fail(&h, RAD_ERR_INVALID_ARG, "out_device is NULL");
+    if (h.fast) return fail(&h, RAD_ERR_UNSUPPORTED, "rad_export_accumulator on a RAD_FLAG_FAST_GRIDDED handle");
     // rows of W*4 doubles out of the padded [R*D][w_pad][4] accumulator; a memcpy keeps its full
     // stream dependencies under RAD_FLAG_OVERLAP_STEPS (it runs after every fold queued before)
     const size_t row = (size_t)h.W * 4 * sizeof(double);
@@ -854,6 +1070,7 @@ rad_status rad_import_accumulator(rad_handle *hh, const double *amp4_device, voi
     rad_status st = check_handle(hh, guard);
     if (st != RAD_OK) return st;
     if (!amp4_device) return fail(&hh->h, RAD_ERR_INVALID_ARG, "amp4_device is NULL");
+    if (hh->h.fast) return fail(&hh->h, RAD_ERR_UNSUPPORTED, "rad_import_accumulator on a RAD_FLAG_FAST_GRIDDED handle");
     RAD_CUDA(&hh->h, launch_import_accumulator(hh->h, amp4_device, (cudaStream_t)cuda_stream));
     hh->h.launches += 1;
     return RAD_OK;
@@ -880,6 +1097,14 @@ rad_status rad_reset(rad_handle *hh, void *cuda_stream)
     Handle &h = hh->h;
     RAD_CUDA(&h, cudaMemsetAsync(h.acc_d, 0, (size_t)h.R * h.D * h.w_pad * 4 * sizeof(double),
                                  (cudaStream_t)cuda_stream));
+    if (h.fast) {
+        cudaStream_t s = (cudaStream_t)cuda_stream;
+        RAD_CUDA(&h, cudaMemsetAsync(h.g_delta_d, 0, sizeof(float2) * (size_t)h.D * h.g_M, s));
+        RAD_CUDA(&h, cudaMemsetAsync(h.g_master_d, 0, sizeof(double2) * (size_t)h.D * h.g_M, s));
+        RAD_CUDA(&h, cudaMemsetAsync(h.g_oob_d, 0, sizeof(unsigned long long), s));
+        h.g_pending = 0;
+        h.g_acc_valid = true;
+    }
     return RAD_OK;
 }
 

@@ -109,6 +109,25 @@ __device__ __forceinline__ void phase_sincos(uint32_t F, float Ff, float fl, uin
     __sincosf(fmaf(v, kTwoPi, q), &sn, &cs);
 }
 
+// exp(i 2 pi f tau) for the evaluation sweep of the fast gridded path.  There the terms sit on a
+// regular grid and carry the coherent low-frequency content of the signal, so a SYSTEMATIC error of
+// the sin/cos at the phases a bin visits periodically (w_max visits the quarter turns: h w_max =
+// pi / 2) leaks that content into the bin.  Hence the argument stays in TURNS and exact:
+// v = frac - 1/2 in [-1/2, 1/2) (exact), t = v + phi_j T' / 2^32 (the small fraction term), and
+// sin.approx / cos.approx see x = t * C with C = 0x40c90fdc, the fp32 just above 2 pi for which
+// C * 0.15915494f = 1 + 6.3e-8: their own first instruction, x * 0.15915494f rounded towards zero,
+// then returns t itself (exactly for every t whose mantissa is below 1.88, one ulp high otherwise),
+// i.e. MUFU.SIN/COS are fed the exact turn -- 0, 1/4, 1/2 give exact 0 and 1.  The centring shifts
+// every phase by half a turn: the caller's per-bin factor (g_corr) carries the -1.
+__device__ __forceinline__ void phase_sincos_grid(uint32_t F, float fl, uint32_t T, float sf_turns,
+                                                  float &sn, float &cs)
+{
+    const uint32_t u = F * T;
+    const float v = __uint_as_float(0x3f800000u | (u >> 9)) - 1.5f;
+    const float t = fmaf(fl, sf_turns, v);
+    __sincosf(t * __uint_as_float(0x40c90fdcu), &sn, &cs);
+}
+
 // The same exp(i 2 pi f tau) WITHOUT the XU pipe: the reduced phase goes through FMA-pipe
 // polynomials.  t = frac + q/(2 pi) turns; r = t - rint(2t)/2 in [-1/4, 1/4]; sin(2 pi r) and
 // cos(2 pi r) by near-minimax odd/even polynomials (fp32 abs. error 1.9e-7 / 2.9e-7, below

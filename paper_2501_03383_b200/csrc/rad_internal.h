@@ -83,6 +83,19 @@ struct AccumParams {
     float sFf[16], sfl[16];
     float sF2[16];         // form factor: F^2 of bin b = d * WB + j
     DirRec sdir[2];
+    // fast gridded path (rad_gridded.cu; rad.h RAD_FLAG_FAST_GRIDDED): per direction a uniform grid in
+    // retarded time, point m at tau = (g_s0[dir] + m) h, h = g_hs in s32 units (s32 = tau f_unit 2^32)
+    float2 *g_delta;             // [D][g_M] fp32 (A1, A2) deposits since the last fold
+    const double2 *g_master;     // [D][g_M] fp64 grid (evaluation reads it)
+    const double *g_s0;          // [D] index of grid point 0 in units of h: tau_m = (g_s0[n] + m) h (integers)
+    const double2 *g_corr;       // [w_pad] complex 1 / (Phi(w_j) (1 - exp(i w_j h))): deconvolution of the
+                                 // spreading kernel and of the first differences the evaluation sums
+    double g_hs, g_ihs;          // grid spacing in s32 units and its inverse
+    int g_M;                     // grid points per direction (even)
+    int g_jdiff;                 // evaluation: frequency tiles starting at bins >= g_jdiff sum first differences
+    float g_beta2;               // ES kernel exponent beta * log2(e)
+    unsigned long long *g_oob;   // terms that fell outside the grid
+    int dir0, dir1;              // spreading: directions [dir0, dir1) of this launch
     // uniform-grid variant only: LW*(f_1 - f_0)/f_unit = rot_G + rot_gl (integer + fraction)
     uint32_t rot_G;
     float rot_Gf, rot_gl;
@@ -114,6 +127,9 @@ cudaError_t launch_accumulate_stream(const Handle &h, const AccumParams &p, bool
 int stream_tile_particles(int nb, bool state_f64);
 int stream_blocks_per_sm(int nb);
 int stream_shape(int D, int W, int *nd);
+cudaError_t launch_spread(const Handle &h, const AccumParams &p, bool state_f64, cudaStream_t s);
+cudaError_t launch_grid_fold(const Handle &h, cudaStream_t s);
+cudaError_t launch_eval_grid(const Handle &h, const AccumParams &p, cudaStream_t s);
 cudaError_t launch_spectrum(const Handle &h, double *out_dev, cudaStream_t s);
 cudaError_t launch_amplitude(const Handle &h, double *out_dev, cudaStream_t s);
 cudaError_t launch_add_amplitude(const Handle &h, const double *amp_dev, cudaStream_t s);
@@ -174,6 +190,22 @@ struct Handle {
     int *reg_cstart_h = nullptr, *reg_cstart_d = nullptr; // [R+1] first chunk of each region
     size_t reg_cap = 0;
     cudaEvent_t reg_uploaded = nullptr;
+    // fast gridded path (RAD_FLAG_FAST_GRIDDED)
+    bool fast = false;
+    int g_w = 0, g_M = 0;            // kernel width (grid points, even), grid points per direction
+    int g_jdiff = 0;                 // first bin of the frequency tiles evaluated from first differences
+    double g_hs = 0, g_beta = 0;     // grid spacing in s32 units, ES kernel parameter
+    double g_box_min[3] = {0, 0, 0}, g_box_max[3] = {0, 0, 0};
+    long long g_step_min = 0, g_step_max = 0;
+    double *g_s0_d = nullptr;
+    double2 *g_corr_d = nullptr;
+    uint32_t *Fg_d = nullptr;        // frequency tables of the evaluation sweep, in units of 1 / (h 2^32)
+    float *Ffg_d = nullptr, *flg_d = nullptr;
+    float2 *g_delta_d = nullptr;
+    double2 *g_master_d = nullptr;
+    unsigned long long *g_oob_d = nullptr;
+    int g_pending = 0;               // accumulate calls since the last fold of delta into master
+    bool g_acc_valid = false;        // acc_d holds the evaluation of the current grid
     double *out_d = nullptr;         // scratch for HOST-destination results
     size_t out_bytes = 0;
     int64_t launches = 0;

@@ -33,11 +33,28 @@ using namespace dev;
 
 // a3: fold one thread's fp32 partials into the fp64 accumulator (or the deterministic
 // per-chunk workspace).
-template <int S, int LW>
+template <int S, int LW, bool GRID = false>
 __device__ __forceinline__ void fold(const AccumParams &P, const float (&acc)[S][4], int dir,
                                      int jbase, int ci, int region)
 {
     if (dir >= P.n_dir) return;
+    if (GRID) {  // fast gridded path: the partial is divided by the spreading kernel's transform
+        double *dst = P.acc + (size_t)dir * (size_t)P.w_pad * 4;
+#pragma unroll
+        for (int i = 0; i < S; ++i) {
+            const int j = jbase + i * LW;
+            if (j < P.n_omega) {
+                // complex factor 1 / (Phi_j (1 - exp(i w_j h))): kernel transform and first differences
+                const double2 c = __ldg(P.g_corr + j);
+                const double p0 = acc[i][0], p1 = acc[i][1], p2 = acc[i][2], p3 = acc[i][3];
+                atomicAdd(dst + (size_t)j * 4 + 0, c.x * p0 - c.y * p1);
+                atomicAdd(dst + (size_t)j * 4 + 1, c.x * p1 + c.y * p0);
+                atomicAdd(dst + (size_t)j * 4 + 2, c.x * p2 - c.y * p3);
+                atomicAdd(dst + (size_t)j * 4 + 3, c.x * p3 + c.y * p2);
+            }
+        }
+        return;
+    }
     if (P.partial) {
         double *dst = P.partial + ((size_t)ci * P.n_dir + dir) * (size_t)P.w_pad * 4;
 #pragma unroll
@@ -98,9 +115,13 @@ __device__ __forceinline__ bool decode_task(const AccumParams &P, int warp, int 
 // FF: macro-particle form factor (rad.h, reading FF1) -- every update's (cos, sin) is scaled by
 // g = sqrt(w + (w^2 - w) F^2): F^2 of the thread's S bins in registers, (w, w^2 - w) of the batch's
 // particles in shared memory; one FFMA + MUFU.SQRT + 2 FMUL more per update.
-template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ, bool FF>
+// GRID: evaluation of the fast gridded path (rad.h RAD_FLAG_FAST_GRIDDED) -- the "particles" are the
+// points of the per-direction retarded-time grids: point m of direction n has phase s32 = g_s0[n] +
+// m g_hs and amplitude g_master[n][m]; the sweep and the phase arithmetic are those of the general grid.
+template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ, bool FF, bool GRID = false>
 __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
 {
+    static_assert(!GRID || (!UNI && !NYQ && !FF), "grid evaluation runs the plain general-grid sweep");
     static_assert(!(UNI && NYQ), "the limiter runs on the general-grid kernel");
     constexpr int DPW = 32 / LW;
     constexpr int NC = UNI ? 1 : S;  // per-thread frequency constants held in registers
@@ -146,7 +167,42 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
     float2 *ws = s_w[FF ? warp : 0];
 
     for (long long kb = k0; kb < k1; kb += kBatch) {
-        {  // a1: stage
+        if (GRID) {  // stage grid point m = kb + lane for the warp's directions
+            // Phase unit of the evaluation = one grid step (frequency tables built with f_unit' =
+            // 1 / (h 2^32), rad_api.cu): tau_m / h = g_s0[n] + m is an INTEGER, so the integer phase
+            // F'_j * T mod 2^32 is the whole phase and no fp32 term depends on the position within a
+            // period of f_max.  (With the direct path's unit the fractional part of tau f_max repeats
+            // every 4 grid points; its fp32 rounding then modulates the coherent low-frequency content
+            // of the grid with exactly the period of w_max and leaks 5e-7 of the PEAK into the top bin.)
+            const long long m = kb + lane;
+#pragma unroll(DPW > 2 ? 1 : DPW)
+            for (int dd = 0; dd < DPW; ++dd) {
+                const int dir = min(dg * DPW + dd, P.n_dir - 1);
+                const double t_units = __ldg(P.g_s0 + dir) + (double)m;   // exact integer
+                // Frequency tiles from bin g_jdiff on sum FIRST DIFFERENCES of the grid, g_m - g_(m-1) (fp64):
+                // sum_m (g_m - g_(m-1)) z^m = (1 - z) sum_m g_m z^m, undone per bin at fold time (g_corr).
+                // The grid is dominated by the coherent low-frequency part of the signal (all deposits of
+                // one sign); the differences are not, so the systematic part of the fp32 sin/cos error (a
+                // fixed function of the phase, sampled on a regular grid) has no coherent content left to
+                // leak into the dark high-frequency bins (measured without: a white floor of 1e-7 of the
+                // peak amplitude, 3e-4 ... 8e-4 on bins at 1e-6 of the peak).  Dividing by 1 - z amplifies
+                // the rounding noise by 1 / (w h), so the low-frequency tiles (w h < 2.5e-3), where the
+                // signal itself is the coherent peak, sum the grid as it is.
+                double2 g = make_double2(0.0, 0.0);
+                if (m < k1) {
+                    const double2 *row = P.g_master + (size_t)dir * P.g_M;
+                    g = __ldg(row + m);
+                    if (m > 0 && ft * (LW * S) >= P.g_jdiff) {
+                        const double2 gp = __ldg(row + m - 1);
+                        g.x -= gp.x;
+                        g.y -= gp.y;
+                    }
+                }
+                rec[lane * DPW + dd] = make_float4(__uint_as_float((uint32_t)__double2loint(t_units + kMagic)), 0.0f,
+                                                   to_f32(g.x), to_f32(g.y));
+                sfs[lane * DPW + dd] = to_f32(t_units) * 2.3283064365386963e-10f;   // T' / 2^32 (turns per unit fraction)
+            }
+        } else {  // a1: stage
             const long long k = kb + lane;
             const Particle p = load_particle<ST, true>(P, k, k < k1, FF);
             if (FF) ws[lane] = make_float2(p.w, p.ww);
@@ -216,7 +272,9 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
 #pragma unroll
                 for (int i = 0; i < S; ++i) {
                     float sn, cs;
-                    if (i >= S - n_poly)
+                    if (GRID)
+                        phase_sincos_grid(F[i % NC], fl[i % NC], T, sf, sn, cs);
+                    else if (i >= S - n_poly)
                         phase_sincos_poly(F[i % NC], Ff[i % NC], fl[i % NC], T, r4.y, sf, sn, cs);
                     else
                         phase_sincos(F[i % NC], Ff[i % NC], fl[i % NC], T, r4.y, sf, sn, cs);
@@ -251,7 +309,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
         __syncwarp();
     }
     pdl_wait();  // the accumulator (and the deterministic workspace) belong to earlier work until here
-    fold<S, LW>(P, acc, dg * DPW + ld, jbase, ci, region);
+    fold<S, LW, GRID>(P, acc, dg * DPW + ld, jbase, ci, region);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -283,6 +341,19 @@ template <typename ST, bool UNI, bool NYQ>
 static cudaError_t dispatch(const Handle &h, const AccumParams &p, cudaStream_t s)
 {
     return p.F2 ? dispatch_lw<ST, UNI, NYQ, true>(h, p, s) : dispatch_lw<ST, UNI, NYQ, false>(h, p, s);
+}
+
+// fast gridded path: A(n, w_j) = (1/Phi_j) sum_m g_m(n) exp(i w_j tau_m) over the grid points
+cudaError_t launch_eval_grid(const Handle &h, const AccumParams &p, cudaStream_t s)
+{
+    const long long n_tasks = (long long)p.n_wtiles * p.n_chunks;
+    const unsigned grid = (unsigned)((n_tasks + kWarpsPerBlock - 1) / kWarpsPerBlock);
+    switch (h.lw) {
+        case 32: return launch_kernel(rad_accum<float, 32, kStrip, kMinBlocks, false, false, false, true>, dim3(grid), dim3(kThreads), 0, s, h.overlap, p);
+        case 16: return launch_kernel(rad_accum<float, 16, kStrip, kMinBlocks, false, false, false, true>, dim3(grid), dim3(kThreads), 0, s, h.overlap, p);
+        case 8: return launch_kernel(rad_accum<float, 8, kStrip, kMinBlocks, false, false, false, true>, dim3(grid), dim3(kThreads), 0, s, h.overlap, p);
+        default: return launch_kernel(rad_accum<float, 4, kStrip, kMinBlocks, false, false, false, true>, dim3(grid), dim3(kThreads), 0, s, h.overlap, p);
+    }
 }
 
 cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_f64,
