@@ -186,6 +186,8 @@ struct Handle {
     long long reg_stride = 0;
     long long tap_n = -1;                 // tapered plain-call table on the device: its n and chunk
     int tap_chunk = 0;
+    int stp_steps = 0, stp_chunk = 0;     // multi-step table on the device (reg_chunk == -2): its shape
+    long long stp_n = -1, stp_stride = 0;
     ChunkRec *chunks_h = nullptr, *chunks_d = nullptr;   // [reg_cap]
     int *reg_cstart_h = nullptr, *reg_cstart_d = nullptr; // [R+1] first chunk of each region
     size_t reg_cap = 0;

@@ -405,11 +405,12 @@ def test_accumulate_steps_cfg0_all_128_steps_in_one_launch(oracle_mod):
 
 
 @pytest.mark.parametrize("cfg,n,T,pad,flags", [("3c", 1000, 5, 24, 0), ("1", 4100, 3, 0, 0), ("3d", 333, 4, 3, 0),
-                                                ("3c", 500, 3, 0, 1), ("4b", 3000, 3, 8, 0)])
+                                                ("3c", 500, 3, 0, 1), ("4b", 3000, 3, 8, 0),
+                                                ("3c", 40, 50, 8, 0), ("0", 7, 100, 1, 0), ("3b", 33, 64, 0, 0)])
 def test_accumulate_steps_matches_oracle_and_per_step_calls(oracle_mod, cfg, n, T, pad, flags):
     """Late first step index, row stride > n_particles (padding rows hold NaN and must not be
     read), ragged chunk tails; deterministic handles and few-bin detectors take the per-step
-    fallback inside the library."""
+    fallback inside the library.  Also steps with very few particles (7, 33, 40) over many steps."""
     from paper_2501_03383_b200 import binding
     w = wl.make_workload(cfg)
     first = 700 if w.n_steps > 800 else 1
