@@ -253,13 +253,16 @@ def alu_peaks(device, sm_mhz_hint):
         "mufu_per_clk_sm": g("mufu_ex2"), "sin_per_clk_sm": g("mufu_sin"),
         "sincos_pairs_per_clk_sm": g("sincos_pairs"), "ffma_per_clk_sm": g("ffma"),
         "ffma_imm_per_clk_sm": g("ffma_imm"), "ffma2_instr_per_clk_sm": g("ffma2_instr"),
-        "ffma2_fma_per_clk_sm": 2.0 * g("ffma2_instr"), "dfma_per_clk_sm": g("dfma"),
+        "ffma2_fma_per_clk_sm": 2.0 * g("ffma2_instr"), "ffma_var_per_clk_sm": g("ffma_var"),
+        "ffma2_var_fma_per_clk_sm": 2.0 * g("ffma2_var_instr"), "ffma2_bcast_fma_per_clk_sm": 2.0 * g("ffma2_bcast_instr"),
+        "dfma_per_clk_sm": g("dfma"),
         "f2f_f32_from_f64_per_clk_sm": g("f2f_f32_from_f64"), "f2f_f64_from_f32_per_clk_sm": g("f2f_f64_from_f32"),
         "imad_per_clk_sm": g("imad"),
         "sincos_pairs_gops": res["sincos_pairs"]["gops"], "ffma_gops": res["ffma"]["gops"],
         "sm_mhz": sm_mhz_hint,
-        "how": "librad_ubench.so (csrc/rad_ubench.cu): 8 independent chains per thread, 4 x 256 threads per SM; "
-               "per_clk_sm from clock64() inside the kernel, gops from CUDA events",
+        "how": "librad_ubench.so (csrc/rad_ubench.cu): 8 independent chains per thread, loop unrolled 4x, 4 x 256 threads "
+               "per SM; per_clk_sm from clock64() inside the kernel, gops from CUDA events; ffma / ffma2: two loop-invariant "
+               "operands (reuse cache), *_var / *_bcast: three different changing registers per instruction",
     }
 
 
@@ -392,6 +395,11 @@ def measure(cfg, K, W, args, ctx, headline):
             peak_m = n_sm * measured * sm_max * 1e6 / 1e9
             roofline.update({"peak_measured_pipe": peak_m, "frac_of_measured_pipe": achieved / peak_m,
                              "peak_measured_how": f"{n_sm} SMs x {measured:.3f} updates/clk/SM (alu_peaks) x {sm_max:.0f} MHz"})
+        if variant == "uniform" and peaks_alu and peaks_alu.get("ffma_var_per_clk_sm"):
+            # the sweep's FMAs read three different registers each: what the register file feeds the
+            # FMA pipe without operand reuse (alu_peaks ffma_var) is the rate the kernel actually sits on
+            peak_v = n_sm * peaks_alu["ffma_var_per_clk_sm"] / FP32_PER_UPDATE_UNIFORM * sm_max * 1e6 / 1e9
+            roofline.update({"peak_measured_no_operand_reuse": peak_v, "frac_of_measured_no_operand_reuse": achieved / peak_v})
         if clocks.get("sm_mhz"):
             roofline["frac_at_sampled_clock"] = roofline["frac"] * sm_max / clocks["sm_mhz"]
     roofline.update({"kernel": f"rad_accum_{variant}", "kernel_ms": kernel_ms,

@@ -91,22 +91,6 @@ __device__ __forceinline__ bool elect_one()
     return pred != 0;
 }
 
-// two fp32 in one 64-bit register pair, for fma.rn.f32x2
-__device__ __forceinline__ unsigned long long pack2(float lo, float hi)
-{
-    unsigned long long r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void unpack2(unsigned long long v, float &lo, float &hi)
-{
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ void fma2(unsigned long long &acc, unsigned long long a, unsigned long long b)
-{
-    asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc) : "l"(a), "l"(b));
-}
-
 template <typename ST, bool WIN>
 __device__ __forceinline__ Particle make_particle(ST rx, ST ry, ST rz, ST bx, ST by, ST bz, ST dx,
                                                   ST dy, ST dz, ST w, const AccumParams &P)

@@ -13,6 +13,11 @@
 // The roofline denominators derived from them:
 //   general grid   R_gen = sincos pairs/clk/SM (kind SINCOS) x SMs x clock      [nominal 8]
 //   uniform grid   R_lin = FFMA/clk/SM (kind FFMA) / 8 x SMs x clock            [nominal 16]
+// Kinds FFMA / FFMA2 keep two of their three operands loop-invariant (operand-reuse cache hits);
+// FFMA_VAR / FFMA2_VAR / FFMA2_BCAST read three DIFFERENT, changing registers per instruction and
+// measure what the register file feeds the FMA pipe without reuse (about 2 register reads per lane
+// per clock: 75 FFMA, 85 packed FMA per clock per SM) -- the regime of the uniform-grid sweep, whose
+// rotations and accumulates have few repeated operands.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -34,7 +39,10 @@ enum Kind {
     K_F2F_64_32 = 7, // cvt.rn.f32.f64 (+ FADD + DADD to keep the chain alive)
     K_F2F_32_64 = 8, // cvt.f64.f32 (+ DADD)
     K_IMAD = 9,      // mad.lo.u32
-    K_COUNT = 10
+    K_FFMA2_VAR = 10,   // fma.rn.f32x2 whose three operands are all different, changing registers: INSTRUCTIONS
+    K_FFMA2_BCAST = 11, // fma.rn.f32x2 with one operand a broadcast scalar (SASS Rn.F32), as the uniform-grid sweep issues it
+    K_FFMA_VAR = 12,    // fma.rn.f32 whose three operands are all different, changing registers
+    K_COUNT = 13
 };
 
 template <int KIND>
@@ -57,7 +65,9 @@ __global__ void __launch_bounds__(kThreads) pipe_kernel(float *out, float a, flo
     const unsigned long long a2 = ((unsigned long long)__float_as_uint(a) << 32) | __float_as_uint(a);
     const unsigned long long b2 = ((unsigned long long)__float_as_uint(b) << 32) | __float_as_uint(b);
     const long long t0 = clock64();
-#pragma unroll 1
+    // unrolled 4x: with one 8-operation pass per trip the loop's own IADD3 / ISETP / BRA take 3 of 11 issue
+    // slots and cap every one-instruction kind at 93 per clock per SM (round-2 figures: FFMA 85.8)
+#pragma unroll 4
     for (int it = 0; it < kIters; ++it) {
 #pragma unroll
         for (int i = 0; i < kChains; ++i) {
@@ -84,7 +94,16 @@ __global__ void __launch_bounds__(kThreads) pipe_kernel(float *out, float a, flo
                 asm volatile("cvt.f64.f32 %0, %1;" : "=d"(d) : "f"(x[i]));
                 z[i] += d;
             }
-            if (KIND == K_IMAD) w[i] = w[i] * 0x9E3779B9u + 12345u;
+            if (KIND == K_IMAD) asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(w[i]) : "r"(__float_as_uint(a)), "r"(__float_as_uint(b)));
+            if (KIND == K_FFMA2_VAR)
+                asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(y[i]) : "l"(y[(i + 3) & 7]), "l"(y[(i + 5) & 7]));
+            if (KIND == K_FFMA2_BCAST) {
+                unsigned long long bc;
+                asm volatile("mov.b64 %0, {%1, %1};" : "=l"(bc) : "f"(x[(i + 1) & 7]));
+                asm volatile("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(y[i]) : "l"(bc), "l"(y[(i + 5) & 7]));
+            }
+            if (KIND == K_FFMA_VAR)
+                asm volatile("fma.rn.f32 %0, %1, %2, %0;" : "+f"(x[i]) : "f"(x[(i + 3) & 7]), "f"(x[(i + 5) & 7]));
         }
     }
     const long long t1 = clock64();
@@ -160,7 +179,8 @@ __attribute__((visibility("default"))) int rad_ubench_kinds(void) { return K_COU
 __attribute__((visibility("default"))) const char *rad_ubench_name(int kind)
 {
     static const char *names[K_COUNT] = {"ffma", "ffma_imm", "ffma2_instr", "mufu_sin", "sincos_pairs",
-                                         "mufu_ex2", "dfma", "f2f_f32_from_f64", "f2f_f64_from_f32", "imad"};
+                                         "mufu_ex2", "dfma", "f2f_f32_from_f64", "f2f_f64_from_f32", "imad",
+                                         "ffma2_var_instr", "ffma2_bcast_instr", "ffma_var"};
     return kind >= 0 && kind < K_COUNT ? names[kind] : "?";
 }
 
@@ -186,6 +206,9 @@ __attribute__((visibility("default"))) int rad_ubench_run(int device, int kind, 
         case K_F2F_64_32: return run_kind<K_F2F_64_32>(n_sm, blocks_per_sm, reps, per_clk_sm, gops);
         case K_F2F_32_64: return run_kind<K_F2F_32_64>(n_sm, blocks_per_sm, reps, per_clk_sm, gops);
         case K_IMAD: return run_kind<K_IMAD>(n_sm, blocks_per_sm, reps, per_clk_sm, gops);
+        case K_FFMA2_VAR: return run_kind<K_FFMA2_VAR>(n_sm, blocks_per_sm, reps, per_clk_sm, gops);
+        case K_FFMA2_BCAST: return run_kind<K_FFMA2_BCAST>(n_sm, blocks_per_sm, reps, per_clk_sm, gops);
+        case K_FFMA_VAR: return run_kind<K_FFMA_VAR>(n_sm, blocks_per_sm, reps, per_clk_sm, gops);
     }
     return 1;
 }
