@@ -124,12 +124,18 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
     static_assert(!GRID || (!UNI && !NYQ && !FF), "grid evaluation runs the plain general-grid sweep");
     static_assert(!(UNI && NYQ), "the limiter runs on the general-grid kernel");
     constexpr int DPW = 32 / LW;
+    // Shared-memory records are direction-major, rec[direction of the warp][particle of the batch], rows padded
+    // by one record: the staging lanes store 16-byte records at consecutive addresses and the sweep's
+    // DPW different broadcast reads (one per direction) fall into different banks.  (Particle-major
+    // rec[particle][direction] made the stores of a warp 64 or 128 bytes apart: 4- / 8-way bank
+    // conflicts, 1.26e8 conflict cycles per launch on config 3d, profiles/r2_ncu_rad_accum_general_cfg3d.md.)
+    constexpr int PITCH = kBatch + (DPW > 1 ? 1 : 0);
     constexpr int NC = UNI ? 1 : S;  // per-thread frequency constants held in registers
     constexpr int MID = S / 2 - 1;   // anchor bin of the uniform-grid chain
-    __shared__ float4 s_rec[kWarpsPerBlock][kBatch * DPW];
-    __shared__ float s_sf[kWarpsPerBlock][kBatch * DPW];
-    __shared__ float2 s_rot[UNI ? kWarpsPerBlock : 1][UNI ? kBatch * DPW : 1];
-    __shared__ int s_jc[NYQ ? kWarpsPerBlock : 1][NYQ ? kBatch * DPW : 1];
+    __shared__ float4 s_rec[kWarpsPerBlock][PITCH * DPW];
+    __shared__ float s_sf[kWarpsPerBlock][PITCH * DPW];
+    __shared__ float2 s_rot[UNI ? kWarpsPerBlock : 1][UNI ? PITCH * DPW : 1];
+    __shared__ int s_jc[NYQ ? kWarpsPerBlock : 1][NYQ ? PITCH * DPW : 1];
     __shared__ float2 s_w[FF ? kWarpsPerBlock : 1][FF ? kBatch : 1];
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -198,9 +204,9 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                         g.y -= gp.y;
                     }
                 }
-                rec[lane * DPW + dd] = make_float4(__uint_as_float((uint32_t)__double2loint(t_units + kMagic)), 0.0f,
+                rec[dd * PITCH + lane] = make_float4(__uint_as_float((uint32_t)__double2loint(t_units + kMagic)), 0.0f,
                                                    to_f32(g.x), to_f32(g.y));
-                sfs[lane * DPW + dd] = to_f32(t_units) * 2.3283064365386963e-10f;   // T' / 2^32 (turns per unit fraction)
+                sfs[dd * PITCH + lane] = to_f32(t_units) * 2.3283064365386963e-10f;   // T' / 2^32 (turns per unit fraction)
             }
         } else {  // a1: stage
             const long long k = kb + lane;
@@ -214,13 +220,13 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 uint32_t T;
                 double d64;
                 stage_record(p, P.dirs[dir], ts32, r4, sf, &T, &d64);
-                rec[lane * DPW + dd] = r4;
-                sfs[lane * DPW + dd] = sf;
-                if (NYQ) jcs[lane * DPW + dd] = nyquist_count(P, d64);
+                rec[dd * PITCH + lane] = r4;
+                sfs[dd * PITCH + lane] = sf;
+                if (NYQ) jcs[dd * PITCH + lane] = nyquist_count(P, d64);
                 if (UNI) {
                     float sn, cs;
                     phase_sincos(P.rot_G, P.rot_Gf, P.rot_gl, T, r4.y, sf, sn, cs);
-                    rots[lane * DPW + dd] = make_float2(cs, sn);
+                    rots[dd * PITCH + lane] = make_float2(cs, sn);
                 }
             }
         }
@@ -228,9 +234,9 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
         if (UNI) {
 #pragma unroll 2
             for (int kk = 0; kk < kBatch; ++kk) {  // a2': sweep with the rotation recurrence
-                const float4 r4 = rec[kk * DPW + ld];
-                const float sf = sfs[kk * DPW + ld];
-                const float2 rot = rots[kk * DPW + ld];
+                const float4 r4 = rec[ld * PITCH + kk];
+                const float sf = sfs[ld * PITCH + kk];
+                const float2 rot = rots[ld * PITCH + kk];
                 float zi0, zr0;
                 phase_sincos(F[0], Ff[0], fl[0], __float_as_uint(r4.x), r4.y, sf, zi0, zr0);
                 const float2 wq = FF ? ws[kk] : make_float2(0.0f, 0.0f);
@@ -264,10 +270,10 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
             // a2: sweep.  Hybrid: of every two particles, kPolyEven / kPolyOdd of the S bins take
             // the FMA-pipe polynomial sincos instead of MUFU.SIN/COS (balances XU against issue).
             auto sweep_one = [&](const int kk, const int n_poly) {
-                const float4 r4 = rec[kk * DPW + ld];
-                const float sf = sfs[kk * DPW + ld];
+                const float4 r4 = rec[ld * PITCH + kk];
+                const float sf = sfs[ld * PITCH + kk];
                 const uint32_t T = __float_as_uint(r4.x);
-                const int m = NYQ ? jcs[kk * DPW + ld] - jbase : 0;  // bins jbase + i*LW < count are kept
+                const int m = NYQ ? jcs[ld * PITCH + kk] - jbase : 0;  // bins jbase + i*LW < count are kept
                 const float2 wq = FF ? ws[kk] : make_float2(0.0f, 0.0f);
 #pragma unroll
                 for (int i = 0; i < S; ++i) {
