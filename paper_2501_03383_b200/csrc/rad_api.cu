@@ -388,6 +388,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.ts32 = (h.t0 + (double)step * h.dt) * h.f_unit * kTwo32;
     p.dts32 = h.dt * h.f_unit * kTwo32;
     p.nyq_lim = h.nyq_lim; p.dt64 = h.dt; p.omega64 = h.omega_d;
+    p.nyq_mode = h.nyq_mode; p.nyq_a = h.nyq_a; p.nyq_b = h.nyq_b;
     p.win_type = h.win_type;
     for (int c = 0; c < 3; ++c) { p.win_o[c] = h.win_o[c]; p.win_il[c] = h.win_il[c]; }
     p.dt = (float)h.dt;
@@ -615,6 +616,22 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
             // F*T wraps mod one turn anyway); the fp32 copy multiplies the residual and stays unwrapped
             h.rot_G = (uint32_t)((uint64_t)G & 0xffffffffull); h.rot_Gf = (float)G; h.rot_gl = (float)(step - G);
             uni_dw = dw;
+        }
+    }
+    // Nyquist limiter: closed-form guess of the cut-off bin on log-spaced / linear grids (checked against the
+    // exact fp64 predicate on the device, rad_device.cuh nyquist_count); any other grid bisects
+    h.nyq_mode = 0;
+    if (h.nyq_lim > 0.0 && h.W >= 3) {
+        const double w0 = h.omega_h.front(), q = h.omega_h[1] / w0, dw = h.omega_h[1] - w0;
+        bool is_log = true, is_lin = true;
+        for (int j = 1; j < h.W; ++j) {
+            is_log = is_log && std::fabs(h.omega_h[j] / h.omega_h[j - 1] / q - 1.0) <= 1e-9;
+            is_lin = is_lin && std::fabs((h.omega_h[j] - h.omega_h[j - 1]) / dw - 1.0) <= 1e-9;
+        }
+        if (is_log) {
+            h.nyq_mode = 1; h.nyq_a = (float)(1.0 / std::log2(q)); h.nyq_b = (float)(h.nyq_lim / (h.dt * w0));
+        } else if (is_lin) {
+            h.nyq_mode = 2; h.nyq_a = (float)(h.nyq_lim / (h.dt * dw)); h.nyq_b = (float)(-w0 / dw);
         }
     }
     // Frequency tables.  Padded bins [W, w_pad) are never folded, but on a uniform grid a thread's

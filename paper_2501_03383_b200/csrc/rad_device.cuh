@@ -86,7 +86,7 @@ __device__ __forceinline__ float ff_weight(float w, float ww, float F2)
 
 __device__ __forceinline__ void stage_record(const Particle &p, const DirRec &dr, double ts32,
                                              float4 &rec, float &sf, uint32_t *T_out = nullptr,
-                                             double *d_out = nullptr)
+                                             double *d_out = nullptr, float *inv_out = nullptr)
 {
     // phase: s32 = (t - n.r/c) f_unit 2^32 in fp64, split into integer (mod 2^32) + residual
     const double s32 = ts32 - fma(dr.kx, p.rx, fma(dr.ky, p.ry, dr.kz * p.rz));
@@ -112,17 +112,36 @@ __device__ __forceinline__ void stage_record(const Particle &p, const DirRec &dr
     sf = to_f32(s32) * kUnitToRad;
     if (T_out) *T_out = T;
     if (d_out) *d_out = d64;
+    if (inv_out) *inv_out = inv;
 }
 
 // Nyquist limiter (rad.h, reading N1): number of bins j with w_j dt d < pi nu.  The predicate is
-// the oracle's expression in fp64, monotone in j, so a bisection over the sorted w_j finds it.
-__device__ __forceinline__ int nyquist_count(const AccumParams &P, double d)
+// the oracle's expression in fp64 (two correctly rounded multiplications, in its order), monotone
+// in j over the sorted w_j.  On log-spaced and linear grids (detected at rad_create) the count is
+// first GUESSED in closed form from the fp32 Doppler factor -- w_cut = pi nu / (dt d), j = log_q(w_cut / w_0)
+// or (w_cut - w_0) / dw, good to ~1e-4 of a bin -- and then CHECKED with the exact predicate (two independent
+// evaluations: bin guess - 1 must be kept, bin guess must not), so the keep/drop set stays the oracle's bit
+// for bit; when the check fails (the cut-off within the guess's error of a bin: ~1 in 5000) and on other
+// grids the count is bisected (10-12 dependent steps).
+__device__ __forceinline__ bool nyquist_keeps(const AccumParams &P, int j, double d)
+{
+    return __dmul_rn(__dmul_rn(__ldg(P.omega64 + j), P.dt64), d) < P.nyq_lim;
+}
+__device__ __forceinline__ int nyquist_count(const AccumParams &P, double d, float inv_d)
 {
     int lo = 0, hi = P.n_omega;
     if (d != d) return hi;  // NaN state: the comparison is false for every bin, nothing is dropped (NaN propagates)
+    if (P.nyq_mode != 0) {
+        const float g = P.nyq_mode == 1 ? P.nyq_a * __log2f(P.nyq_b * inv_d) : fmaf(P.nyq_a, inv_d, P.nyq_b);
+        const int c = (int)fminf(fmaxf(ceilf(g), 0.0f), (float)hi);  // (NaN / Inf / d <= 0 land on an end of the range)
+        const bool above = c < hi ? nyquist_keeps(P, c, d) : false;     // bin c must be dropped ...
+        const bool below = c > 0 ? nyquist_keeps(P, c - 1, d) : true;   // ... and bin c - 1 kept (independent loads)
+        if (!above && below) return c;
+        // the cut-off lies within the guess's error of a bin (or d <= 0): bisect
+    }
     while (lo < hi) {
         const int mid = (lo + hi) >> 1;
-        if (__dmul_rn(__dmul_rn(__ldg(P.omega64 + mid), P.dt64), d) < P.nyq_lim) lo = mid + 1;
+        if (nyquist_keeps(P, mid, d)) lo = mid + 1;
         else hi = mid;
     }
     return lo;

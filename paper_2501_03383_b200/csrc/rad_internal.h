@@ -70,6 +70,8 @@ struct AccumParams {
     double dts32;          // dt f_unit 2^32: multi-step calls, chunk time = ts32 + chunk.step * dts32
     float dt;              // quadrature weight
     double nyq_lim;        // pi * nyquist_factor, 0: limiter off
+    int nyq_mode;          // cut-off guess: 0 none (bisection), 1 log grid, 2 linear grid
+    float nyq_a, nyq_b;    // log: guess = nyq_a * log2(nyq_b / d); linear: guess = nyq_a / d + nyq_b
     double dt64;           // dt in fp64 (limiter comparison)
     const double *omega64; // [W] fp64 angular frequencies (limiter comparison)
     int win_type;          // RAD_WINDOW_*; 0: none
@@ -149,6 +151,8 @@ struct Handle {
     int stream_nb = 0;               // > 0: D*W <= 16 -> particle-streaming kernel with 8 or 16 bins/thread
     double dt = 0, t0 = 0, scale = 0, f_unit = 0;
     double nyq_lim = 0;              // pi * nyquist_factor
+    int nyq_mode = 0;                // closed-form cut-off guess for log / linear grids (rad_device.cuh nyquist_count)
+    float nyq_a = 0, nyq_b = 0;
     double *omega_d = nullptr;       // [W] fp64 (Nyquist limiter only)
     int win_type = 0;
     double win_o[3] = {0, 0, 0}, win_il[3] = {0, 0, 0};

@@ -22,6 +22,8 @@
 // for any |tau|); the other two are O(1/2 turn) and O(tau f_unit) and are added in fp32.
 #include <math_constants.h>
 
+#include <type_traits>
+
 #include "rad_device.cuh"
 #include "rad_internal.h"
 
@@ -219,10 +221,12 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 float sf;
                 uint32_t T;
                 double d64;
-                stage_record(p, P.dirs[dir], ts32, r4, sf, &T, &d64);
+                float inv_d;
+                stage_record(p, P.dirs[dir], ts32, r4, sf, &T, &d64, &inv_d);
                 rec[dd * PITCH + lane] = r4;
                 sfs[dd * PITCH + lane] = sf;
-                if (NYQ) jcs[dd * PITCH + lane] = nyquist_count(P, d64);
+                // bins below the cut-off, relative to the first bin of the warp's frequency tile
+                if (NYQ) jcs[dd * PITCH + lane] = nyquist_count(P, d64, inv_d) - ft * (LW * S);
                 if (UNI) {
                     float sn, cs;
                     phase_sincos(P.rot_G, P.rot_Gf, P.rot_gl, T, r4.y, sf, sn, cs);
@@ -269,14 +273,25 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
         } else {
             // a2: sweep.  Hybrid: of every two particles, kPolyEven / kPolyOdd of the S bins take
             // the FMA-pipe polynomial sincos instead of MUFU.SIN/COS (balances XU against issue).
-            auto sweep_one = [&](const int kk, const int n_poly) {
-                const float4 r4 = rec[ld * PITCH + kk];
-                const float sf = sfs[ld * PITCH + kk];
+            // One staged record against bins [I0, I1) of the strip.  PRED (limiter only): the four FMAs of
+            // bin i are predicated on "bin below this record's cut-off" (bins i*LW < m of the strip are kept).
+            struct Rec { float4 r4; float sf; int m; float2 wq; };
+            auto load_rec = [&](const int kk, const bool pred) {
+                Rec r;
+                r.r4 = rec[ld * PITCH + kk];
+                r.sf = sfs[ld * PITCH + kk];
+                r.m = pred ? jcs[ld * PITCH + kk] - lf : 0;
+                r.wq = FF ? ws[kk] : make_float2(0.0f, 0.0f);
+                return r;
+            };
+            auto sweep_bins = [&](const Rec &r, const int n_poly, auto pred_tag, auto i0_tag, auto i1_tag) {
+                constexpr bool PRED = decltype(pred_tag)::value;
+                constexpr int I0 = decltype(i0_tag)::value, I1 = decltype(i1_tag)::value;
+                const float4 r4 = r.r4;
+                const float sf = r.sf;
                 const uint32_t T = __float_as_uint(r4.x);
-                const int m = NYQ ? jcs[ld * PITCH + kk] - jbase : 0;  // bins jbase + i*LW < count are kept
-                const float2 wq = FF ? ws[kk] : make_float2(0.0f, 0.0f);
 #pragma unroll
-                for (int i = 0; i < S; ++i) {
+                for (int i = I0; i < I1; ++i) {
                     float sn, cs;
                     if (GRID)
                         phase_sincos_grid(F[i % NC], fl[i % NC], T, sf, sn, cs);
@@ -285,11 +300,11 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                     else
                         phase_sincos(F[i % NC], Ff[i % NC], fl[i % NC], T, r4.y, sf, sn, cs);
                     if (FF) {
-                        const float g = ff_weight(wq.x, wq.y, F2r[FF ? i : 0]);
+                        const float g = ff_weight(r.wq.x, r.wq.y, F2r[FF ? i : 0]);
                         sn *= g;
                         cs *= g;
                     }
-                    if (NYQ) {
+                    if (PRED) {
                         // limiter: one SETP + four predicated FFMAs written in PTX, so that the
                         // compiler keeps the bins' instruction streams interleaved (as C++ it
                         // sinks each bin's sincos into a branch of its own: 2.07 -> 3.08 ms)
@@ -297,7 +312,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                             "@p fma.rn.ftz.f32 %0, %4, %6, %0;\n\t@p fma.rn.ftz.f32 %1, %4, %7, %1;\n\t"
                             "@p fma.rn.ftz.f32 %2, %5, %6, %2;\n\t@p fma.rn.ftz.f32 %3, %5, %7, %3;\n\t}"
                             : "+f"(acc[i][0]), "+f"(acc[i][1]), "+f"(acc[i][2]), "+f"(acc[i][3])
-                            : "f"(r4.z), "f"(r4.w), "f"(cs), "f"(sn), "r"(i * LW), "r"(m));
+                            : "f"(r4.z), "f"(r4.w), "f"(cs), "f"(sn), "r"(i * LW), "r"(r.m));
                     } else {
                         acc[i][0] = fmaf(r4.z, cs, acc[i][0]);
                         acc[i][1] = fmaf(r4.z, sn, acc[i][1]);
@@ -306,10 +321,39 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                     }
                 }
             };
+            using No = std::false_type;
+            using Yes = std::true_type;
+            using I0_ = std::integral_constant<int, 0>;
+            using IS_ = std::integral_constant<int, S>;
+            if constexpr (NYQ) {
+                // Two records per turn, as in the plain sweep.  Per pair of records the warp takes one of three
+                // paths: every bin of the tile below the cut-off of every direction of the warp -> the plain sweep;
+                // every bin above -> nothing to do; else predicated.  (Measured on config 1 with nu = 1, 2.26 ms
+                // when every record is predicated: 2.20 ms with these paths; splitting the predicated strip into
+                // four skippable groups of two bins: 2.23 ms -- the shorter basic blocks cost more instruction-level
+                // parallelism than the skipped bins save; 64-bin tiles (8 lanes x 8 bins): 2.42 ms.)
 #pragma unroll 1
-            for (int kk = 0; kk < kBatch; kk += 2) {
-                sweep_one(kk, kPolyEven);
-                sweep_one(kk + 1, kPolyOdd);
+                for (int kk = 0; kk < kBatch; kk += 2) {
+                    const int ma = jcs[ld * PITCH + kk], mb = jcs[ld * PITCH + kk + 1];
+                    const bool all = __all_sync(0xffffffffu, min(ma, mb) >= LW * S);
+                    const bool none = __all_sync(0xffffffffu, max(ma, mb) <= 0);
+                    if (all) {
+                        const Rec ra = load_rec(kk, false), rb = load_rec(kk + 1, false);
+                        sweep_bins(ra, kPolyEven, No{}, I0_{}, IS_{});
+                        sweep_bins(rb, kPolyOdd, No{}, I0_{}, IS_{});
+                    } else if (!none) {
+                        const Rec ra = load_rec(kk, true), rb = load_rec(kk + 1, true);
+                        sweep_bins(ra, kPolyEven, Yes{}, I0_{}, IS_{});
+                        sweep_bins(rb, kPolyOdd, Yes{}, I0_{}, IS_{});
+                    }
+                }
+            } else {
+#pragma unroll 1
+                for (int kk = 0; kk < kBatch; kk += 2) {
+                    const Rec ra = load_rec(kk, false), rb = load_rec(kk + 1, false);
+                    sweep_bins(ra, kPolyEven, No{}, I0_{}, IS_{});
+                    sweep_bins(rb, kPolyOdd, No{}, I0_{}, IS_{});
+                }
             }
         }
         __syncwarp();

@@ -170,6 +170,7 @@ class Workload:
     t0: float = 0.0
     extra: dict = field(default_factory=dict)
     form_factor: Optional[tuple] = None     # (type name, size[3] in metres) for rad_config / the oracle
+    nyquist: float = 0.0                    # rad_config.nyquist_factor (0: limiter off)
 
     @property
     def n_dir(self) -> int:
@@ -253,6 +254,12 @@ def make_workload(cfg: str) -> Workload:
         return Workload("cfg1f_khi_form_factor", 65536, 1000, 1e-17, dirs_fibonacci(128),
                         omega_log(512), np.float32, BASE_SEED + 1, "khi", extra={"weights": 1e4},
                         form_factor=("gaussian", (3e-8, 3e-8, 3e-8)))
+    if cfg == "1n":
+        # config 1 with the Nyquist limiter at nu = 1 (w dt (1 - beta.n) >= pi dropped: at dt = 1e-17 s the
+        # top ~1/8 of the log grid, the cut-off Doppler-shifted per particle and direction): the limiter
+        # leg of bench.py (not a BASELINE.json config)
+        return Workload("cfg1n_khi_nyquist", 65536, 1000, 1e-17, dirs_fibonacci(128),
+                        omega_log(512), np.float32, BASE_SEED + 1, "khi", nyquist=1.0)
     if cfg == "5r":
         # smallest KHI run = 192 x 256 x 12 cells x 9 particles per cell on 16
         # GPUs -> 331 776 particles per GPU; line 196: one ML sample = the ~3e4 particles of a
@@ -262,4 +269,4 @@ def make_workload(cfg: str) -> Workload:
     raise KeyError(cfg)
 
 
-ALL_CONFIGS = ("0", "1", "1u", "1f", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r")
+ALL_CONFIGS = ("0", "1", "1u", "1f", "1n", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r")
