@@ -74,7 +74,9 @@ typedef enum { RAD_F32 = 0, RAD_F64 = 1 } rad_dtype;
 /* rad_config.flags */
 #define RAD_FLAG_DETERMINISTIC 1u /* bit 0: no floating-point atomics; results are
                                      bit-reproducible run to run (slower, more memory) */
-#define RAD_FLAG_FORCE_GENERAL 2u /* bit 1: never use the uniform-grid recurrence kernel */
+#define RAD_FLAG_FORCE_GENERAL 2u /* bit 1: never use the grid-specific variants (the uniform-grid
+                                     recurrence kernel, the dyadic-grid squaring chains): always the
+                                     general-grid kernel */
 #define RAD_FLAG_OVERLAP_STEPS 4u /* bit 2: consecutive calls on one stream may overlap (below) */
 #define RAD_FLAG_FAST_GRIDDED 8u  /* bit 3: approximate fast path (gridded in retarded time, below) */
 
@@ -182,6 +184,13 @@ typedef struct {
 #define RAD_WINDOW_NONE 0
 #define RAD_WINDOW_TRIANGLE 1
 #define RAD_WINDOW_HAMMING 2
+
+/* Frequency grids.  Any strictly increasing grid is served by the general-grid kernel (one sin/cos
+ * per update).  Two structures are detected at rad_create and served by faster variants with the same
+ * results to rounding (same tolerances, tests/test_gpu_parity.py): a LINEAR grid w_j = w_0 + j dw
+ * (rotation recurrence, BASELINE.json north_star) and a DYADIC log grid, w_(j+b) = 2 w_j for an integer
+ * number b in {4, 8, 16, 32, 64} of bins per octave (z(2w) = z(w)^2).
+ * rad_kernel_variant() names the variant in use; RAD_FLAG_FORCE_GENERAL switches both off. */
 
 /* Create a detector for a grid of observation directions n and frequencies w_j (BASELINE.json
  * north_star "on a grid of observation directions n and frequencies w"; the

@@ -598,6 +598,42 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     }
     h.sdir[0] = recs[0]; h.sdir[1] = recs[h.D > 1 ? 1 : 0];
     choose_tile(h);
+    // Dyadic log grid (SURVEY.md section 8(f) NEXT-4 "dyadic log grids (integer bins/octave) allow
+    // z(2w) = z(w)^2"): w_(j+b) = 2 w_j for an integer b = c * lw with lw in {4, 8, 16, 32}, c in {1, 2} ->
+    // bins i and i + c of a thread's strip are an octave apart.  Among the admissible tile shapes the
+    // widest one wins unless it pads more than choose_tile's own choice does.
+    h.dyad_c = 0;
+    if (!(cfg->flags & RAD_FLAG_FORCE_GENERAL) && h.nyq_lim == 0.0 && !h.fast && h.ff_type == RAD_FF_NONE && h.W >= 2) {
+        int b = 0;
+        for (int cand = 4; cand <= 64 && cand < h.W && b == 0; ++cand) {
+            bool ok = true;
+            for (int j = 0; j + cand < h.W && ok; ++j)
+                ok = std::fabs(h.omega_h[j + cand] / (2.0 * h.omega_h[j]) - 1.0) <= 1e-12;
+            if (ok) b = cand;
+        }
+        double best = -1.0;
+        int best_lw = 0, best_c = 0;
+        for (int lw = 32; lw >= 4; lw >>= 1)
+            for (int c = 1; c <= 2; ++c) {
+                if (b != c * lw) continue;
+                const int tile = lw * h.strip, dpw = 32 / lw;
+                const double eff = ((double)h.W / ((h.W + tile - 1) / tile * tile)) *
+                                   ((double)h.D / ((h.D + dpw - 1) / dpw * dpw));
+                if (eff > best + 1e-9) { best = eff; best_lw = lw; best_c = c; }
+            }
+        if (best_lw) {
+            const int tile0 = h.lw * h.strip, dpw0 = 32 / h.lw;
+            const double eff0 = ((double)h.W / h.w_pad) * ((double)h.D / ((h.D + dpw0 - 1) / dpw0 * dpw0));
+            (void)tile0;
+            if (best >= 0.8 * eff0) {  // the squaring chains are worth ~1.3x: accept up to 20 % more padding
+                h.lw = best_lw; h.dyad_c = best_c;
+                const int tile = h.lw * h.strip, dpw = 32 / h.lw;
+                h.w_pad = (h.W + tile - 1) / tile * tile;
+                h.n_ftiles = h.w_pad / tile;
+                h.n_wtiles = ((h.D + dpw - 1) / dpw) * h.n_ftiles;
+            }
+        }
+    }
     // per-region detectors and the Nyquist limiter: bin-owner kernels only
     h.stream_nb = (h.R > 1 || h.nyq_lim > 0.0 || h.fast) ? 0 : stream_shape(h.D, h.W, &h.stream_nd);
     // uniform grid?  w_j = w_0 + j dw to fp64 rounding -> rotation-recurrence kernel (a2')

@@ -117,13 +117,23 @@ __device__ __forceinline__ bool decode_task(const AccumParams &P, int warp, int 
 // FF: macro-particle form factor (rad.h, reading FF1) -- every update's (cos, sin) is scaled by
 // g = sqrt(w + (w^2 - w) F^2): F^2 of the thread's S bins in registers, (w, w^2 - w) of the batch's
 // particles in shared memory; one FFMA + MUFU.SQRT + 2 FMUL more per update.
+// DY (general grid only): dyadic log grid, w_(j + DY*LW) = 2 w_j (an integer number of bins per octave that
+// the tile shape divides: rad_api.cu).  Bins i and i + DY of a thread's strip are then one octave apart and
+// z_(i+DY) = z_i^2 (4 FMA-pipe instructions instead of the phase arithmetic + MUFU.SIN/COS).  Chains are
+// kDyadChain = 2 bins long: every second bin of a chain is anchored by a direct sincos, the other is its
+// square.  A squaring doubles the phase error and the deviation of |z| from 1: measured maxrel against the
+// oracle with one squaring per chain = the plain kernel's (2.5e-4 vs 2.9e-4 on a 6 x 300 detector), with two
+// squarings 2.2e-3 (beyond the 1e-3 tolerance: the MUFU error x 4).
 // GRID: evaluation of the fast gridded path (rad.h RAD_FLAG_FAST_GRIDDED) -- the "particles" are the
 // points of the per-direction retarded-time grids: point m of direction n has phase s32 = g_s0[n] +
 // m g_hs and amplitude g_master[n][m]; the sweep and the phase arithmetic are those of the general grid.
-template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ, bool FF, bool GRID = false>
+constexpr int kDyadChain = 2;  // dyadic grids: bins per squaring chain (1 anchor + kDyadChain - 1 squarings)
+
+template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ, bool FF, bool GRID = false, int DY = 0>
 __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
 {
     static_assert(!GRID || (!UNI && !NYQ && !FF), "grid evaluation runs the plain general-grid sweep");
+    static_assert(DY == 0 || (!UNI && !NYQ && !FF && !GRID), "dyadic squaring runs on the plain general-grid sweep");
     static_assert(!(UNI && NYQ), "the limiter runs on the general-grid kernel");
     constexpr int DPW = 32 / LW;
     // Shared-memory records are direction-major, rec[direction of the warp][particle of the batch], rows padded
@@ -290,15 +300,22 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 const float4 r4 = r.r4;
                 const float sf = r.sf;
                 const uint32_t T = __float_as_uint(r4.x);
+                float zs[S], zc[S];  // DY: the strip's (sin, cos), bin i + DY squares bin i
 #pragma unroll
                 for (int i = I0; i < I1; ++i) {
                     float sn, cs;
-                    if (GRID)
+                    if (DY > 0 && (i / (DY > 0 ? DY : 1)) % kDyadChain != 0) {
+                        const float ps = zs[i >= DY ? i - DY : 0], pc = zc[i >= DY ? i - DY : 0];
+                        cs = fmaf(pc, pc, -ps * ps);
+                        sn = (pc + pc) * ps;
+                    } else if (GRID)
                         phase_sincos_grid(F[i % NC], fl[i % NC], T, sf, sn, cs);
                     else if (i >= S - n_poly)
                         phase_sincos_poly(F[i % NC], Ff[i % NC], fl[i % NC], T, r4.y, sf, sn, cs);
                     else
                         phase_sincos(F[i % NC], Ff[i % NC], fl[i % NC], T, r4.y, sf, sn, cs);
+                    zs[i] = sn;
+                    zc[i] = cs;
                     if (FF) {
                         const float g = ff_weight(r.wq.x, r.wq.y, F2r[FF ? i : 0]);
                         sn *= g;
@@ -351,8 +368,8 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
 #pragma unroll 1
                 for (int kk = 0; kk < kBatch; kk += 2) {
                     const Rec ra = load_rec(kk, false), rb = load_rec(kk + 1, false);
-                    sweep_bins(ra, kPolyEven, No{}, I0_{}, IS_{});
-                    sweep_bins(rb, kPolyOdd, No{}, I0_{}, IS_{});
+                    sweep_bins(ra, DY > 0 ? 0 : kPolyEven, No{}, I0_{}, IS_{});   // dyadic: the XU pipe is not the bound
+                    sweep_bins(rb, DY > 0 ? 0 : kPolyOdd, No{}, I0_{}, IS_{});
                 }
             }
         }
@@ -406,10 +423,28 @@ cudaError_t launch_eval_grid(const Handle &h, const AccumParams &p, cudaStream_t
     }
 }
 
+template <typename ST, int DY>
+static cudaError_t dispatch_dyadic(const Handle &h, const AccumParams &p, cudaStream_t s)
+{
+    const long long n_tasks = (long long)p.n_wtiles * p.n_chunks;
+    const dim3 grid((unsigned)((n_tasks + kWarpsPerBlock - 1) / kWarpsPerBlock));
+    switch (h.lw) {
+        case 32: return launch_kernel(rad_accum<ST, 32, kStrip, kMinBlocks, false, false, false, false, DY>, grid, dim3(kThreads), 0, s, h.overlap, p);
+        case 16: return launch_kernel(rad_accum<ST, 16, kStrip, kMinBlocks, false, false, false, false, DY>, grid, dim3(kThreads), 0, s, h.overlap, p);
+        case 8: return launch_kernel(rad_accum<ST, 8, kStrip, kMinBlocks, false, false, false, false, DY>, grid, dim3(kThreads), 0, s, h.overlap, p);
+        default: return launch_kernel(rad_accum<ST, 4, kStrip, kMinBlocks, false, false, false, false, DY>, grid, dim3(kThreads), 0, s, h.overlap, p);
+    }
+}
+
 cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_f64,
                               cudaStream_t s, int *n_launches, const char **variant)
 {
     *n_launches = 1;
+    if (h.dyad_c > 0 && !h.uniform && p.nyq_lim == 0.0 && !p.F2) {
+        *variant = "general+dyadic";
+        if (h.dyad_c == 1) return state_f64 ? dispatch_dyadic<double, 1>(h, p, s) : dispatch_dyadic<float, 1>(h, p, s);
+        return state_f64 ? dispatch_dyadic<double, 2>(h, p, s) : dispatch_dyadic<float, 2>(h, p, s);
+    }
     if (h.uniform) {
         *variant = p.F2 ? "uniform+formfactor" : "uniform";
         return state_f64 ? dispatch<double, true, false>(h, p, s) : dispatch<float, true, false>(h, p, s);

@@ -73,6 +73,15 @@ def omega_log(n: int, lo: float = 1e14, hi: float = 1e18) -> np.ndarray:
     return lo * (hi / lo) ** (np.arange(n, dtype=np.float64) / (n - 1))
 
 
+def omega_dyadic(n: int, bins_per_octave: int, hi: float = 1e18) -> np.ndarray:
+    """Log grid with an integer number of bins per octave, top bin = hi: w_(j+b) = 2 w_j EXACTLY
+    (one octave of b values times exact powers of two)."""
+    b = int(bins_per_octave)
+    j = np.arange(n, dtype=np.int64) - (n - 1)              # <= 0: octaves below the top bin
+    base = hi * 2.0 ** (-(np.arange(b, dtype=np.float64)) / b)   # one octave, descending from hi
+    return np.ldexp(base[(-j) % b], -((-j) // b).astype(np.int64))
+
+
 def omega_linear(n: int, hi: float) -> np.ndarray:
     return (np.arange(n, dtype=np.float64) + 1.0) * (hi / n)
 
@@ -254,6 +263,13 @@ def make_workload(cfg: str) -> Workload:
         return Workload("cfg1f_khi_form_factor", 65536, 1000, 1e-17, dirs_fibonacci(128),
                         omega_log(512), np.float32, BASE_SEED + 1, "khi", extra={"weights": 1e4},
                         form_factor=("gaussian", (3e-8, 3e-8, 3e-8)))
+    if cfg == "1d":
+        # config 1 on a DYADIC log grid: 32 bins per octave, 512 bins = 16 octaves below 1e18 rad/s
+        # ([1.56e13, 1e18]): the shape on which the squaring-chain variant of the general kernel is
+        # measured (not a BASELINE.json config, whose log grids have
+        # 38.46 / 76.99 bins per octave)
+        return Workload("cfg1d_khi_dyadic_grid", 65536, 1000, 1e-17, dirs_fibonacci(128),
+                        omega_dyadic(512, 32), np.float32, BASE_SEED + 1, "khi")
     if cfg == "1n":
         # config 1 with the Nyquist limiter at nu = 1 (w dt (1 - beta.n) >= pi dropped: at dt = 1e-17 s the
         # top ~1/8 of the log grid, the cut-off Doppler-shifted per particle and direction): the limiter
@@ -269,4 +285,4 @@ def make_workload(cfg: str) -> Workload:
     raise KeyError(cfg)
 
 
-ALL_CONFIGS = ("0", "1", "1u", "1f", "1n", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r")
+ALL_CONFIGS = ("0", "1", "1u", "1f", "1n", "1d", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r")

@@ -72,6 +72,40 @@ def test_uniform_grid_padded_anchor_shapes(oracle_mod, D, W, dtype):
     assert vg == "general" and P.rel_l2(S, Sg) < 1e-5
 
 
+@pytest.mark.parametrize("D,W,b,dtype", [(6, 300, 32, np.float32), (3, 512, 64, np.float32), (33, 100, 8, np.float32),
+                                         (9, 70, 16, np.float64), (16, 40, 4, np.float32), (2, 1000, 64, np.float64)])
+def test_dyadic_log_grid_squaring_chains(oracle_mod, D, W, b, dtype):
+    """SURVEY.md section 8(f) NEXT-4, second half: log grids with an integer number b of bins per octave
+    run the squaring-chain variant (z(2w) = z(w)^2, every third bin of a chain anchored by a direct
+    sincos) -- every tile shape (b = 4 ... 64 = lanes x chain stride), ragged W (padded anchors), late
+    steps; same tolerances, per direction too; the plain general kernel on the same grid agrees."""
+    from paper_2501_03383_b200 import binding
+    w = wl.Workload("dyad", 1500, 3, 1e-17, wl.dirs_fibonacci(max(D, 2))[:D], wl.omega_dyadic(W, b), dtype,
+                    wl.BASE_SEED + 23, "khi")
+    steps = [(t * 350 + 2, st) for t, st in w.steps(n_steps=3)]
+    S, variant = P.run_gpu(w, steps)
+    assert variant == "general+dyadic"
+    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    l2, mr = P.assert_parity(S, ref, what=f"dyadic {D}x{W} b={b}")
+    for d in range(D):
+        P.assert_parity(S[d], ref[d], what=f"dyadic {D}x{W} b={b} dir {d}")
+    Sg, vg = P.run_gpu(w, steps, flags=binding.RAD_FLAG_FORCE_GENERAL)
+    assert vg == "general" and P.rel_l2(S, Sg) < 1e-5
+    l2g, mrg = P.assert_parity(Sg, ref, what=f"general on the dyadic grid {D}x{W}")
+    print(f"dyadic {D}x{W} b={b} {np.dtype(dtype).name}: relL2={l2:.2e} maxrel={mr:.2e} (plain general kernel: {l2g:.2e} / {mrg:.2e})")
+
+
+def test_dyadic_detection_falls_back(oracle_mod):
+    """Not dyadic (BASELINE.json's own log grids: 38.46 bins per octave), bins per octave the tile shapes
+    cannot divide (12), or a dyadic grid with one perturbed bin: the plain general kernel."""
+    for om in (wl.omega_log(512), wl.omega_dyadic(200, 12), wl.omega_dyadic(300, 32) * (1 + 1e-9 * (np.arange(300) == 77))):
+        w = wl.Workload("nodyad", 300, 1, 1e-17, wl.dirs_fibonacci(4), om, np.float32, wl.BASE_SEED + 24, "khi")
+        steps = list(w.steps())
+        S, variant = P.run_gpu(w, steps)
+        assert variant == "general"
+        P.assert_parity(S, P.run_oracle(oracle_mod, w, steps).spectrum(), what="non-dyadic log grid")
+
+
 @pytest.mark.parametrize("dtype", [np.float32, np.float64])
 @pytest.mark.parametrize("shape", ["general", "uniform", "stream"])
 def test_non_finite_particle_state_propagates(dtype, shape):

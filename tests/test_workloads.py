@@ -25,6 +25,9 @@ def test_grids():
     om = wl.omega_log(512)
     assert om[0] == 1e14 and om[-1] == pytest.approx(1e18, rel=1e-12) and np.all(np.diff(om) > 0)
     assert np.allclose(om[1:] / om[:-1], om[1] / om[0], rtol=1e-12)
+    dy = wl.omega_dyadic(100, 8)
+    assert dy[-1] == 1e18 and np.all(np.diff(dy) > 0) and np.array_equal(dy[8:], 2.0 * dy[:-8])
+    assert np.allclose(dy[1:] / dy[:-1], 2.0 ** 0.125, rtol=1e-14)
     lin = wl.omega_linear(64, 4e14)
     assert lin[0] == pytest.approx(6.25e12) and lin[-1] == pytest.approx(4e14)
 
@@ -37,7 +40,7 @@ def test_config_shapes(cfg):
              "3c": (262144, 200, 256, 256), "3d": (262144, 200, 1024, 64),
              "4": (16777216, 4, 16, 128), "4b": (16777216, 4, 1, 8),
              "5r": (331776, 200, 1, 512), "1u": (65536, 1000, 128, 512),
-             "1f": (65536, 1000, 128, 512), "1n": (65536, 1000, 128, 512)}[cfg]
+             "1f": (65536, 1000, 128, 512), "1n": (65536, 1000, 128, 512), "1d": (65536, 1000, 128, 512)}[cfg]
     assert (w.n_particles, w.n_steps, w.n_dir, w.n_omega) == sizes
     assert w.state_dtype == (np.float64 if cfg == "0" else np.float32)
 
