@@ -95,6 +95,54 @@ def test_dyadic_log_grid_squaring_chains(oracle_mod, D, W, b, dtype):
     print(f"dyadic {D}x{W} b={b} {np.dtype(dtype).name}: relL2={l2:.2e} maxrel={mr:.2e} (plain general kernel: {l2g:.2e} / {mrg:.2e})")
 
 
+def test_dyadic_grid_with_regions_multi_step_deterministic_and_overlap(oracle_mod):
+    """The squaring-chain variant under the other call forms: per-region handle (ragged regions, one
+    launch), rad_accumulate_steps (one launch for all steps), deterministic mode (bit-reproducible),
+    RAD_FLAG_OVERLAP_STEPS with a spectrum between steps."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    w = wl.Workload("dyad2", 2600, 4, 1e-17, wl.dirs_fibonacci(5), wl.omega_dyadic(200, 16), np.float32,
+                    wl.BASE_SEED + 25, "khi")
+    steps = list(w.steps())
+    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    off = np.array([0, 700, 700, 701, 1500, 2600], dtype=np.int64)
+    ro = oracle_mod.RegionOracle(5, w.dirs, w.omega, w.dt, scale=1.0)
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, n_regions=5) as det:
+        for t, st in steps:
+            det.accumulate_step_regions(t, off, P.to_device(st))
+            ro.accumulate_step(t, off, *st)
+        assert det.kernel_variant == "general+dyadic"
+        Sr, St = det.spectrum(), det.spectrum_total()
+    P.assert_parity(St, ref, what="dyadic regions total")
+    Rr = ro.spectrum()
+    for r in (0, 3, 4):
+        P.assert_parity(Sr[r], Rr[r], what=f"dyadic region {r}")
+    assert np.all(Sr[1] == 0.0)
+    stacked = [torch.from_numpy(np.stack([st[c] for _, st in steps])).cuda() for c in range(10)]
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0) as det:
+        det.accumulate_steps(0, stacked)
+        assert det.kernel_variant == "general+dyadic"
+        P.assert_parity(det.spectrum(), ref, what="dyadic multi-step")
+    runs = []
+    for _ in range(2):
+        S, v = P.run_gpu(w, steps, flags=binding.RAD_FLAG_DETERMINISTIC)
+        assert v == "general+dyadic"
+        runs.append(S)
+    assert np.array_equal(runs[0], runs[1])
+    P.assert_parity(runs[0], ref, what="dyadic deterministic")
+    devs = [P.to_device(st) for _, st in steps]
+    torch.cuda.synchronize()
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, flags=binding.RAD_FLAG_OVERLAP_STEPS) as det:
+        mids = []
+        for (t, _), dev in zip(steps, devs):
+            det.accumulate_step(t, dev)
+            mids.append(det.spectrum())
+        o = oracle_mod.Oracle(w.dirs, w.omega, w.dt, scale=1.0)
+        for (t, st), S in zip(steps, mids):
+            o.accumulate_step(t, *st)
+            P.assert_parity(S, o.spectrum(), what=f"dyadic overlap after step {t}")
+
+
 def test_dyadic_detection_falls_back(oracle_mod):
     """Not dyadic (BASELINE.json's own log grids: 38.46 bins per octave), bins per octave the tile shapes
     cannot divide (12), or a dyadic grid with one perturbed bin: the plain general kernel."""
