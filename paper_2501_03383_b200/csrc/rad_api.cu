@@ -622,9 +622,8 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
                 if (eff > best + 1e-9) { best = eff; best_lw = lw; best_c = c; }
             }
         if (best_lw) {
-            const int tile0 = h.lw * h.strip, dpw0 = 32 / h.lw;
+            const int dpw0 = 32 / h.lw;
             const double eff0 = ((double)h.W / h.w_pad) * ((double)h.D / ((h.D + dpw0 - 1) / dpw0 * dpw0));
-            (void)tile0;
             if (best >= 0.8 * eff0) {  // the squaring chains are worth ~1.3x: accept up to 20 % more padding
                 h.lw = best_lw; h.dyad_c = best_c;
                 const int tile = h.lw * h.strip, dpw = 32 / h.lw;
