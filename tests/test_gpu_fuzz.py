@@ -119,3 +119,37 @@ def test_random_case_matches_oracle(oracle_mod, case):
         assert np.all(S == 0.0), what
     if "nyquist" in c["opts"]:                              # the keep/drop decision is exact: identical zero sets
         assert np.array_equal(S == 0.0, ref == 0.0), what
+
+
+@pytest.mark.parametrize("case", range(24))
+def test_random_case_fast_gridded_matches_exact_oracle(oracle_mod, case):
+    """The approximate fast path (RAD_FLAG_FAST_GRIDDED, default gridding tolerance) on drawn shapes, grids,
+    dtypes and step windows against the EXACT oracle with the exact path's tolerances."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    rng = np.random.default_rng(9900 + case)
+    D = int(rng.choice([1, 3, 8, 33]))
+    W = int(rng.choice([8, 40, 64, 100, 300]))
+    kind = str(rng.choice(["log", "linear", "random", "dyadic"]))
+    omega = {"log": lambda: wl.omega_log(W) * rng.uniform(0.5, 2.0),
+             "linear": lambda: np.linspace(2e14, rng.uniform(1e17, 6e17), W),
+             "random": lambda: np.sort(10.0 ** rng.uniform(14, 18, W)) * (1 + 1e-3 * np.arange(W)),
+             "dyadic": lambda: wl.omega_dyadic(W, 16, hi=rng.uniform(2e17, 1e18))}[kind]()
+    dtype = np.float64 if rng.random() < 0.3 else np.float32
+    n, T, t_first = int(rng.choice([33, 1000, 3000])), int(rng.integers(1, 5)), int(rng.choice([0, 40, 700]))
+    window = ("hamming", (0.1 * L, 0.0, 0.0), (0.8 * L, 0.0, 0.0)) if rng.random() < 0.25 else None
+    w = wl.Workload(f"fuzzfast{case}", n, T, 1e-17, wl.dirs_fibonacci(max(D, 2))[:D], omega, dtype,
+                    int(rng.integers(1, 10 ** 6)), "khi")
+    steps = [(t_first + t, st) for t, st in w.steps()]
+    o = oracle_mod.Oracle(w.dirs, w.omega, w.dt, scale=1.0, window=window)
+    for t, st in steps:
+        o.accumulate_step(t, *st)
+    box = ((-0.02 * L,) * 3, (1.02 * L,) * 3)
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, state_dtype=dtype, flags=binding.RAD_FLAG_FAST_GRIDDED,
+                          window=window, fast=(box[0], box[1], t_first, t_first + T - 1, 0.0)) as det:
+        for t, st in steps:
+            det.accumulate_step(t, P.to_device(st))
+        torch.cuda.synchronize()
+        S = det.spectrum()
+        assert det.kernel_variant == "gridded"
+    P.assert_parity(S, o.spectrum(), what=f"fuzz fast {case}: {D}x{W} {kind} {np.dtype(dtype).name} n={n} T={T} t0={t_first}")
