@@ -9,7 +9,7 @@ rad_spectrum (a4).  Metric (BASELINE.json): particle*direction*frequency updates
 in G/s, whole job.  Headline workload = BASELINE.json configs[2] ("production-like": 1 048 576
 electrons x 256 directions x 1024 log-spaced frequencies, fp32 state), the largest single-GPU
 configuration.  The same invocation also runs short legs of every other configuration (1, 3a-d,
-4, 4b, 5r, 0, 1u, 1f, 1n, 1d) and reports them under "configs", runs the pipe microbenchmarks
+4, 4b, 5r, 5s, 0, 1u, 1f, 1n, 1d) and reports them under "configs", runs the pipe microbenchmarks
 (librad_ubench.so) and reports the measured ALU peaks under "alu_peaks", and compares the
 spectrum left by the timed region with the fp64 oracle on sampled bins ("parity").
 
@@ -47,7 +47,7 @@ FP32_PER_UPDATE_UNIFORM = 8  # 4 (complex rotation) + 4 (accumulate) FMA-pipe in
 L2_BYTES = 126 * 2 ** 20
 # short legs run after the headline: (config, timed steps, warm-up steps)
 LEGS = (("1", 50, 3), ("3a", 10, 3), ("3b", 10, 3), ("3c", 10, 3), ("3d", 10, 3), ("4", 3, 1), ("4b", 200, 3),
-        ("5r", 200, 5), ("0", 500, 5), ("1u", 50, 3), ("1f", 50, 3), ("1n", 50, 3), ("1d", 50, 3))
+        ("5r", 200, 5), ("5s", 200, 5), ("0", 500, 5), ("1u", 50, 3), ("1f", 50, 3), ("1n", 50, 3), ("1d", 50, 3))
 
 
 def parse_args():

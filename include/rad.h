@@ -190,7 +190,10 @@ typedef struct {
  * results to rounding (same tolerances, tests/test_gpu_parity.py): a LINEAR grid w_j = w_0 + j dw
  * (rotation recurrence, BASELINE.json north_star) and a DYADIC log grid, w_(j+b) = 2 w_j for an integer
  * number b in {4, 8, 16, 32, 64} of bins per octave (z(2w) = z(w)^2).
- * rad_kernel_variant() names the variant in use; RAD_FLAG_FORCE_GENERAL switches both off. */
+ * rad_kernel_variant() names the variant in use; RAD_FLAG_FORCE_GENERAL switches both off.
+ * Detector shapes: any n_dir >= 1, n_omega >= 1.  n_dir * n_omega <= 16 (up to 2 directions) runs the
+ * particle-streaming kernel; detectors with few directions and a moderate number of frequencies let the lane
+ * groups of a warp split the particles instead of idling ("+split" in the variant name). */
 
 /* Create a detector for a grid of observation directions n and frequencies w_j (BASELINE.json
  * north_star "on a grid of observation directions n and frequencies w"; the

@@ -64,22 +64,40 @@ void free_all(Handle &h)
     if (h.copy_stream) cudaStreamDestroy(h.copy_stream);
 }
 
-// Tile shape: lw lanes along frequency x 8 bins per lane, 32/lw directions per warp.
-// Pick the shape wasting the fewest padded bins / padded directions; ties -> wider lw.
-void choose_tile(Handle &h)
+// Tile shape: lw lanes along frequency x 8 bins per lane, 32/lw directions per warp.  A detector with
+// fewer directions than a warp holds (D <= dpw / 2) does not leave the other lane groups idle: 2^ps groups
+// share one direction and split the particles of a batch between them ("particle split", rad_kernels.cu).
+// -> fraction of the warp's lanes x bins that are real work; *ps = log2 of the groups per direction.
+double tile_efficiency(const Handle &h, int lw, int *ps, bool allow_split)
 {
-    double best = -1.0;
-    for (int lw = 32; lw >= 4; lw >>= 1) {
-        const int tile = lw * h.strip, dpw = 32 / lw;
-        const int w_pad = (h.W + tile - 1) / tile * tile;
-        const int d_pad = (h.D + dpw - 1) / dpw * dpw;
-        const double eff = ((double)h.W / w_pad) * ((double)h.D / d_pad);
-        if (eff > best + 1e-9) { best = eff; h.lw = lw; }
-    }
-    const int tile = h.lw * h.strip, dpw = 32 / h.lw;
+    const int tile = lw * h.strip, dpw = 32 / lw;
+    const int w_pad = (h.W + tile - 1) / tile * tile;
+    *ps = 0;
+    while (allow_split && dpw > 1 && (h.D << (*ps + 1)) <= dpw) ++*ps;
+    const int d_pad = *ps > 0 ? dpw : (h.D + dpw - 1) / dpw * dpw;
+    return ((double)h.W / w_pad) * ((double)(h.D << *ps) / d_pad);
+}
+
+void set_tile(Handle &h, int lw, int ps)
+{
+    const int tile = lw * h.strip, dpw = 32 / lw;
+    h.lw = lw; h.psplit = ps;
     h.w_pad = (h.W + tile - 1) / tile * tile;
     h.n_ftiles = h.w_pad / tile;
-    h.n_wtiles = ((h.D + dpw - 1) / dpw) * h.n_ftiles;
+    h.n_wtiles = (((h.D << ps) + dpw - 1) / dpw) * h.n_ftiles;
+}
+
+// Pick the shape wasting the fewest padded bins / padded directions; ties -> wider lw.
+void choose_tile(Handle &h, bool allow_split)
+{
+    double best = -1.0;
+    int best_lw = 32, best_ps = 0;
+    for (int lw = 32; lw >= 4; lw >>= 1) {
+        int ps;
+        const double eff = tile_efficiency(h, lw, &ps, allow_split);
+        if (eff > best + 1e-9) { best = eff; best_lw = lw; best_ps = ps; }
+    }
+    set_tile(h, best_lw, best_ps);
 }
 
 // Particles per block: enough blocks for >= ~8 waves of (SMs x resident blocks) so that the
@@ -383,7 +401,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     // per-region calls: every region rounds its own chunk count up -> leave room for that
     p.chunk = choose_chunk(h, (region_off ? n + (long long)h.R * 64 : n) * n_steps);
     p.n_dir = h.D; p.n_omega = h.W; p.w_pad = h.w_pad;
-    p.n_ftiles = h.n_ftiles; p.n_wtiles = h.n_wtiles;
+    p.n_ftiles = h.n_ftiles; p.n_wtiles = h.n_wtiles; p.psplit = h.psplit;
     p.dirs = h.dirs_d; p.F = h.F_d; p.Ff = h.Ff_d; p.fl = h.fl_d; p.F2 = h.F2_d;
     p.ts32 = (h.t0 + (double)step * h.dt) * h.f_unit * kTwo32;
     p.dts32 = h.dt * h.f_unit * kTwo32;
@@ -597,7 +615,8 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         r.pad[0] = r.pad[1] = r.pad[2] = 0.0f;
     }
     h.sdir[0] = recs[0]; h.sdir[1] = recs[h.D > 1 ? 1 : 0];
-    choose_tile(h);
+    // particle split: the plain general / uniform sweeps only (rad_kernels.cu SPLIT instantiations)
+    choose_tile(h, h.nyq_lim == 0.0 && h.ff_type == RAD_FF_NONE && !h.fast);
     // Dyadic log grid (SURVEY.md section 8(f) NEXT-4 "dyadic log grids (integer bins/octave) allow
     // z(2w) = z(w)^2"): w_(j+b) = 2 w_j for an integer b = c * lw with lw in {4, 8, 16, 32}, c in {1, 2} ->
     // bins i and i + c of a thread's strip are an octave apart.  Among the admissible tile shapes the
@@ -612,25 +631,19 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
             if (ok) b = cand;
         }
         double best = -1.0;
-        int best_lw = 0, best_c = 0;
+        int best_lw = 0, best_c = 0, best_ps = 0;
         for (int lw = 32; lw >= 4; lw >>= 1)
             for (int c = 1; c <= 2; ++c) {
                 if (b != c * lw) continue;
-                const int tile = lw * h.strip, dpw = 32 / lw;
-                const double eff = ((double)h.W / ((h.W + tile - 1) / tile * tile)) *
-                                   ((double)h.D / ((h.D + dpw - 1) / dpw * dpw));
-                if (eff > best + 1e-9) { best = eff; best_lw = lw; best_c = c; }
+                int ps;
+                const double eff = tile_efficiency(h, lw, &ps, false);   // the squaring chains run without the split
+                if (eff > best + 1e-9) { best = eff; best_lw = lw; best_c = c; best_ps = ps; }
             }
-        if (best_lw) {
-            const int dpw0 = 32 / h.lw;
-            const double eff0 = ((double)h.W / h.w_pad) * ((double)h.D / ((h.D + dpw0 - 1) / dpw0 * dpw0));
-            if (best >= 0.8 * eff0) {  // the squaring chains are worth ~1.3x: accept up to 20 % more padding
-                h.lw = best_lw; h.dyad_c = best_c;
-                const int tile = h.lw * h.strip, dpw = 32 / h.lw;
-                h.w_pad = (h.W + tile - 1) / tile * tile;
-                h.n_ftiles = h.w_pad / tile;
-                h.n_wtiles = ((h.D + dpw - 1) / dpw) * h.n_ftiles;
-            }
+        int ps0;
+        if (best_lw && best >= 0.8 * tile_efficiency(h, h.lw, &ps0, true)) {
+            // the squaring chains are worth ~1.3x: accept up to 20 % more padding than the free choice
+            set_tile(h, best_lw, best_ps);
+            h.dyad_c = best_c;
         }
     }
     // per-region detectors and the Nyquist limiter: bin-owner kernels only

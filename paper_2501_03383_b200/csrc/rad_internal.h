@@ -61,6 +61,7 @@ struct AccumParams {
     int w_pad;             // W padded to the frequency tile
     int n_ftiles;          // frequency tiles per direction group
     int n_wtiles;          // warp tiles = direction groups * n_ftiles
+    int psplit;            // particle split: 2^psplit lane groups of a warp share one direction (0: off)
     const DirRec *dirs;    // [D]
     const uint32_t *F;     // [w_pad] integer part of f_j / f_unit
     const float *Ff;       // [w_pad] (float)F_j
@@ -147,6 +148,7 @@ struct Handle {
     int R = 1;                            // per-region detectors: acc is [R][D][w_pad][4]
     int lw = 32, strip = kStrip;          // lanes along frequency, bins per lane
     int n_ftiles = 0, n_wtiles = 0;
+    int psplit = 0;                       // log2 of the lane groups per direction (few-direction detectors)
     int stream_nd = 1;
     int stream_nb = 0;               // > 0: D*W <= 16 -> particle-streaming kernel with 8 or 16 bins/thread
     double dt = 0, t0 = 0, scale = 0, f_unit = 0;

@@ -129,11 +129,12 @@ __device__ __forceinline__ bool decode_task(const AccumParams &P, int warp, int 
 // m g_hs and amplitude g_master[n][m]; the sweep and the phase arithmetic are those of the general grid.
 constexpr int kDyadChain = 2;  // dyadic grids: bins per squaring chain (1 anchor + kDyadChain - 1 squarings)
 
-template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ, bool FF, bool GRID = false, int DY = 0>
+template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ, bool FF, bool GRID = false, int DY = 0, bool SPLIT = false>
 __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
 {
     static_assert(!GRID || (!UNI && !NYQ && !FF), "grid evaluation runs the plain general-grid sweep");
     static_assert(DY == 0 || (!UNI && !NYQ && !FF && !GRID), "dyadic squaring runs on the plain general-grid sweep");
+    static_assert(!SPLIT || (LW < 32 && !NYQ && !FF && !GRID && DY == 0), "particle split: plain general / uniform sweep, >= 2 lane groups");
     static_assert(!(UNI && NYQ), "the limiter runs on the general-grid kernel");
     constexpr int DPW = 32 / LW;
     // Shared-memory records are direction-major, rec[direction of the warp][particle of the batch], rows padded
@@ -159,6 +160,14 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
     const int dg = wt / P.n_ftiles, ft = wt - dg * P.n_ftiles;
     const int ld = lane / LW, lf = lane - ld * LW;
     const int jbase = ft * (LW * S) + lf;
+    // Particle split (P.psplit = PS > 0; detectors with fewer directions than a warp holds, rad_api.cu
+    // choose_tile): 2^PS lane groups share ONE direction and take every 2^PS-th record of a batch each, so no
+    // lane idles on a padded direction; their partial sums meet in a shuffle reduction before the fold.
+    const int PS = SPLIT ? P.psplit : 0;     // compile-time 0 in every other instantiation
+    const int rl = ld >> PS;                    // row of this lane's direction in the staged records
+    const int psub = ld & ((1 << PS) - 1);      // which records of a batch this lane group sweeps
+    const int dir0 = (dg * DPW) >> PS;          // first direction of the warp
+    const int n_rows = DPW >> PS;               // directions staged per warp
 
     uint32_t F[NC];
     float Ff[NC], fl[NC], acc[S][4];
@@ -173,7 +182,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
     for (int i = 0; i < S; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.0f;
     float F2r[FF ? S : 1];
     if (FF) {
-        const float *row = P.F2 + (size_t)min(dg * DPW + ld, P.n_dir - 1) * P.w_pad + jbase;
+        const float *row = P.F2 + (size_t)min(dir0 + rl, P.n_dir - 1) * P.w_pad + jbase;
 #pragma unroll
         for (int i = 0; i < S; ++i) F2r[FF ? i : 0] = __ldg(row + i * LW);
     }
@@ -225,8 +234,8 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
             const Particle p = load_particle<ST, true>(P, k, k < k1, FF);
             if (FF) ws[lane] = make_float2(p.w, p.ww);
 #pragma unroll(DPW > 2 ? 1 : DPW)  // 4 or 8 directions per warp: keep the staging code out of the register budget
-            for (int dd = 0; dd < DPW; ++dd) {
-                const int dir = min(dg * DPW + dd, P.n_dir - 1);
+            for (int dd = 0; dd < n_rows; ++dd) {
+                const int dir = min(dir0 + dd, P.n_dir - 1);
                 float4 r4;
                 float sf;
                 uint32_t T;
@@ -247,10 +256,10 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
         __syncwarp();
         if (UNI) {
 #pragma unroll 2
-            for (int kk = 0; kk < kBatch; ++kk) {  // a2': sweep with the rotation recurrence
-                const float4 r4 = rec[ld * PITCH + kk];
-                const float sf = sfs[ld * PITCH + kk];
-                const float2 rot = rots[ld * PITCH + kk];
+            for (int kk = psub; kk < kBatch; kk += 1 << PS) {  // a2': sweep with the rotation recurrence
+                const float4 r4 = rec[rl * PITCH + kk];
+                const float sf = sfs[rl * PITCH + kk];
+                const float2 rot = rots[rl * PITCH + kk];
                 float zi0, zr0;
                 phase_sincos(F[0], Ff[0], fl[0], __float_as_uint(r4.x), r4.y, sf, zi0, zr0);
                 const float2 wq = FF ? ws[kk] : make_float2(0.0f, 0.0f);
@@ -288,9 +297,9 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
             struct Rec { float4 r4; float sf; int m; float2 wq; };
             auto load_rec = [&](const int kk, const bool pred) {
                 Rec r;
-                r.r4 = rec[ld * PITCH + kk];
-                r.sf = sfs[ld * PITCH + kk];
-                r.m = pred ? jcs[ld * PITCH + kk] - lf : 0;
+                r.r4 = rec[rl * PITCH + kk];
+                r.sf = sfs[rl * PITCH + kk];
+                r.m = pred ? jcs[rl * PITCH + kk] - lf : 0;
                 r.wq = FF ? ws[kk] : make_float2(0.0f, 0.0f);
                 return r;
             };
@@ -350,24 +359,26 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 // four skippable groups of two bins: 2.23 ms -- the shorter basic blocks cost more instruction-level
                 // parallelism than the skipped bins save; 64-bin tiles (8 lanes x 8 bins): 2.42 ms.)
 #pragma unroll 1
-                for (int kk = 0; kk < kBatch; kk += 2) {
-                    const int ma = jcs[ld * PITCH + kk], mb = jcs[ld * PITCH + kk + 1];
+                for (int m2 = 0; m2 < (kBatch >> PS); m2 += 2) {
+                    const int kk = (m2 << PS) + psub, kk2 = kk + (1 << PS);
+                    const int ma = jcs[rl * PITCH + kk], mb = jcs[rl * PITCH + kk2];
                     const bool all = __all_sync(0xffffffffu, min(ma, mb) >= LW * S);
                     const bool none = __all_sync(0xffffffffu, max(ma, mb) <= 0);
                     if (all) {
-                        const Rec ra = load_rec(kk, false), rb = load_rec(kk + 1, false);
+                        const Rec ra = load_rec(kk, false), rb = load_rec(kk2, false);
                         sweep_bins(ra, kPolyEven, No{}, I0_{}, IS_{});
                         sweep_bins(rb, kPolyOdd, No{}, I0_{}, IS_{});
                     } else if (!none) {
-                        const Rec ra = load_rec(kk, true), rb = load_rec(kk + 1, true);
+                        const Rec ra = load_rec(kk, true), rb = load_rec(kk2, true);
                         sweep_bins(ra, kPolyEven, Yes{}, I0_{}, IS_{});
                         sweep_bins(rb, kPolyOdd, Yes{}, I0_{}, IS_{});
                     }
                 }
             } else {
 #pragma unroll 1
-                for (int kk = 0; kk < kBatch; kk += 2) {
-                    const Rec ra = load_rec(kk, false), rb = load_rec(kk + 1, false);
+                for (int m2 = 0; m2 < (kBatch >> PS); m2 += 2) {
+                    const int kk = (m2 << PS) + psub;
+                    const Rec ra = load_rec(kk, false), rb = load_rec(kk + (1 << PS), false);
                     sweep_bins(ra, DY > 0 ? 0 : kPolyEven, No{}, I0_{}, IS_{});   // dyadic: the XU pipe is not the bound
                     sweep_bins(rb, DY > 0 ? 0 : kPolyOdd, No{}, I0_{}, IS_{});
                 }
@@ -375,8 +386,16 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
         }
         __syncwarp();
     }
+    if (SPLIT) {  // particle split: sum the lane groups of a direction (fixed order), group 0 folds
+        for (int o = LW; o < (LW << PS); o <<= 1) {
+#pragma unroll
+            for (int i = 0; i < S; ++i)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) acc[i][c] += __shfl_xor_sync(0xffffffffu, acc[i][c], o);
+        }
+    }
     pdl_wait();  // the accumulator (and the deterministic workspace) belong to earlier work until here
-    fold<S, LW, GRID>(P, acc, dg * DPW + ld, jbase, ci, region);
+    fold<S, LW, GRID>(P, acc, psub == 0 ? dir0 + rl : P.n_dir, jbase, ci, region);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -436,10 +455,27 @@ static cudaError_t dispatch_dyadic(const Handle &h, const AccumParams &p, cudaSt
     }
 }
 
+template <typename ST, bool UNI>
+static cudaError_t dispatch_split(const Handle &h, const AccumParams &p, cudaStream_t s)
+{
+    const long long n_tasks = (long long)p.n_wtiles * p.n_chunks;
+    const dim3 grid((unsigned)((n_tasks + kWarpsPerBlock - 1) / kWarpsPerBlock));
+    switch (h.lw) {
+        case 16: return launch_kernel(rad_accum<ST, 16, kStrip, kMinBlocks, UNI, false, false, false, 0, true>, grid, dim3(kThreads), 0, s, h.overlap, p);
+        case 8: return launch_kernel(rad_accum<ST, 8, kStrip, kMinBlocks, UNI, false, false, false, 0, true>, grid, dim3(kThreads), 0, s, h.overlap, p);
+        default: return launch_kernel(rad_accum<ST, 4, kStrip, kMinBlocks, UNI, false, false, false, 0, true>, grid, dim3(kThreads), 0, s, h.overlap, p);
+    }
+}
+
 cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_f64,
                               cudaStream_t s, int *n_launches, const char **variant)
 {
     *n_launches = 1;
+    if (p.psplit > 0) {  // few directions: lane groups split the particles (rad_create allows it on the plain sweeps only)
+        *variant = h.uniform ? "uniform+split" : "general+split";
+        if (h.uniform) return state_f64 ? dispatch_split<double, true>(h, p, s) : dispatch_split<float, true>(h, p, s);
+        return state_f64 ? dispatch_split<double, false>(h, p, s) : dispatch_split<float, false>(h, p, s);
+    }
     if (h.dyad_c > 0 && !h.uniform && p.nyq_lim == 0.0 && !p.F2) {
         *variant = "general+dyadic";
         if (h.dyad_c == 1) return state_f64 ? dispatch_dyadic<double, 1>(h, p, s) : dispatch_dyadic<float, 1>(h, p, s);

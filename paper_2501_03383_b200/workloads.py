@@ -282,7 +282,13 @@ def make_workload(cfg: str) -> Workload:
         # sub-volume -> 12 sub-volumes; line 184: "spectrum observed in one direction".
         return Workload("cfg5r_regions_12x1x512", 331776, 200, 1e-17, np.array([[1.0, 0.0, 0.0]]),
                         omega_log(512), np.float32, BASE_SEED + 5, "khi", extra={"regions": (2, 6)})
+    if cfg == "5s":
+        # config 5r with a COARSER spectrum per sub-volume, 1 direction x 128 frequencies: a few-direction detector whose
+        # frequency tile (16 lanes x 8 bins) would leave half of every warp idle; the lane groups then split the
+        # particles of a batch ("particle split").  Not a BASELINE.json config.
+        return Workload("cfg5s_regions_12x1x128", 331776, 200, 1e-17, np.array([[1.0, 0.0, 0.0]]),
+                        omega_log(128), np.float32, BASE_SEED + 5, "khi", extra={"regions": (2, 6)})
     raise KeyError(cfg)
 
 
-ALL_CONFIGS = ("0", "1", "1u", "1f", "1n", "1d", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r")
+ALL_CONFIGS = ("0", "1", "1u", "1f", "1n", "1d", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r", "5s")

@@ -31,6 +31,12 @@ def assert_parity(S, S_ref, peak=None, what=""):
     return l2, mr
 
 
+def base_variant(v):
+    """Kernel variant name without the "+split" suffix (few-direction detectors: lane groups of a warp
+    share a direction and split the particles; same sweep, same results)."""
+    return v.replace("+split", "")
+
+
 def to_device(state):
     import torch
     return [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in state]
