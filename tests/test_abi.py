@@ -128,3 +128,39 @@ def test_product_path_never_touches_the_oracle():
         text = p.read_text()
         assert not re.search(r"^\s*(from|import)\s+oracle\b", text, re.M), p
         assert "rad_oracle" not in text and "_work/" not in text, p
+
+
+def _build_c_client(tmp_path):
+    import subprocess
+    from paper_2501_03383_b200 import binding, build
+    build.build()
+    exe = tmp_path / "rad_client"
+    subprocess.run(["gcc", "-std=c11", "-Wall", "-Werror", "-I", str(ROOT / "include"), str(ROOT / "examples" / "rad_client.c"),
+                    "-L", str(binding.LIB_PATH.parent), "-lrad", "-lm", "-o", str(exe)], check=True)
+    import os
+    env = dict(os.environ, LD_LIBRARY_PATH=str(binding.LIB_PATH.parent) + ":" + os.environ.get("LD_LIBRARY_PATH", ""))
+    return subprocess.run([str(exe)], capture_output=True, text=True, env=env)
+
+
+def test_c_client_compiles_against_the_header_and_fails_loudly_without_a_gpu(tmp_path):
+    """examples/rad_client.c: include/rad.h is a plain C11 header (-Wall -Werror), the program links against
+    librad.so alone (no torch, no Python, no CUDA headers), and without a CUDA device rad_create reports
+    RAD_ERR_CUDA -- no CPU fallback.  (On a GPU box the same binary runs the path: see the gpu test.)"""
+    res = _build_c_client(tmp_path)
+    try:
+        import torch
+        has_gpu = torch.cuda.is_available()
+    except Exception:
+        has_gpu = False
+    if has_gpu:
+        assert res.returncode == 0 and "rad_client OK" in res.stdout, res.stdout + res.stderr
+    else:
+        assert res.returncode == 2 and "RAD_ERR_CUDA" in res.stderr, res.stdout + res.stderr
+
+
+@pytest.mark.gpu
+def test_c_client_runs_the_abi_from_plain_c(tmp_path):
+    """The whole path (host buffers in, spectrum out) driven from plain C against a closed form."""
+    res = _build_c_client(tmp_path)
+    assert res.returncode == 0 and "rad_client OK" in res.stdout, res.stdout + res.stderr
+    print(res.stdout.strip())
