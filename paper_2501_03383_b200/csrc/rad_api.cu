@@ -1216,6 +1216,6 @@ const char *rad_status_string(rad_status s)
 
 const char *rad_last_error(const rad_handle *hh) { return hh ? hh->h.err.c_str() : g_create_error.c_str(); }
 
-const char *rad_version(void) { return "rad-b200 0.3 (sm_100a)"; }
+const char *rad_version(void) { return "rad-b200 0.4 (sm_100a)"; }
 
 }  // extern "C"
