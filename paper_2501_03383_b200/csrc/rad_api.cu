@@ -73,7 +73,7 @@ double tile_efficiency(const Handle &h, int lw, int *ps, bool allow_split)
     const int tile = lw * h.strip, dpw = 32 / lw;
     const int w_pad = (h.W + tile - 1) / tile * tile;
     *ps = 0;
-    while (allow_split && dpw > 1 && (h.D << (*ps + 1)) <= dpw) ++*ps;
+    while (allow_split && h.D <= (dpw >> (*ps + 1))) ++*ps;   // D * 2^(ps+1) <= dpw, without shifting D
     const int d_pad = *ps > 0 ? dpw : (h.D + dpw - 1) / dpw * dpw;
     return ((double)h.W / w_pad) * ((double)(h.D << *ps) / d_pad);
 }

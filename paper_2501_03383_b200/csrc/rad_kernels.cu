@@ -263,7 +263,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
         }
         __syncwarp();
         if (UNI) {
-#pragma unroll 2
+#pragma unroll 4
             for (int kk = psub; kk < kBatch; kk += 1 << PS) {  // a2': sweep with the rotation recurrence
                 const float4 r4 = rec[rl * PITCH + kk];
                 const float sf = sfs[rl * PITCH + kk];
