@@ -133,8 +133,8 @@ typedef struct {
  * Instead of W sin/cos pairs per term, every term is SPREAD onto a uniform grid in tau that the
  * handle keeps per direction (spacing h = pi / (2 w_max), i.e. twofold oversampling of the highest
  * frequency; a compactly supported "exponential of semicircle" kernel of width 4..12 grid points,
- * chosen from fast_tolerance), at a cost independent of W: about 5 vector atomics per (particle,
- * direction).  rad_spectrum / rad_amplitude then evaluate
+ * chosen from fast_tolerance), at a cost independent of W: 4 vector atomics per (particle,
+ * direction) at the default width.  rad_spectrum / rad_amplitude then evaluate
  *     A(n, w_j) = (1 / Phi(w_j)) sum_m g_m(n) exp(i w_j tau_m)
  * exactly (a direct sum over the grid points with the integer-phase sin/cos of the direct path,
  * no FFT) and divide by the kernel's Fourier transform Phi.  The result approximates the exact

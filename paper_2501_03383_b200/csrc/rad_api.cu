@@ -350,8 +350,9 @@ rad_status accumulate_gridded(Handle &h, int64_t step, int64_t n, const void *co
     p.win_type = h.win_type;
     for (int c = 0; c < 3; ++c) { p.win_o[c] = h.win_o[c]; p.win_il[c] = h.win_il[c]; }
     grid_params(h, p);
-    // direction groups whose delta rows stay L2 resident (~48 MB); the 40 B/particle are re-read per group
-    const int per = (int)std::max<long long>(1, (48LL << 20) / ((long long)h.g_M * (long long)sizeof(float2)));
+    // direction groups whose two deposit grids stay L2 resident (96 of the 126 MB); the 40 B/particle are re-read per
+    // group (measured on config 2: 24 ... 112 MB per group within 5 %, smaller groups lose to the extra launches)
+    const int per = (int)std::max<long long>(1, (96LL << 20) / ((long long)h.g_M * 2 * (long long)sizeof(float2)));
     for (int d0 = 0; d0 < h.D; d0 += per) {
         p.dir0 = d0; p.dir1 = std::min(h.D, d0 + per);
         RAD_CUDA(&h, launch_spread(h, p, h.state_f64, s));
@@ -753,7 +754,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
             M = std::max(M, (long long)std::ceil((tau_hi - tau_lo) / h_tau) + wd + 8);
         }
         M = (M + 63) / 64 * 64;
-        if ((double)M * h.D * 24.0 > 64e9) {
+        if ((double)M * h.D * 32.0 > 64e9) {
             delete hh;
             return fail(nullptr, RAD_ERR_INVALID_ARG, "RAD_FLAG_FAST_GRIDDED: the box / window needs more than 64 GB of grid");
         }
@@ -822,7 +823,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
                            cudaMalloc(&h.Fg_d, sizeof(uint32_t) * h.w_pad) == cudaSuccess &&
                            cudaMalloc(&h.Ffg_d, sizeof(float) * h.w_pad) == cudaSuccess &&
                            cudaMalloc(&h.flg_d, sizeof(float) * h.w_pad) == cudaSuccess &&
-                           cudaMalloc(&h.g_delta_d, sizeof(float2) * (size_t)h.D * h.g_M) == cudaSuccess &&
+                           cudaMalloc(&h.g_delta_d, sizeof(float2) * 2 * (size_t)h.D * h.g_M) == cudaSuccess &&
                            cudaMalloc(&h.g_master_d, sizeof(double2) * (size_t)h.D * h.g_M) == cudaSuccess &&
                            cudaMalloc(&h.g_oob_d, sizeof(unsigned long long)) == cudaSuccess));
     if (!ok) {
@@ -840,7 +841,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
                       cudaMemcpy(h.Fg_d, Fg.data(), sizeof(uint32_t) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
                       cudaMemcpy(h.Ffg_d, Ffg.data(), sizeof(float) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
                       cudaMemcpy(h.flg_d, flg.data(), sizeof(float) * h.w_pad, cudaMemcpyHostToDevice) == cudaSuccess &&
-                      cudaMemset(h.g_delta_d, 0, sizeof(float2) * (size_t)h.D * h.g_M) == cudaSuccess &&
+                      cudaMemset(h.g_delta_d, 0, sizeof(float2) * 2 * (size_t)h.D * h.g_M) == cudaSuccess &&
                       cudaMemset(h.g_master_d, 0, sizeof(double2) * (size_t)h.D * h.g_M) == cudaSuccess &&
                       cudaMemset(h.g_oob_d, 0, sizeof(unsigned long long)) == cudaSuccess)) &&
          (!h.F2_d || cudaMemcpy(h.F2_d, h.F2_h.data(), sizeof(float) * h.F2_h.size(), cudaMemcpyHostToDevice) == cudaSuccess) &&
@@ -1174,7 +1175,7 @@ rad_status rad_reset(rad_handle *hh, void *cuda_stream)
                                  (cudaStream_t)cuda_stream));
     if (h.fast) {
         cudaStream_t s = (cudaStream_t)cuda_stream;
-        RAD_CUDA(&h, cudaMemsetAsync(h.g_delta_d, 0, sizeof(float2) * (size_t)h.D * h.g_M, s));
+        RAD_CUDA(&h, cudaMemsetAsync(h.g_delta_d, 0, sizeof(float2) * 2 * (size_t)h.D * h.g_M, s));
         RAD_CUDA(&h, cudaMemsetAsync(h.g_master_d, 0, sizeof(double2) * (size_t)h.D * h.g_M, s));
         RAD_CUDA(&h, cudaMemsetAsync(h.g_oob_d, 0, sizeof(unsigned long long), s));
         h.g_pending = 0;

@@ -17,8 +17,8 @@
 // Mapping: thread <-> particle (coalesced SoA loads, state read once), loop over the directions of
 // the launch; per (particle, direction): the fp64 phase and Doppler factor and the fp32 transverse
 // amplitude of the direct path (stage_record), WD + 2 kernel values (FFMA, MUFU.SQRT, FFMA,
-// MUFU.EX2 each), and (WD + 2) / 2 16-byte vector reductions red.global.add.v4.f32 (SASS
-// REDG.E.ADD.F32x4) of {a1 phi_m, a2 phi_m, a1 phi_m+1, a2 phi_m+1} into the fp32 delta grid.
+// MUFU.EX2 each), and WD / 2 16-byte vector reductions red.global.add.v4.f32 (SASS
+// REDG.E.ADD.F32x4) of {a1 phi_m, a2 phi_m, a1 phi_m+1, a2 phi_m+1} into one of the two fp32 delta grids.
 // A fold kernel adds the delta grid into the fp64 master grid after every call: the low-frequency
 // (coherent) part of the signal makes all deposits of a grid point equal in sign, and the rounding
 // of thousands of fp32 additions onto such a point shows up in the dark high-frequency bins
@@ -44,13 +44,12 @@ template <typename ST, int WD>
 __global__ void __launch_bounds__(kSpreadThreads) rad_spread(const AccumParams P)
 {
     static_assert(WD % 2 == 0 && WD >= 4 && WD <= 12, "kernel width");
-    constexpr int NP = WD + 2;  // deposited points: an even start index, the outermost ones carry phi = 0
     constexpr float kInvHalf = 2.0f / WD;
     pdl_trigger();
     const long long k = (long long)blockIdx.x * kSpreadThreads + threadIdx.x;
     const bool valid = k < P.n_particles;
     const Particle p = load_particle<ST, true>(P, valid ? k : 0, valid, false);
-    pdl_wait();  // the delta grid belongs to earlier work (a fold zeroes it) until here
+    pdl_wait();  // the delta grids belong to earlier work (a fold zeroes them) until here
     if (!valid) return;
     unsigned long long lost = 0;
     for (int dir = P.dir0; dir < P.dir1; ++dir) {
@@ -67,18 +66,17 @@ __global__ void __launch_bounds__(kSpreadThreads) rad_spread(const AccumParams P
         const float inv = 1.0f / d;
         const float pre = -p.wdt * inv * inv;
         const float a1 = pre * fmaf(e1b, g, e1d * d), a2 = pre * fmaf(e2b, g, e2d * d);
-        // grid coordinate u (fp64), first point inside the support, rounded down to an even index
+        // grid coordinate u (fp64); the support |m - u| < WD/2 holds the WD points m_first ... m_first + WD - 1
         const double u = fma(s32, P.g_ihs, -__ldg(P.g_s0 + dir));  // tau / h - (index of grid point 0)
         const long long m_first = (long long)floor(u - 0.5 * WD) + 1;
-        const long long m0 = m_first & ~1LL;
-        if (m0 < 0 || m0 + NP >= P.g_M) {  // outside the box / window given at rad_create (the last point stays 0)
+        if (m_first < 1 || m_first + WD >= P.g_M) {  // outside the box / window given at rad_create
             ++lost;
             continue;
         }
-        const float x0 = to_f32((double)m0 - u) * kInvHalf;  // x of point m0, in [-1 - 4/WD, -1 + 2/WD)
-        float phi[NP];
+        const float x0 = to_f32((double)m_first - u) * kInvHalf;  // x of point m_first, in (-1, -1 + 2/WD]
+        float phi[WD];
 #pragma unroll
-        for (int i = 0; i < NP; ++i) {
+        for (int i = 0; i < WD; ++i) {
             const float x = fmaf((float)i, kInvHalf, x0);
             const float t = fmaf(-x, x, 1.0f);
             // correctly rounded square root: beta multiplies its error (sqrt.approx's 2^-22 would put a
@@ -88,25 +86,45 @@ __global__ void __launch_bounds__(kSpreadThreads) rad_spread(const AccumParams P
             asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(P.g_beta2 * (sq - 1.0f)));
             phi[i] = t > 0.0f ? e : 0.0f;
         }
-        float2 *row = P.g_delta + (size_t)dir * P.g_M + m0;
+        // WD / 2 16-byte reductions, never a half-empty one: a 16-byte chunk holds two consecutive grid points,
+        // and there are TWO deposit grids per direction, one whose chunks start at even points and one whose
+        // chunks start at odd points (stored one point to the left); the term goes to the grid whose chunk
+        // boundaries coincide with its first point.  (The kernel is bound by the rate at which L2 takes these
+        // reductions: a single even-aligned grid needs WD/2 + 1 chunks for every second term, measured 5.67 ms
+        // per config-2 step with 4.5 chunks per term on average, 6.31 ms with 5.)
+        const int odd = (int)(m_first & 1);
+        float2 *row = P.g_delta + ((size_t)dir * 2 + odd) * P.g_M + (m_first - odd);
 #pragma unroll
-        for (int i = 0; i < NP; i += 2) red_add_v4(row + i, a1 * phi[i], a2 * phi[i], a1 * phi[i + 1], a2 * phi[i + 1]);
+        for (int i = 0; i < WD; i += 2) red_add_v4(row + i, a1 * phi[i], a2 * phi[i], a1 * phi[i + 1], a2 * phi[i + 1]);
     }
     if (lost) atomicAdd(P.g_oob, lost);
 }
 
-// master += delta, delta := 0 (fp32 partial sums never grow beyond a few calls)
-__global__ void rad_grid_fold_kernel(double2 *__restrict__ master, float2 *__restrict__ delta, long long n)
+// master += even-aligned deposits + odd-aligned deposits (stored one point to the left); both := 0
+// (fp32 partial sums never grow beyond one call)
+__global__ void rad_grid_fold_kernel(double2 *__restrict__ master, float2 *__restrict__ delta, int M, long long n)
 {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const float2 dl = delta[i];
-    if (dl.x != 0.0f || dl.y != 0.0f) {
-        double2 m = master[i];
-        m.x += (double)dl.x;
-        m.y += (double)dl.y;
-        master[i] = m;
-        delta[i] = make_float2(0.0f, 0.0f);
+    const long long dir = i / M;
+    const int m = (int)(i - dir * M);
+    float2 *ev = delta + (size_t)dir * 2 * M, *od = ev + M;
+    float2 dl = ev[m];
+    const bool he = dl.x != 0.0f || dl.y != 0.0f;
+    bool ho = false;
+    if (m > 0) {
+        const float2 q = od[m - 1];
+        ho = q.x != 0.0f || q.y != 0.0f;
+        dl.x += q.x;
+        dl.y += q.y;
+    }
+    if (he || ho) {
+        double2 mm = master[i];
+        mm.x += (double)dl.x;
+        mm.y += (double)dl.y;
+        master[i] = mm;
+        if (he) ev[m] = make_float2(0.0f, 0.0f);
+        if (ho) od[m - 1] = make_float2(0.0f, 0.0f);
     }
 }
 
@@ -133,7 +151,7 @@ cudaError_t launch_spread(const Handle &h, const AccumParams &p, bool state_f64,
 cudaError_t launch_grid_fold(const Handle &h, cudaStream_t s)
 {
     const long long n = (long long)h.D * h.g_M;
-    rad_grid_fold_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(h.g_master_d, h.g_delta_d, n);
+    rad_grid_fold_kernel<<<(unsigned)((n + 255) / 256), 256, 0, s>>>(h.g_master_d, h.g_delta_d, h.g_M, n);
     return cudaGetLastError();
 }
 

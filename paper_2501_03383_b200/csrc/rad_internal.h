@@ -88,7 +88,8 @@ struct AccumParams {
     DirRec sdir[2];
     // fast gridded path (rad_gridded.cu; rad.h RAD_FLAG_FAST_GRIDDED): per direction a uniform grid in
     // retarded time, point m at tau = (g_s0[dir] + m) h, h = g_hs in s32 units (s32 = tau f_unit 2^32)
-    float2 *g_delta;             // [D][g_M] fp32 (A1, A2) deposits since the last fold
+    float2 *g_delta;             // [D][2][g_M] fp32 (A1, A2) deposits since the last fold: chunks starting at
+                                 // even points, and chunks starting at odd points (stored one point to the left)
     const double2 *g_master;     // [D][g_M] fp64 grid (evaluation reads it)
     const double *g_s0;          // [D] index of grid point 0 in units of h: tau_m = (g_s0[n] + m) h (integers)
     const double2 *g_corr;       // [w_pad] complex 1 / (Phi(w_j) (1 - exp(i w_j h))): deconvolution of the
