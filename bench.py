@@ -258,6 +258,7 @@ def alu_peaks(device, sm_mhz_hint):
         "dfma_per_clk_sm": g("dfma"),
         "f2f_f32_from_f64_per_clk_sm": g("f2f_f32_from_f64"), "f2f_f64_from_f32_per_clk_sm": g("f2f_f64_from_f32"),
         "imad_per_clk_sm": g("imad"),
+        "red_v4_f32_per_clk_sm": g("red_v4_f32"), "red_v4_f32_gops": res["red_v4_f32"]["gops"],
         "sincos_pairs_gops": res["sincos_pairs"]["gops"], "ffma_gops": res["ffma"]["gops"],
         "sm_mhz": sm_mhz_hint,
         "how": "librad_ubench.so (csrc/rad_ubench.cu): 8 independent chains per thread, loop unrolled 4x, 4 x 256 threads "
@@ -541,8 +542,21 @@ def measure_fast(cfg, K, W, args, ctx):
                                        "spectrum_every_100_steps": updates * 100 / ((100 * ms_acc + ms_spec) * 1e-3) / 1e9,
                                        "spectrum_every_step": updates / ((ms_acc + ms_spec) * 1e-3) / 1e9},
            "gpu_launches": int(launches), "kernel": "rad_spread + rad_grid_fold (per step), rad_accum<GRID> (per spectrum)",
+           "roofline": None,
            "note": "effective = direct-sum updates this replaces / time; an approximation (gridding tolerance 1e-6), "
                    "checked against the exact oracle with the exact path's tolerances"}
+    # the spreading kernel is bound by the rate at which L2 takes its 16-byte vector reductions: WD/2 = 4 per
+    # (particle, direction) term at the default width; peak = the measured rate of the same instruction on
+    # scattered places of an L2-resident buffer (alu_peaks red_v4_f32)
+    pk = ctx.get("alu_peaks") or {}
+    red_per_s = n * w.n_dir * 4 / (ms_acc * 1e-3) / 1e9
+    if pk.get("red_v4_f32_gops"):
+        out["roofline"] = {"bound": "l2-reductions", "achieved": red_per_s, "peak": pk["red_v4_f32_gops"],
+                           "unit": "G red.v4.f32/s", "frac": red_per_s / pk["red_v4_f32_gops"],
+                           "kernel": "rad_spread (+ rad_grid_fold)", "reductions_per_term": 4,
+                           "peak_how": "alu_peaks red_v4_f32 (csrc/rad_ubench.cu): the same instruction, runs of 4 consecutive "
+                                       "chunks at scattered places of a 64 MB L2-resident buffer, CUDA events; the kernel's own "
+                                       "deposits are denser (tens of terms per grid point and step), so it can exceed this figure"}
     if not args.no_cpu_baseline:
         out["parity"] = parity_vs_oracle(w, n, states_np, ring, W + K, S, budget_updates=5.0e8)
     det.close()

@@ -42,7 +42,9 @@ enum Kind {
     K_FFMA2_VAR = 10,   // fma.rn.f32x2 whose three operands are all different, changing registers: INSTRUCTIONS
     K_FFMA2_BCAST = 11, // fma.rn.f32x2 with one operand a broadcast scalar (SASS Rn.F32), as the uniform-grid sweep issues it
     K_FFMA_VAR = 12,    // fma.rn.f32 whose three operands are all different, changing registers
-    K_COUNT = 13
+    K_RED_V4 = 13,      // red.global.add.v4.f32 (16-byte vector reduction), runs of 4 consecutive chunks at scattered places of a 64 MB, L2-resident
+                        // buffer: the rate at which L2 takes the reductions of the fast gridded path's spreading kernel
+    K_COUNT = 14
 };
 
 template <int KIND>
@@ -122,13 +124,48 @@ __global__ void __launch_bounds__(kThreads) pipe_kernel(float *out, float a, flo
     }
 }
 
+// 16-byte vector reductions to pseudo-random 16-byte-aligned places of buf[n_chunks] (n_chunks a power of two)
+__global__ void __launch_bounds__(kThreads) red_kernel(float4 *buf, unsigned n_mask, long long *clk)
+{
+    unsigned x = (blockIdx.x * kThreads + threadIdx.x) * 2654435761u + 12345u;
+    const long long t0 = clock64();
+#pragma unroll 1
+    for (int it = 0; it < kIters / 4; ++it) {
+#pragma unroll
+        for (int i = 0; i < kChains; i += 4) {  // runs of four consecutive chunks from a random chunk, as the spreading kernel issues them
+            x = x * 1664525u + 1013904223u;
+            float4 *q = buf + ((x >> 7) & n_mask);
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+                asm volatile("red.global.v4.f32.add [%0], {%1, %1, %1, %1};" ::"l"(q + c), "f"(1.0f) : "memory");
+        }
+    }
+    const long long t1 = clock64();
+    if ((threadIdx.x & 31) == 0) {
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        if (smid < kMaxSmid) {
+            atomicMin(clk + smid, t0);
+            atomicMax(clk + kMaxSmid + smid, t1);
+            atomicAdd(reinterpret_cast<unsigned long long *>(clk + 2 * kMaxSmid + smid), 1ull);
+        }
+    }
+}
+
 template <int KIND>
 int run_kind(int n_sm, int blocks_per_sm, int reps, double *per_clk_sm, double *gops)
 {
     const int grid = n_sm * blocks_per_sm;
     float *out = nullptr;
     long long *clk = nullptr;
-    if (cudaMalloc(&out, (size_t)grid * kThreads * sizeof(float)) != cudaSuccess) return 1;
+    constexpr unsigned kRedChunks = 1u << 22;  // x 16 B = 64 MB
+    const int iters = KIND == K_RED_V4 ? kIters / 4 : kIters;
+    if (cudaMalloc(&out, KIND == K_RED_V4 ? (size_t)(kRedChunks + 4) * 16 : (size_t)grid * kThreads * sizeof(float)) != cudaSuccess) return 1;
+    if (KIND == K_RED_V4) cudaMemset(out, 0, (size_t)kRedChunks * 16);
+    auto launch = [&]() {
+        if (KIND == K_RED_V4) red_kernel<<<grid, kThreads>>>(reinterpret_cast<float4 *>(out), kRedChunks - 1, clk);
+        else pipe_kernel<KIND><<<grid, kThreads>>>(out, 1.0001f, 0.5f, clk);
+    };
     const size_t clk_bytes = (size_t)3 * kMaxSmid * sizeof(long long);
     if (cudaMalloc(&clk, clk_bytes) != cudaSuccess) { cudaFree(out); return 1; }
     long long *h = new long long[3 * kMaxSmid];
@@ -140,14 +177,14 @@ int run_kind(int n_sm, int blocks_per_sm, int reps, double *per_clk_sm, double *
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
     reset_clk();
-    for (int r = 0; r < 2; ++r) pipe_kernel<KIND><<<grid, kThreads>>>(out, 1.0001f, 0.5f, clk);  // warm-up
+    for (int r = 0; r < 2; ++r) launch();  // warm-up
     cudaDeviceSynchronize();
     reset_clk();
-    pipe_kernel<KIND><<<grid, kThreads>>>(out, 1.0001f, 0.5f, clk);  // the launch the per-SM cycle windows are read from
+    launch();  // the launch the per-SM cycle windows are read from
     int rc = cudaDeviceSynchronize() == cudaSuccess ? 0 : 2;
     if (cudaMemcpy(h, clk, clk_bytes, cudaMemcpyDeviceToHost) != cudaSuccess) rc = 2;
     cudaEventRecord(e0);
-    for (int r = 0; r < reps; ++r) pipe_kernel<KIND><<<grid, kThreads>>>(out, 1.0001f, 0.5f, clk);
+    for (int r = 0; r < reps; ++r) launch();
     cudaEventRecord(e1);
     if (cudaDeviceSynchronize() != cudaSuccess) rc = 2;
     float ms = 0.0f;
@@ -156,10 +193,10 @@ int run_kind(int n_sm, int blocks_per_sm, int reps, double *per_clk_sm, double *
     int used = 0;
     for (int i = 0; i < kMaxSmid; ++i) {
         const double warps = (double)h[2 * kMaxSmid + i], cyc = (double)(h[kMaxSmid + i] - h[i]);
-        if (warps > 0.0 && cyc > 0.0) { rate += warps * 32.0 * kIters * kChains / cyc; ++used; }
+        if (warps > 0.0 && cyc > 0.0) { rate += warps * 32.0 * iters * kChains / cyc; ++used; }
     }
     delete[] h;
-    const double ops_per_sm = (double)kIters * kChains * kThreads * blocks_per_sm;  // thread-level results
+    const double ops_per_sm = (double)iters * kChains * kThreads * blocks_per_sm;  // thread-level results
     *per_clk_sm = used ? rate / used : 0.0;
     *gops = ms > 0.0f ? ops_per_sm * n_sm * reps / (ms * 1e-3) / 1e9 : 0.0;
     cudaEventDestroy(e0);
@@ -180,7 +217,7 @@ __attribute__((visibility("default"))) const char *rad_ubench_name(int kind)
 {
     static const char *names[K_COUNT] = {"ffma", "ffma_imm", "ffma2_instr", "mufu_sin", "sincos_pairs",
                                          "mufu_ex2", "dfma", "f2f_f32_from_f64", "f2f_f64_from_f32", "imad",
-                                         "ffma2_var_instr", "ffma2_bcast_instr", "ffma_var"};
+                                         "ffma2_var_instr", "ffma2_bcast_instr", "ffma_var", "red_v4_f32"};
     return kind >= 0 && kind < K_COUNT ? names[kind] : "?";
 }
 
@@ -209,6 +246,7 @@ __attribute__((visibility("default"))) int rad_ubench_run(int device, int kind, 
         case K_FFMA2_VAR: return run_kind<K_FFMA2_VAR>(n_sm, blocks_per_sm, reps, per_clk_sm, gops);
         case K_FFMA2_BCAST: return run_kind<K_FFMA2_BCAST>(n_sm, blocks_per_sm, reps, per_clk_sm, gops);
         case K_FFMA_VAR: return run_kind<K_FFMA_VAR>(n_sm, blocks_per_sm, reps, per_clk_sm, gops);
+        case K_RED_V4: return run_kind<K_RED_V4>(n_sm, blocks_per_sm, reps, per_clk_sm, gops);
     }
     return 1;
 }
