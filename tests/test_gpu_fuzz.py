@@ -117,6 +117,9 @@ def test_random_case_matches_oracle(oracle_mod, case):
                 assert np.all(row == 0.0), what
     else:
         assert np.all(S == 0.0), what
+    if ref.max() > 0:
+        rows = [(S.reshape(-1, c["W"])[k], ref.reshape(-1, c["W"])[k]) for k in range(S.reshape(-1, c["W"]).shape[0])]
+        print(f"{what}: maxrel {P.max_rel(S, ref):.2e} worst row {max(P.max_rel(a, b) for a, b in rows if b.max() > 0):.2e}")
     if "nyquist" in c["opts"]:                              # the keep/drop decision is exact: identical zero sets
         assert np.array_equal(S == 0.0, ref == 0.0), what
 
@@ -152,4 +155,5 @@ def test_random_case_fast_gridded_matches_exact_oracle(oracle_mod, case):
         torch.cuda.synchronize()
         S = det.spectrum()
         assert det.kernel_variant == "gridded"
-    P.assert_parity(S, o.spectrum(), what=f"fuzz fast {case}: {D}x{W} {kind} {np.dtype(dtype).name} n={n} T={T} t0={t_first}")
+    l2, mr = P.assert_parity(S, o.spectrum(), what=f"fuzz fast {case}: {D}x{W} {kind} {np.dtype(dtype).name} n={n} T={T} t0={t_first}")
+    print(f"fuzz fast {case}: {D}x{W} {kind} {np.dtype(dtype).name} n={n} T={T}: relL2 {l2:.2e} maxrel {mr:.2e}")
