@@ -214,18 +214,22 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": el / max(args.steps, 1) * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": workload_config(w, n, 1, None, None),
+        "data": "synthetic", "config": workload_config(w, n, 1),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }))
 
 
-def workload_config(w, n, world, flags, l2):
-    """The `config` object: the same keys in both arms (the reference arm leaves the GPU-only ones null)."""
+def workload_config(w, n, world):
+    """The `config` object: the workload, identical in both arms (what is specific to the GPU run -- handle flags,
+    ring size -- is reported under "launch")."""
     return {"workload": w.name, "n_particles_per_gpu": n, "n_regions": w.n_regions, "n_dir": w.n_dir,
             "n_omega": w.n_omega, "state_dtype": np.dtype(w.state_dtype).name,
-            "parallelism": f"particle-shard x{world}", "flags": flags, "l2": l2}
+            "parallelism": f"particle-shard x{world}",
+            "l2": "GPU arm: the timed steps cycle through a ring of distinct PIC steps that is either one input per step "
+                  "or larger than twice the L2, after an L2 flush (a 252 MiB fill) before the timed region; CPU arm: not "
+                  "applicable"}
 
 
 # ------------------------------------------------------------------------------ our arm
@@ -418,9 +422,10 @@ def measure(cfg, K, W, args, ctx, headline):
 
     out = {"value": value, "unit": UNIT, "steps": K, "warmup": W, "ms_per_step": ms_total / K,
            "kernel": f"rad_accum_{variant}", "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
-           "config": workload_config(w, n, world, "none" if args.no_overlap else "RAD_FLAG_OVERLAP_STEPS",
-                                     f"ring of {ring} distinct step inputs ({ring * bytes_per_step / 2**20:.0f} MiB) + "
-                                     f"L2 flush before the timed region")}
+           "config": workload_config(w, n, world),
+           "launch": {"flags": "none" if args.no_overlap else "RAD_FLAG_OVERLAP_STEPS",
+                      "l2": f"ring of {ring} distinct step inputs ({ring * bytes_per_step / 2**20:.0f} MiB) + "
+                            f"L2 flush before the timed region"}}
 
     # parity of what the timed region computed (outside the timed region; rank 0's own shard)
     if world == 1 and not args.no_cpu_baseline:
@@ -612,7 +617,7 @@ def run_ours(args):
             "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32 phase/amplitude, f64 set-up and accumulators", "data": "synthetic",
-            "config": head["config"], "clocks": head["clocks"], "e2e": head.get("e2e"),
+            "config": head["config"], "launch": head["launch"], "clocks": head["clocks"], "e2e": head.get("e2e"),
             "gpu_launches": head["gpu_launches"], "roofline": head["roofline"],
             "cpu_baseline": head.get("cpu_baseline"), "parity": head.get("parity"),
             "multi_step": head.get("multi_step"), "alu_peaks": ctx["alu_peaks"], "configs": legs,
