@@ -249,7 +249,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 uint32_t T;
                 double d64;
                 float inv_d;
-                stage_record(p, P.dirs[dir], ts32, r4, sf, &T, &d64, &inv_d);
+                stage_record<(DPW == 1 && !UNI && !NYQ && DY == 0)>(p, P.dirs[dir], ts32, r4, sf, &T, &d64, &inv_d);
                 rec[dd * PITCH + lane] = r4;
                 sfs[dd * PITCH + lane] = sf;
                 // bins below the cut-off, relative to the first bin of the warp's frequency tile
