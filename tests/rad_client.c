@@ -7,7 +7,7 @@
  *   S(n, w) = scale w_k^2 (|b|^2 - (n.b)^2) dt^2 sin^2(w T dt / 2) / sin^2(w dt / 2)
  *
  * Build and run (tests/test_abi.py::test_c_client_runs_the_abi_from_plain_c does exactly this):
- *   gcc -std=c11 -I include examples/rad_client.c -L paper_2501_03383_b200 -lrad -lm -o rad_client
+ *   gcc -std=c11 -I include tests/rad_client.c -L paper_2501_03383_b200 -lrad -lm -o rad_client
  *   LD_LIBRARY_PATH=paper_2501_03383_b200 ./rad_client
  * Exit code 0 and a line "rad_client OK ..." on success.
  */

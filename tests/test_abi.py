@@ -135,7 +135,7 @@ def _build_c_client(tmp_path):
     from paper_2501_03383_b200 import binding, build
     build.build()
     exe = tmp_path / "rad_client"
-    subprocess.run(["gcc", "-std=c11", "-Wall", "-Werror", "-I", str(ROOT / "include"), str(ROOT / "examples" / "rad_client.c"),
+    subprocess.run(["gcc", "-std=c11", "-Wall", "-Werror", "-I", str(ROOT / "include"), str(ROOT / "tests" / "rad_client.c"),
                     "-L", str(binding.LIB_PATH.parent), "-lrad", "-lm", "-o", str(exe)], check=True)
     import os
     env = dict(os.environ, LD_LIBRARY_PATH=str(binding.LIB_PATH.parent) + ":" + os.environ.get("LD_LIBRARY_PATH", ""))
@@ -143,7 +143,7 @@ def _build_c_client(tmp_path):
 
 
 def test_c_client_compiles_against_the_header_and_fails_loudly_without_a_gpu(tmp_path):
-    """examples/rad_client.c: include/rad.h is a plain C11 header (-Wall -Werror), the program links against
+    """tests/rad_client.c: include/rad.h is a plain C11 header (-Wall -Werror), the program links against
     librad.so alone (no torch, no Python, no CUDA headers), and without a CUDA device rad_create reports
     RAD_ERR_CUDA -- no CPU fallback.  (On a GPU box the same binary runs the path: see the gpu test.)"""
     res = _build_c_client(tmp_path)
