@@ -307,7 +307,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
         } else {
             // a2: sweep.  Hybrid: of every two particles, kPolyEven / kPolyOdd of the S bins take
             // the FMA-pipe polynomial sincos instead of MUFU.SIN/COS (balances XU against issue).
-            // One staged record against bins [I0, I1) of the strip.  PRED (limiter only): the four FMAs of
+            // One staged record against the S bins of the strip.  PRED (limiter only): the four FMAs of
             // bin i are predicated on "bin below this record's cut-off" (bins i*LW < m of the strip are kept).
             struct Rec { float4 r4; float sf; int m; float2 wq; };
             auto load_rec = [&](const int kk, const bool pred) {
@@ -318,15 +318,14 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 r.wq = FF ? ws[kk] : make_float2(0.0f, 0.0f);
                 return r;
             };
-            auto sweep_bins = [&](const Rec &r, const int n_poly, auto pred_tag, auto i0_tag, auto i1_tag) {
+            auto sweep_bins = [&](const Rec &r, const int n_poly, auto pred_tag) {
                 constexpr bool PRED = decltype(pred_tag)::value;
-                constexpr int I0 = decltype(i0_tag)::value, I1 = decltype(i1_tag)::value;
                 const float4 r4 = r.r4;
                 const float sf = r.sf;
                 const uint32_t T = __float_as_uint(r4.x);
                 float zs[S], zc[S];  // DY: the strip's (sin, cos), bin i + DY squares bin i
 #pragma unroll
-                for (int i = I0; i < I1; ++i) {
+                for (int i = 0; i < S; ++i) {
                     float sn, cs;
                     if (DY > 0 && (i / (DY > 0 ? DY : 1)) % kDyadChain != 0) {
                         const float ps = zs[i >= DY ? i - DY : 0], pc = zc[i >= DY ? i - DY : 0];
@@ -368,8 +367,6 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
             };
             using No = std::false_type;
             using Yes = std::true_type;
-            using I0_ = std::integral_constant<int, 0>;
-            using IS_ = std::integral_constant<int, S>;
             if constexpr (NYQ) {
                 // Two records per turn, as in the plain sweep.  Per pair of records the warp takes one of three
                 // paths: every bin of the tile below the cut-off of every direction of the warp -> the plain sweep;
@@ -385,12 +382,12 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                     const bool none = __all_sync(0xffffffffu, max(ma, mb) <= 0);
                     if (all) {
                         const Rec ra = load_rec(kk, false), rb = load_rec(kk2, false);
-                        sweep_bins(ra, kPolyEven, No{}, I0_{}, IS_{});
-                        sweep_bins(rb, kPolyOdd, No{}, I0_{}, IS_{});
+                        sweep_bins(ra, kPolyEven, No{});
+                        sweep_bins(rb, kPolyOdd, No{});
                     } else if (!none) {
                         const Rec ra = load_rec(kk, true), rb = load_rec(kk2, true);
-                        sweep_bins(ra, kPolyEven, Yes{}, I0_{}, IS_{});
-                        sweep_bins(rb, kPolyOdd, Yes{}, I0_{}, IS_{});
+                        sweep_bins(ra, kPolyEven, Yes{});
+                        sweep_bins(rb, kPolyOdd, Yes{});
                     }
                 }
             } else {
@@ -398,8 +395,8 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 for (int m2 = 0; m2 < (kBatch >> PS); m2 += 2) {
                     const int kk = (m2 << PS) + psub;
                     const Rec ra = load_rec(kk, false), rb = load_rec(kk + (1 << PS), false);
-                    sweep_bins(ra, DY > 0 ? 0 : kPolyEven, No{}, I0_{}, IS_{});   // dyadic: the XU pipe is not the bound
-                    sweep_bins(rb, DY > 0 ? 0 : kPolyOdd, No{}, I0_{}, IS_{});
+                    sweep_bins(ra, DY > 0 ? 0 : kPolyEven, No{});   // dyadic: the XU pipe is not the bound
+                    sweep_bins(rb, DY > 0 ? 0 : kPolyOdd, No{});
                 }
             }
         }
