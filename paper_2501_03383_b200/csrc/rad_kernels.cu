@@ -249,7 +249,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 uint32_t T;
                 double d64;
                 float inv_d;
-                stage_record<(DPW == 1 && !UNI && !NYQ && DY == 0)>(p, P.dirs[dir], ts32, r4, sf, &T, &d64, &inv_d);
+                stage_record<(DPW == 1 && !UNI && DY == 0)>(p, P.dirs[dir], ts32, r4, sf, &T, &d64, &inv_d);
                 rec[dd * PITCH + lane] = r4;
                 sfs[dd * PITCH + lane] = sf;
                 // bins below the cut-off, relative to the first bin of the warp's frequency tile
@@ -307,8 +307,9 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
         } else {
             // a2: sweep.  Hybrid: of every two particles, kPolyEven / kPolyOdd of the S bins take
             // the FMA-pipe polynomial sincos instead of MUFU.SIN/COS (balances XU against issue).
-            // One staged record against the S bins of the strip.  PRED (limiter only): the four FMAs of
-            // bin i are predicated on "bin below this record's cut-off" (bins i*LW < m of the strip are kept).
+            // One staged record against the S bins of the strip.  Limiter only: bins [0, KLO) are accumulated
+            // unconditionally, the four FMAs of a bin in [KLO, KHI) are predicated on "bin below this record's
+            // cut-off" (bins i*LW < m of the strip are kept), bins [KHI, S) are not computed at all.
             struct Rec { float4 r4; float sf; int m; float2 wq; };
             auto load_rec = [&](const int kk, const bool pred) {
                 Rec r;
@@ -318,14 +319,14 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 r.wq = FF ? ws[kk] : make_float2(0.0f, 0.0f);
                 return r;
             };
-            auto sweep_bins = [&](const Rec &r, const int n_poly, auto pred_tag) {
-                constexpr bool PRED = decltype(pred_tag)::value;
+            auto sweep_bins = [&](const Rec &r, const int n_poly, auto klo_tag, auto khi_tag) {
+                constexpr int KLO = decltype(klo_tag)::value, KHI = decltype(khi_tag)::value;
                 const float4 r4 = r.r4;
                 const float sf = r.sf;
                 const uint32_t T = __float_as_uint(r4.x);
                 float zs[S], zc[S];  // DY: the strip's (sin, cos), bin i + DY squares bin i
 #pragma unroll
-                for (int i = 0; i < S; ++i) {
+                for (int i = 0; i < (KHI < S ? KHI : S); ++i) {
                     float sn, cs;
                     if (DY > 0 && (i / (DY > 0 ? DY : 1)) % kDyadChain != 0) {
                         const float ps = zs[i >= DY ? i - DY : 0], pc = zc[i >= DY ? i - DY : 0];
@@ -344,7 +345,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                         sn *= g;
                         cs *= g;
                     }
-                    if (PRED) {
+                    if (i >= KLO) {
                         // limiter: one SETP + four predicated FFMAs written in PTX, so that the
                         // compiler keeps the bins' instruction streams interleaved (as C++ it
                         // sinks each bin's sincos into a branch of its own: 2.07 -> 3.08 ms)
@@ -365,29 +366,52 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                     }
                 }
             };
-            using No = std::false_type;
-            using Yes = std::true_type;
+            using KS = std::integral_constant<int, S>;
             if constexpr (NYQ) {
-                // Two records per turn, as in the plain sweep.  Per pair of records the warp takes one of three
-                // paths: every bin of the tile below the cut-off of every direction of the warp -> the plain sweep;
-                // every bin above -> nothing to do; else predicated.  (Measured on config 1 with nu = 1, 2.26 ms
-                // when every record is predicated: 2.20 ms with these paths; splitting the predicated strip into
-                // four skippable groups of two bins: 2.23 ms -- the shorter basic blocks cost more instruction-level
-                // parallelism than the skipped bins save; 64-bin tiles (8 lanes x 8 bins): 2.42 ms.)
+                // The cut-offs of a batch's records lie close together (the Doppler factor moves them by a few
+                // per cent): per BATCH the warp finds their range, [mn, mx) relative to the tile's first bin, and
+                // runs the batch with the bins below every cut-off unconditional (klo = mn / LW bins of the strip:
+                // the bins of a strip are LW apart, "bin i of every lane" is a block of LW frequencies), the
+                // next two predicated and the rest not computed -- one of S + 1 straight-line sweeps, so nothing
+                // inside a sweep branches.  A batch whose cut-offs span more than two blocks runs fully predicated.
+                // (History, config 1 with nu = 1: every record predicated 2.26 ms; all / none / predicated paths
+                // per pair of records 2.20 ms; skippable 2-bin groups inside the predicated strip 2.23 ms; 64-bin
+                // tiles 2.42 ms.)
+                int mn = jcs[lane], mx = mn;
+                for (int dd = 1; dd < n_rows; ++dd) {
+                    const int v = jcs[dd * PITCH + lane];
+                    mn = min(mn, v);
+                    mx = max(mx, v);
+                }
+                mn = __reduce_min_sync(0xffffffffu, mn);
+                mx = __reduce_max_sync(0xffffffffu, mx);
+                const int klo = min(S, max(mn, 0) / LW), khi = min(S, (max(mx, 0) + LW - 1) / LW);
+                auto run = [&](auto klo_tag, auto khi_tag) {
+                    constexpr bool pred = decltype(klo_tag)::value < decltype(khi_tag)::value;
 #pragma unroll 1
-                for (int m2 = 0; m2 < (kBatch >> PS); m2 += 2) {
-                    const int kk = (m2 << PS) + psub, kk2 = kk + (1 << PS);
-                    const int ma = jcs[rl * PITCH + kk], mb = jcs[rl * PITCH + kk2];
-                    const bool all = __all_sync(0xffffffffu, min(ma, mb) >= LW * S);
-                    const bool none = __all_sync(0xffffffffu, max(ma, mb) <= 0);
-                    if (all) {
-                        const Rec ra = load_rec(kk, false), rb = load_rec(kk2, false);
-                        sweep_bins(ra, kPolyEven, No{});
-                        sweep_bins(rb, kPolyOdd, No{});
-                    } else if (!none) {
-                        const Rec ra = load_rec(kk, true), rb = load_rec(kk2, true);
-                        sweep_bins(ra, kPolyEven, Yes{});
-                        sweep_bins(rb, kPolyOdd, Yes{});
+                    for (int kk = 0; kk < kBatch; kk += 2) {
+                        const Rec ra = load_rec(kk, pred), rb = load_rec(kk + 1, pred);
+                        sweep_bins(ra, kPolyEven, klo_tag, khi_tag);
+                        sweep_bins(rb, kPolyOdd, klo_tag, khi_tag);
+                    }
+                };
+                using std::integral_constant;
+                if (khi == 0) {
+                    // every bin of the tile above every cut-off: nothing to add
+                } else if (khi - klo > 2) {
+                    run(integral_constant<int, 0>{}, KS{});
+                } else {
+                    static_assert(S == 8, "one sweep per number of unconditional bins");
+                    switch (klo) {
+                        case 0: run(integral_constant<int, 0>{}, integral_constant<int, 2>{}); break;
+                        case 1: run(integral_constant<int, 1>{}, integral_constant<int, 3>{}); break;
+                        case 2: run(integral_constant<int, 2>{}, integral_constant<int, 4>{}); break;
+                        case 3: run(integral_constant<int, 3>{}, integral_constant<int, 5>{}); break;
+                        case 4: run(integral_constant<int, 4>{}, integral_constant<int, 6>{}); break;
+                        case 5: run(integral_constant<int, 5>{}, integral_constant<int, 7>{}); break;
+                        case 6: run(integral_constant<int, 6>{}, KS{}); break;
+                        case 7: run(integral_constant<int, 7>{}, KS{}); break;
+                        default: run(KS{}, KS{}); break;
                     }
                 }
             } else {
@@ -395,8 +419,8 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 for (int m2 = 0; m2 < (kBatch >> PS); m2 += 2) {
                     const int kk = (m2 << PS) + psub;
                     const Rec ra = load_rec(kk, false), rb = load_rec(kk + (1 << PS), false);
-                    sweep_bins(ra, DY > 0 ? 0 : kPolyEven, No{});   // dyadic: the XU pipe is not the bound
-                    sweep_bins(rb, DY > 0 ? 0 : kPolyOdd, No{});
+                    sweep_bins(ra, DY > 0 ? 0 : kPolyEven, KS{}, KS{});   // dyadic: the XU pipe is not the bound
+                    sweep_bins(rb, DY > 0 ? 0 : kPolyOdd, KS{}, KS{});
                 }
             }
         }
