@@ -157,7 +157,7 @@ typedef struct {
  * (the spatial window, if any, still multiplies it; weights must be >= 0).
  *     RAD_FF_GAUSSIAN    F = exp( -1/2 sum_c (w_j n_c s_c / c)^2 )           s_c: standard deviations
  *     RAD_FF_CIC         F = prod_c sinc^2( w_j n_c s_c / (2c) )             s_c: cell sizes (cloud in cell)
- *     RAD_FF_INCOHERENT  F = 0: g = sqrt(w)
+ *     RAD_FF_INCOHERENT  F = 0: g = sqrt(w) (a per-particle weight: costs nothing per update)
  * w = 1 is the identity for every shape; zero sizes give F = 1, g = w (the detector as
  * BASELINE.json states it).  F^2 is tabulated per (direction, frequency) at rad_create in fp64;
  * the square root is taken per update (a third special-function operation per update). */

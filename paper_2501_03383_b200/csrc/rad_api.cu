@@ -404,6 +404,7 @@ rad_status accumulate_device(Handle &h, int64_t step, int64_t n, const void *con
     p.n_dir = h.D; p.n_omega = h.W; p.w_pad = h.w_pad;
     p.n_ftiles = h.n_ftiles; p.n_wtiles = h.n_wtiles; p.psplit = h.psplit;
     p.dirs = h.dirs_d; p.F = h.F_d; p.Ff = h.Ff_d; p.fl = h.fl_d; p.F2 = h.F2_d;
+    p.w_sqrt = h.ff_type == RAD_FF_INCOHERENT;
     p.ts32 = (h.t0 + (double)step * h.dt) * h.f_unit * kTwo32;
     p.dts32 = h.dt * h.f_unit * kTwo32;
     p.nyq_lim = h.nyq_lim; p.dt64 = h.dt; p.omega64 = h.omega_d;
@@ -572,6 +573,9 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     }
     if (h.win_il[0] == 0.0 && h.win_il[1] == 0.0 && h.win_il[2] == 0.0) h.win_type = RAD_WINDOW_NONE;
     h.ff_type = cfg->form_factor_type;
+    // F = 0 for every bin (RAD_FF_INCOHERENT): g = sqrt(w) is a per-particle weight -- no table, no per-update square
+    // root, every kernel variant stays available
+    h.ff_table = h.ff_type == RAD_FF_GAUSSIAN || h.ff_type == RAD_FF_CIC;
     h.dt = cfg->dt; h.t0 = cfg->t0;
     h.scale = cfg->scale == 0.0 ? default_scale() : cfg->scale;
     h.state_f64 = cfg->state_dtype == RAD_F64;
@@ -617,13 +621,13 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     }
     h.sdir[0] = recs[0]; h.sdir[1] = recs[h.D > 1 ? 1 : 0];
     // particle split: the plain general / uniform sweeps only (rad_kernels.cu SPLIT instantiations)
-    choose_tile(h, h.nyq_lim == 0.0 && h.ff_type == RAD_FF_NONE && !h.fast);
+    choose_tile(h, h.nyq_lim == 0.0 && !h.ff_table && !h.fast);
     // Dyadic log grid (SURVEY.md section 8(f) NEXT-4 "dyadic log grids (integer bins/octave) allow
     // z(2w) = z(w)^2"): w_(j+b) = 2 w_j for an integer b = c * lw with lw in {4, 8, 16, 32}, c in {1, 2} ->
     // bins i and i + c of a thread's strip are an octave apart.  Among the admissible tile shapes the
     // widest one wins unless it pads more than choose_tile's own choice does.
     h.dyad_c = 0;
-    if (!(cfg->flags & RAD_FLAG_FORCE_GENERAL) && h.nyq_lim == 0.0 && !h.fast && h.ff_type == RAD_FF_NONE && h.W >= 2) {
+    if (!(cfg->flags & RAD_FLAG_FORCE_GENERAL) && h.nyq_lim == 0.0 && !h.fast && !h.ff_table && h.W >= 2) {
         int b = 0;
         for (int cand = 4; cand <= 64 && cand < h.W && b == 0; ++cand) {
             bool ok = true;
@@ -700,7 +704,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     }
 
     // macro-particle form factor (rad.h, reading FF1): F^2(n, w_j) per (direction, frequency), fp64 -> fp32
-    if (h.ff_type != RAD_FF_NONE) {
+    if (h.ff_table) {
         h.F2_h.assign((size_t)h.D * h.w_pad, 0.0f);
         const double *sz = cfg->form_factor_size;
         for (int d = 0; d < h.D; ++d)

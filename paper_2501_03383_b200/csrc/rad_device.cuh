@@ -261,7 +261,7 @@ __device__ __forceinline__ Particle load_particle(const AccumParams &P, long lon
         p.bdx = (float)dx; p.bdy = (float)dy; p.bdz = (float)dz;
         p.w = (float)w;
         p.ww = fmaf(p.w, p.w, -p.w);
-        p.wdt = ff ? P.dt : p.w * P.dt;
+        p.wdt = ff ? P.dt : (P.w_sqrt ? __fsqrt_rn(p.w) : p.w) * P.dt;
         if (WIN) p.wdt *= window_weight(P, p.rx, p.ry, p.rz);
     } else {  // padding lane: zero amplitude, harmless phase
         p.rx = p.ry = p.rz = p.bx = p.by = p.bz = 0.0;

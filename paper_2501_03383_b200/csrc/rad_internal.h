@@ -67,6 +67,7 @@ struct AccumParams {
     const float *Ff;       // [w_pad] (float)F_j
     const float *fl;       // [w_pad] f_j / f_unit - F_j  in [-0.5, 0.5]
     const float *F2;       // form factor: [D][w_pad] F^2(n, w_j) (rad.h, reading FF1), NULL: off
+    int w_sqrt;            // 1: the amplitude weight of a particle is sqrt(w) (RAD_FF_INCOHERENT: F = 0, g = sqrt(w) per particle)
     double ts32;           // (t0 + step dt) f_unit 2^32
     double dts32;          // dt f_unit 2^32: multi-step calls, chunk time = ts32 + chunk.step * dts32
     float dt;              // quadrature weight
@@ -175,6 +176,7 @@ struct Handle {
     uint32_t *F_d = nullptr;
     float *Ff_d = nullptr, *fl_d = nullptr;
     int ff_type = 0;                 // RAD_FF_*
+    bool ff_table = false;           // Gaussian / CIC shape: per-update weight from the F^2 table (incoherent: sqrt(w) per particle)
     float *F2_d = nullptr;           // form factor on: [D][w_pad] F^2(n, w_j)
     std::vector<float> F2_h;         // host copy (streaming shapes pass it in the parameter bank)
     double *acc_d = nullptr;         // [D][w_pad][4]

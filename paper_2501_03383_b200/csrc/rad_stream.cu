@@ -102,7 +102,7 @@ __device__ __forceinline__ Particle make_particle(ST rx, ST ry, ST rz, ST bx, ST
     p.bdx = (float)dx; p.bdy = (float)dy; p.bdz = (float)dz;
     p.w = (float)w;
     p.ww = fmaf(p.w, p.w, -p.w);
-    p.wdt = (WIN && P.F2) ? P.dt : p.w * P.dt;  // form factor on: the weight enters per update (ff_weight)
+    p.wdt = (WIN && P.F2) ? P.dt : (P.w_sqrt ? __fsqrt_rn(p.w) : p.w) * P.dt;  // form factor table on: the weight enters per update (ff_weight)
     if (WIN) p.wdt *= window_weight(P, p.rx, p.ry, p.rz);
     return p;
 }
