@@ -18,7 +18,7 @@ LIB_PATH = _PKG / "librad.so"
 
 RAD_OK, RAD_ERR_INVALID_ARG, RAD_ERR_ALLOC, RAD_ERR_CUDA, RAD_ERR_STATE, RAD_ERR_UNSUPPORTED = range(6)
 RAD_F32, RAD_F64 = 0, 1
-RAD_FLAG_DETERMINISTIC, RAD_FLAG_FORCE_GENERAL, RAD_FLAG_OVERLAP_STEPS, RAD_FLAG_FAST_GRIDDED = 1, 2, 4, 8
+RAD_FLAG_DETERMINISTIC, RAD_FLAG_FORCE_GENERAL, RAD_FLAG_OVERLAP_STEPS, RAD_FLAG_FAST_GRIDDED, RAD_FLAG_PRECISE = 1, 2, 4, 8, 16
 RAD_OUT_HOST, RAD_OUT_DEVICE, RAD_OUT_HOST_ASYNC = 0, 1, 2
 RAD_WINDOW_NONE, RAD_WINDOW_TRIANGLE, RAD_WINDOW_HAMMING = 0, 1, 2
 WINDOW_TYPES = {"none": RAD_WINDOW_NONE, "triangle": RAD_WINDOW_TRIANGLE, "hamming": RAD_WINDOW_HAMMING}

@@ -523,7 +523,8 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         return fail(nullptr, RAD_ERR_INVALID_ARG, "dt must be finite and > 0; t0, scale finite; scale >= 0");
     if (cfg->state_dtype != RAD_F32 && cfg->state_dtype != RAD_F64)
         return fail(nullptr, RAD_ERR_INVALID_ARG, "state_dtype must be RAD_F32 or RAD_F64");
-    if (cfg->flags & ~(RAD_FLAG_DETERMINISTIC | RAD_FLAG_FORCE_GENERAL | RAD_FLAG_OVERLAP_STEPS | RAD_FLAG_FAST_GRIDDED))
+    if (cfg->flags & ~(RAD_FLAG_DETERMINISTIC | RAD_FLAG_FORCE_GENERAL | RAD_FLAG_OVERLAP_STEPS | RAD_FLAG_FAST_GRIDDED |
+                       RAD_FLAG_PRECISE))
         return fail(nullptr, RAD_ERR_INVALID_ARG, "unknown flag bits");
     if (cfg->n_regions < 0) return fail(nullptr, RAD_ERR_INVALID_ARG, "n_regions must be >= 0");
     if (!std::isfinite(cfg->nyquist_factor) || cfg->nyquist_factor < 0.0)
@@ -560,6 +561,11 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
             return fail(nullptr, RAD_ERR_UNSUPPORTED,
                         "RAD_FLAG_FAST_GRIDDED: no regions, Nyquist limiter, form factor or deterministic mode");
     }
+    const bool precise = (cfg->flags & RAD_FLAG_PRECISE) != 0;
+    if (precise && (fast || cfg->nyquist_factor > 0.0 || cfg->form_factor_type == RAD_FF_GAUSSIAN ||
+                    cfg->form_factor_type == RAD_FF_CIC))
+        return fail(nullptr, RAD_ERR_UNSUPPORTED,
+                    "RAD_FLAG_PRECISE: no Nyquist limiter, Gaussian / CIC form factor or RAD_FLAG_FAST_GRIDDED");
     rad_handle *hh = new (std::nothrow) rad_handle();
     if (!hh) return fail(nullptr, RAD_ERR_ALLOC, "out of host memory");
     Handle &h = hh->h;
@@ -582,6 +588,7 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     h.deterministic = (cfg->flags & RAD_FLAG_DETERMINISTIC) != 0;
     h.overlap = (cfg->flags & RAD_FLAG_OVERLAP_STEPS) != 0;
     h.fast = fast;
+    h.precise = precise;
 
     // directions: normalise in fp64 (Q8), build e1, e2 with e1 x e2 = n
     h.dirs_h.resize((size_t)h.D * 3);
@@ -621,13 +628,13 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
     }
     h.sdir[0] = recs[0]; h.sdir[1] = recs[h.D > 1 ? 1 : 0];
     // particle split: the plain general / uniform sweeps only (rad_kernels.cu SPLIT instantiations)
-    choose_tile(h, h.nyq_lim == 0.0 && !h.ff_table && !h.fast);
+    choose_tile(h, h.nyq_lim == 0.0 && !h.ff_table && !h.fast && !h.precise);
     // Dyadic log grid (SURVEY.md section 8(f) NEXT-4 "dyadic log grids (integer bins/octave) allow
     // z(2w) = z(w)^2"): w_(j+b) = 2 w_j for an integer b = c * lw with lw in {4, 8, 16, 32}, c in {1, 2} ->
     // bins i and i + c of a thread's strip are an octave apart.  Among the admissible tile shapes the
     // widest one wins unless it pads more than choose_tile's own choice does.
     h.dyad_c = 0;
-    if (!(cfg->flags & RAD_FLAG_FORCE_GENERAL) && h.nyq_lim == 0.0 && !h.fast && !h.ff_table && h.W >= 2) {
+    if (!(cfg->flags & RAD_FLAG_FORCE_GENERAL) && h.nyq_lim == 0.0 && !h.fast && !h.ff_table && !h.precise && h.W >= 2) {
         int b = 0;
         for (int cand = 4; cand <= 64 && cand < h.W && b == 0; ++cand) {
             bool ok = true;
@@ -652,11 +659,11 @@ rad_status rad_create(const rad_config *cfg, rad_handle **out)
         }
     }
     // per-region detectors and the Nyquist limiter: bin-owner kernels only
-    h.stream_nb = (h.R > 1 || h.nyq_lim > 0.0 || h.fast) ? 0 : stream_shape(h.D, h.W, &h.stream_nd);
+    h.stream_nb = (h.R > 1 || h.nyq_lim > 0.0 || h.fast || h.precise) ? 0 : stream_shape(h.D, h.W, &h.stream_nd);
     // uniform grid?  w_j = w_0 + j dw to fp64 rounding -> rotation-recurrence kernel (a2')
     h.uniform = false;
     double uni_dw = 0.0;
-    if (h.W >= 2 * h.strip && !(cfg->flags & RAD_FLAG_FORCE_GENERAL) && h.nyq_lim == 0.0 && !h.fast) {
+    if (h.W >= 2 * h.strip && !(cfg->flags & RAD_FLAG_FORCE_GENERAL) && h.nyq_lim == 0.0 && !h.fast && !h.precise) {
         const double dw = (h.omega_h.back() - h.omega_h.front()) / (h.W - 1);
         bool uni = true;
         for (int j = 0; j < h.W && uni; ++j)

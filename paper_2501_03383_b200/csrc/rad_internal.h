@@ -162,6 +162,7 @@ struct Handle {
     double win_o[3] = {0, 0, 0}, win_il[3] = {0, 0, 0};
     bool state_f64 = false, deterministic = false, uniform = false;
     bool overlap = false;            // RAD_FLAG_OVERLAP_STEPS
+    bool precise = false;            // RAD_FLAG_PRECISE: all-polynomial sincos on the general-grid kernel
     int dyad_c = 0;                  // > 0: dyadic log grid, w_(j + dyad_c*lw) = 2 w_j -> squaring chains (rad_kernels.cu DY)
     uint32_t rot_G = 0;              // uniform grid: rotator frequency LW*df in f_unit units
     float rot_Gf = 0, rot_gl = 0;

@@ -129,12 +129,14 @@ __device__ __forceinline__ bool decode_task(const AccumParams &P, int warp, int 
 // m g_hs and amplitude g_master[n][m]; the sweep and the phase arithmetic are those of the general grid.
 constexpr int kDyadChain = 2;  // dyadic grids: bins per squaring chain (1 anchor + kDyadChain - 1 squarings)
 
-template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ, bool FF, bool GRID = false, int DY = 0, bool SPLIT = false>
+template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ, bool FF, bool GRID = false, int DY = 0, bool SPLIT = false,
+          bool PREC = false>
 __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
 {
     static_assert(!GRID || (!UNI && !NYQ && !FF), "grid evaluation runs the plain general-grid sweep");
     static_assert(DY == 0 || (!UNI && !NYQ && !FF && !GRID), "dyadic squaring runs on the plain general-grid sweep");
     static_assert(!SPLIT || (LW < 32 && !NYQ && !FF && !GRID && DY == 0), "particle split: plain general / uniform sweep, >= 2 lane groups");
+    static_assert(!PREC || (!UNI && !NYQ && !FF && !GRID && DY == 0 && !SPLIT), "RAD_FLAG_PRECISE: the plain general-grid sweep, every bin by the polynomial");
     static_assert(!(UNI && NYQ), "the limiter runs on the general-grid kernel");
     constexpr int DPW = 32 / LW;
     // Shared-memory records are direction-major, rec[direction of the warp][particle of the batch], rows padded
@@ -249,7 +251,7 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 uint32_t T;
                 double d64;
                 float inv_d;
-                stage_record<(DPW == 1 && !UNI && DY == 0)>(p, P.dirs[dir], ts32, r4, sf, &T, &d64, &inv_d);
+                stage_record<(DPW == 1 && !UNI && DY == 0 && !PREC)>(p, P.dirs[dir], ts32, r4, sf, &T, &d64, &inv_d);
                 rec[dd * PITCH + lane] = r4;
                 sfs[dd * PITCH + lane] = sf;
                 // bins below the cut-off, relative to the first bin of the warp's frequency tile
@@ -419,8 +421,8 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 for (int m2 = 0; m2 < (kBatch >> PS); m2 += 2) {
                     const int kk = (m2 << PS) + psub;
                     const Rec ra = load_rec(kk, false), rb = load_rec(kk + (1 << PS), false);
-                    sweep_bins(ra, DY > 0 ? 0 : kPolyEven, KS{}, KS{});   // dyadic: the XU pipe is not the bound
-                    sweep_bins(rb, DY > 0 ? 0 : kPolyOdd, KS{}, KS{});
+                    sweep_bins(ra, PREC ? S : DY > 0 ? 0 : kPolyEven, KS{}, KS{});   // dyadic: the XU pipe is not the bound
+                    sweep_bins(rb, PREC ? S : DY > 0 ? 0 : kPolyOdd, KS{}, KS{});
                 }
             }
         }
@@ -514,10 +516,27 @@ static cudaError_t dispatch_split(const Handle &h, const AccumParams &p, cudaStr
     }
 }
 
+template <typename ST>
+static cudaError_t dispatch_precise(const Handle &h, const AccumParams &p, cudaStream_t s)
+{
+    const long long n_tasks = (long long)p.n_wtiles * p.n_chunks;
+    const dim3 grid((unsigned)((n_tasks + kWarpsPerBlock - 1) / kWarpsPerBlock));
+    switch (h.lw) {
+        case 32: return launch_kernel(rad_accum<ST, 32, kStrip, kMinBlocks, false, false, false, false, 0, false, true>, grid, dim3(kThreads), 0, s, h.overlap, p);
+        case 16: return launch_kernel(rad_accum<ST, 16, kStrip, kMinBlocks, false, false, false, false, 0, false, true>, grid, dim3(kThreads), 0, s, h.overlap, p);
+        case 8: return launch_kernel(rad_accum<ST, 8, kStrip, kMinBlocks, false, false, false, false, 0, false, true>, grid, dim3(kThreads), 0, s, h.overlap, p);
+        default: return launch_kernel(rad_accum<ST, 4, kStrip, kMinBlocks, false, false, false, false, 0, false, true>, grid, dim3(kThreads), 0, s, h.overlap, p);
+    }
+}
+
 cudaError_t launch_accumulate(const Handle &h, const AccumParams &p, bool state_f64,
                               cudaStream_t s, int *n_launches, const char **variant)
 {
     *n_launches = 1;
+    if (h.precise) {  // RAD_FLAG_PRECISE: every sincos by the fp32 polynomial (rad_create keeps the other variants off)
+        *variant = "general+precise";
+        return state_f64 ? dispatch_precise<double>(h, p, s) : dispatch_precise<float>(h, p, s);
+    }
     if (p.psplit > 0) {  // few directions: lane groups split the particles (rad_create allows it on the plain sweeps only)
         *variant = h.uniform ? "uniform+split" : "general+split";
         if (h.uniform) return state_f64 ? dispatch_split<double, true>(h, p, s) : dispatch_split<float, true>(h, p, s);

@@ -72,6 +72,43 @@ def test_uniform_grid_padded_anchor_shapes(oracle_mod, D, W, dtype):
     assert P.base_variant(vg) == "general" and P.rel_l2(S, Sg) < 1e-5
 
 
+def test_precise_flag_all_polynomial_sincos(oracle_mod):
+    """RAD_FLAG_PRECISE: every sin/cos by the fp32 polynomial on the general-grid kernel, whatever the grid (log,
+    linear, few bins).  (a) parity on the usual shapes; (b) the dark-bin case a 1200-case random hunt found
+    (33 directions x 17 linear frequencies, three sub-volumes of 210 / 768 / 2022 particles,
+    a bin at 2.8e-6 of the peak where the default kernels reach 1.2e-3 / 1.6e-3): within the tolerance with the
+    flag, and at least 2x closer to the oracle than the default general kernel; (c) unsupported combinations."""
+    from paper_2501_03383_b200 import binding
+    for D, W, om in ((5, 96, wl.omega_log(96)), (3, 40, np.linspace(2e14, 2e17, 40)), (1, 8, wl.omega_log(8))):
+        w = wl.Workload("prec", 1500, 2, 1e-17, wl.dirs_fibonacci(max(D, 2))[:D], om, np.float32, wl.BASE_SEED + 27, "khi")
+        steps = list(w.steps())
+        S, variant = P.run_gpu(w, steps, flags=binding.RAD_FLAG_PRECISE)
+        assert variant == "general+precise"
+        P.assert_parity(S, P.run_oracle(oracle_mod, w, steps).spectrum(), what=f"precise {D}x{W}")
+    rng = np.random.default_rng(7700 + 148)          # the drawn case 148 of a 1200-case run of tests/test_gpu_fuzz.py
+    om = np.linspace(3.71364082e14, 2.12037748e17, 17)
+    w = wl.Workload("dark", 3000, 3, 1e-17, wl.dirs_fibonacci(33), om, np.float64, 169478, "khi")
+    steps = list(w.steps())
+    off = np.array([0, 210, 978, 3000], dtype=np.int64)
+    o = oracle_mod.RegionOracle(3, w.dirs, w.omega, w.dt, scale=1.0)
+    for t, st in steps:
+        o.accumulate_step(t, off, *st)
+    ref = o.spectrum()
+    err = {}
+    for name, flags in (("default", binding.RAD_FLAG_FORCE_GENERAL), ("precise", binding.RAD_FLAG_PRECISE)):
+        with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, state_dtype=np.float64, flags=flags, n_regions=3) as det:
+            for t, st in steps:
+                det.accumulate_step_regions(t, off, P.to_device(st))
+            err[name] = P.max_rel(det.spectrum(), ref)
+    print(f"dark-bin case: maxrel default general kernel {err['default']:.2e}, RAD_FLAG_PRECISE {err['precise']:.2e}")
+    assert err["precise"] <= P.MAX_REL_TOL and err["precise"] < 0.5 * err["default"]
+    for kw in (dict(nyquist=0.5), dict(form_factor=("gaussian", (1e-8,) * 3)),
+               dict(flags=binding.RAD_FLAG_FAST_GRIDDED, fast=((0, 0, 0), (1e-5, 1e-5, 1e-5), 0, 1, 0.0))):
+        kw["flags"] = kw.get("flags", 0) | binding.RAD_FLAG_PRECISE
+        with pytest.raises(binding.RadError, match="UNSUPPORTED"):
+            binding.Detector(w.dirs, w.omega, w.dt, **kw)
+
+
 @pytest.mark.parametrize("D,W,grid,dtype", [(1, 64, "log", np.float32), (1, 128, "log", np.float32), (2, 64, "log", np.float64),
                                             (1, 100, "log", np.float32), (3, 24, "log", np.float32), (1, 40, "linear", np.float32),
                                             (2, 60, "linear", np.float64), (1, 17, "log", np.float32)])
