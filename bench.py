@@ -9,7 +9,7 @@ rad_spectrum (a4).  Metric (BASELINE.json): particle*direction*frequency updates
 in G/s, whole job.  Headline workload = BASELINE.json configs[2] ("production-like": 1 048 576
 electrons x 256 directions x 1024 log-spaced frequencies, fp32 state), the largest single-GPU
 configuration.  The same invocation also runs short legs of every other configuration (1, 3a-d,
-4, 4b, 5r, 5s, 0, 1u, 1f, 1n, 1d) and reports them under "configs", runs the pipe microbenchmarks
+4, 4b, 5r, 5s, 0, 1u, 1f, 1n, 1d, 1p) and reports them under "configs", runs the pipe microbenchmarks
 (librad_ubench.so) and reports the measured ALU peaks under "alu_peaks", and compares the
 spectrum left by the timed region with the fp64 oracle on sampled bins ("parity").
 
@@ -47,7 +47,7 @@ FP32_PER_UPDATE_UNIFORM = 8  # 4 (complex rotation) + 4 (accumulate) FMA-pipe in
 L2_BYTES = 126 * 2 ** 20
 # short legs run after the headline: (config, timed steps, warm-up steps)
 LEGS = (("1", 50, 3), ("3a", 10, 3), ("3b", 10, 3), ("3c", 10, 3), ("3d", 10, 3), ("4", 3, 1), ("4b", 200, 3),
-        ("5r", 200, 5), ("5s", 200, 5), ("0", 500, 5), ("1u", 50, 3), ("1f", 50, 3), ("1n", 50, 3), ("1d", 50, 3))
+        ("5r", 200, 5), ("5s", 200, 5), ("0", 500, 5), ("1u", 50, 3), ("1f", 50, 3), ("1n", 50, 3), ("1d", 50, 3), ("1p", 30, 3))
 
 
 def parse_args():
@@ -301,6 +301,8 @@ def measure(cfg, K, W, args, ctx, headline):
     # here: device-resident inputs are uploaded and synchronised before the timed region, host inputs
     # reach the kernels through an event of the library's copy stream.
     flags = 0 if args.no_overlap else binding.RAD_FLAG_OVERLAP_STEPS
+    if w.precise:
+        flags |= binding.RAD_FLAG_PRECISE
     det = binding.Detector(w.dirs, w.omega, w.dt, t0=w.t0, scale=0.0, state_dtype=w.state_dtype,
                            device=local, n_regions=R if R > 1 else 0, flags=flags, form_factor=w.form_factor,
                            nyquist=w.nyquist)
@@ -385,6 +387,11 @@ def measure(cfg, K, W, args, ctx, headline):
         if variant == "uniform":  # rotation recurrence: 4 FP32 rotate + 4 FMA accumulate per update
             per_clk_sm, pipe = FP32_LANES_PER_SM / FP32_PER_UPDATE_UNIFORM, "FP32 (8 FMA-pipe instr per update)"
             measured = peaks_alu["ffma_per_clk_sm"] / FP32_PER_UPDATE_UNIFORM if peaks_alu else None
+        elif variant == "general+precise":
+            # RAD_FLAG_PRECISE: every sincos by the fp32 polynomial: 23 + 4 accumulate + ~1 loop / load instructions per
+            # update on the FMA and ALU pipes, no MUFU: bound by issue slots
+            per_clk_sm, pipe = FP32_LANES_PER_SM / 28.0, "issue (28 instructions per update: polynomial sincos)"
+            measured = None
         elif variant == "general+dyadic":
             # dyadic log grid: per two bins one anchor (phase + sincos: 8 instructions) + one squaring (4) +
             # 2 x 4 accumulates = 10 instructions per update at 1 MUFU per update: bound by issue slots
@@ -423,7 +430,7 @@ def measure(cfg, K, W, args, ctx, headline):
     out = {"value": value, "unit": UNIT, "steps": K, "warmup": W, "ms_per_step": ms_total / K,
            "kernel": f"rad_accum_{variant}", "roofline": roofline, "clocks": clocks, "gpu_launches": int(launches),
            "config": workload_config(w, n, world),
-           "launch": {"flags": "none" if args.no_overlap else "RAD_FLAG_OVERLAP_STEPS",
+           "launch": {"flags": ("none" if args.no_overlap else "RAD_FLAG_OVERLAP_STEPS") + (" | RAD_FLAG_PRECISE" if w.precise else ""),
                       "l2": f"ring of {ring} distinct step inputs ({ring * bytes_per_step / 2**20:.0f} MiB) + "
                             f"L2 flush before the timed region"}}
 

@@ -180,6 +180,7 @@ class Workload:
     extra: dict = field(default_factory=dict)
     form_factor: Optional[tuple] = None     # (type name, size[3] in metres) for rad_config / the oracle
     nyquist: float = 0.0                    # rad_config.nyquist_factor (0: limiter off)
+    precise: bool = False                   # RAD_FLAG_PRECISE (all-polynomial sincos)
 
     @property
     def n_dir(self) -> int:
@@ -270,6 +271,10 @@ def make_workload(cfg: str) -> Workload:
         # 38.46 / 76.99 bins per octave)
         return Workload("cfg1d_khi_dyadic_grid", 65536, 1000, 1e-17, dirs_fibonacci(128),
                         omega_dyadic(512, 32), np.float32, BASE_SEED + 1, "khi")
+    if cfg == "1p":
+        # config 1 with RAD_FLAG_PRECISE (every sincos by the fp32 polynomial): the precise-mode leg of bench.py
+        return Workload("cfg1p_khi_precise", 65536, 1000, 1e-17, dirs_fibonacci(128),
+                        omega_log(512), np.float32, BASE_SEED + 1, "khi", precise=True)
     if cfg == "1n":
         # config 1 with the Nyquist limiter at nu = 1 (w dt (1 - beta.n) >= pi dropped: at dt = 1e-17 s the
         # top ~1/8 of the log grid, the cut-off Doppler-shifted per particle and direction): the limiter
@@ -291,4 +296,4 @@ def make_workload(cfg: str) -> Workload:
     raise KeyError(cfg)
 
 
-ALL_CONFIGS = ("0", "1", "1u", "1f", "1n", "1d", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r", "5s")
+ALL_CONFIGS = ("0", "1", "1u", "1f", "1n", "1d", "1p", "2", "3a", "3b", "3c", "3d", "4", "4b", "5r", "5s")

@@ -40,7 +40,7 @@ def test_config_shapes(cfg):
              "3c": (262144, 200, 256, 256), "3d": (262144, 200, 1024, 64),
              "4": (16777216, 4, 16, 128), "4b": (16777216, 4, 1, 8),
              "5r": (331776, 200, 1, 512), "1u": (65536, 1000, 128, 512),
-             "1f": (65536, 1000, 128, 512), "1n": (65536, 1000, 128, 512), "1d": (65536, 1000, 128, 512), "5s": (331776, 200, 1, 128)}[cfg]
+             "1f": (65536, 1000, 128, 512), "1n": (65536, 1000, 128, 512), "1d": (65536, 1000, 128, 512), "5s": (331776, 200, 1, 128), "1p": (65536, 1000, 128, 512)}[cfg]
     assert (w.n_particles, w.n_steps, w.n_dir, w.n_omega) == sizes
     assert w.state_dtype == (np.float64 if cfg == "0" else np.float32)
 
