@@ -623,7 +623,9 @@ def run_ours(args):
         line = {
             "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f32 phase/amplitude, f64 set-up and accumulators", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f32",
+            "dtype_detail": "f32 phase arithmetic, sincos and per-chunk partial sums; f64 phase set-up, Doppler factor and accumulators",
+            "data": "synthetic",
             "config": head["config"], "launch": head["launch"], "clocks": head["clocks"], "e2e": head.get("e2e"),
             "gpu_launches": head["gpu_launches"], "roofline": head["roofline"],
             "cpu_baseline": head.get("cpu_baseline"), "parity": head.get("parity"),
