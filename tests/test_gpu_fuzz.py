@@ -52,6 +52,10 @@ def _draw(case):
     form = str(rng.choice(["step", "step", "host", "steps", "regions"]))
     flags = int(rng.choice([0, 0, 1, 4, 5, 2]))      # DETERMINISTIC = 1, FORCE_GENERAL = 2, OVERLAP_STEPS = 4
     weights = 1e3 if "form_factor" in opts else None
+    # RAD_FLAG_PRECISE = 16 on some of the cases it combines with (its own generator: the other draws stay as they were)
+    if "nyquist" not in opts and opts.get("form_factor", ("incoherent",))[0] == "incoherent" \
+            and np.random.default_rng(8800 + case).random() < 0.15:
+        flags |= 16
     return dict(D=D, W=W, kind=str(kind), omega=omega, dtype=dtype, n=n, T=T, t_first=t_first, opts=opts, form=form,
                 flags=flags, weights=weights, seed=int(rng.integers(1, 10 ** 6)))
 
