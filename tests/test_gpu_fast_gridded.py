@@ -134,3 +134,26 @@ def test_fast_gridded_errors():
         buf = torch.empty(3, 32, 4, dtype=torch.float64, device="cuda")
         with pytest.raises(binding.RadError, match="UNSUPPORTED"):
             det.export_accumulator(buf)
+
+
+def test_fast_gridded_host_buffers_and_multi_step_entry(oracle_mod):
+    """The other entry points on a fast handle: rad_accumulate_step_host (state in host memory, staged through the
+    handle's double buffer) and rad_accumulate_steps (runs as one spreading pass per step); spectrum to pinned host
+    memory with RAD_OUT_HOST_ASYNC."""
+    import torch
+    from paper_2501_03383_b200 import binding
+    w = wl.Workload("fasth", 2500, 4, 1e-17, wl.dirs_fibonacci(4), wl.omega_log(80), np.float32, wl.BASE_SEED + 94, "khi")
+    steps = list(w.steps())
+    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    fast = (BOX[0], BOX[1], 0, 3, 0.0)
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, flags=binding.RAD_FLAG_FAST_GRIDDED, fast=fast) as det:
+        for t, st in steps:
+            det.accumulate_step_host(t, st)
+        pinned = torch.empty(4, 80, dtype=torch.float64).pin_memory()
+        det.spectrum(out=pinned)
+        torch.cuda.synchronize()
+        P.assert_parity(pinned.numpy(), ref, what="fast gridded, host buffers")
+    stacked = [torch.from_numpy(np.stack([st[c] for _, st in steps])).cuda() for c in range(10)]
+    with binding.Detector(w.dirs, w.omega, w.dt, scale=1.0, flags=binding.RAD_FLAG_FAST_GRIDDED, fast=fast) as det:
+        det.accumulate_steps(0, stacked)
+        P.assert_parity(det.spectrum(), ref, what="fast gridded, multi-step entry")
