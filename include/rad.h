@@ -358,6 +358,39 @@ RAD_API const char *rad_status_string(rad_status s);
 RAD_API const char *rad_last_error(const rad_handle *h);
 RAD_API const char *rad_version(void);
 
+/* The detector as ONE call that allocates nothing -- for callers that cannot call cudaMalloc (code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid it).  No handle:
+ *   out_device[n_dir][n_omega] (DEVICE, fp64, overwritten) = scale * |A(n, w_j)|^2,
+ *   A = the sum at the top of this header over the steps first_step_index ... + n_steps - 1 and
+ *       n_particles particles per step (plain detector: one region, no window, limiter or form factor),
+ * with every argument the caller's: dirs_device DEVICE [n_dir][3] fp64 (any non-zero length),
+ * omega_device DEVICE [n_omega] fp64 rad/s (NOT validated: device memory is not read back), the 10
+ * state arrays DEVICE in the rad_accumulate_steps layout (step s at elements [s*step_stride,
+ * s*step_stride + n_particles), `state_dtype` elements), dt/t0/scale as in rad_config (scale 0 ->
+ * SI).  n_steps == 0 or n_particles == 0 gives out = 0.  Runs on the calling thread's CURRENT
+ * device, asynchronously on cuda_stream.
+ * The fp64 amplitude accumulator the kernel folds into is a static __device__ array inside the
+ * library, RAD_STATIC_MAX_BINS * 32 B = 2 MiB, which every GPU that loads the library holds until the
+ * process exits: n_dir * n_omega > RAD_STATIC_MAX_BINS fails with RAD_ERR_UNSUPPORTED.  The call
+ * uses no cudaMalloc / cudaFree or other allocating routine (it clears the part of the array it
+ * uses, launches the accumulate kernel -- a variant of the general-grid kernel that needs no set-up
+ * tables, same tolerances against the oracle -- and the |A|^2 kernel); its first call on a device
+ * looks up the array's address (cudaGetSymbolAddress), so make one call before capturing.
+ * ALL calls on a device share the array: calls that overlap on the GPU (different streams without
+ * an ordering, or several threads) race on it and give wrong results; calls on one stream are safe.
+ * Other error codes: RAD_ERR_INVALID_ARG (NULL pointer, negative size, dt <= 0, bad dtype,
+ * step_stride < n_particles), RAD_ERR_CUDA; message via rad_static_last_error() (per thread). */
+#define RAD_STATIC_MAX_BINS 65536
+RAD_API rad_status rad_spectrum_static(int32_t n_dir, const double *dirs_device, int32_t n_omega,
+                                       const double *omega_device, double dt, double t0, double scale,
+                                       int32_t state_dtype, int64_t first_step_index, int32_t n_steps,
+                                       int64_t n_particles, int64_t step_stride,
+                                       const void *rx, const void *ry, const void *rz,
+                                       const void *bx, const void *by, const void *bz,
+                                       const void *bdx, const void *bdy, const void *bdz,
+                                       const void *w, double *out_device, void *cuda_stream);
+RAD_API const char *rad_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

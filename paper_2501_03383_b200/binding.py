@@ -33,7 +33,9 @@ ABI_SYMBOLS = (
     "rad_spectrum_total", "rad_amplitude", "rad_add_amplitude", "rad_export_accumulator",
     "rad_import_accumulator", "rad_spectrum_of", "rad_reset", "rad_destroy", "rad_launch_count",
     "rad_kernel_variant", "rad_status_string", "rad_last_error", "rad_version",
+    "rad_spectrum_static", "rad_static_last_error",
 )
+RAD_STATIC_MAX_BINS = 65536
 
 
 class rad_config(ctypes.Structure):
@@ -115,6 +117,11 @@ def load(path: Optional[Path] = None) -> ctypes.CDLL:
     lib.rad_status_string.argtypes = [ctypes.c_int]
     lib.rad_version.restype = ctypes.c_char_p
     lib.rad_version.argtypes = []
+    lib.rad_spectrum_static.restype = ctypes.c_int
+    lib.rad_spectrum_static.argtypes = ([ctypes.c_int32, vp, ctypes.c_int32, vp, dbl, dbl, dbl, ctypes.c_int32, i64,
+                                         ctypes.c_int32, i64, i64] + [vp] * 10 + [vp, vp])
+    lib.rad_static_last_error.restype = ctypes.c_char_p
+    lib.rad_static_last_error.argtypes = []
     if path is None:
         _lib = lib
     return lib
@@ -253,6 +260,17 @@ def rad_launch_count(handle: int) -> int:
 
 def rad_kernel_variant(handle: int) -> str:
     return load().rad_kernel_variant(handle).decode()
+
+
+def rad_spectrum_static(n_dir: int, dirs_device_ptr: int, n_omega: int, omega_device_ptr: int, dt: float, t0: float,
+                        scale: float, state_dtype: int, first_step_index: int, n_steps: int, n_particles: int,
+                        step_stride: int, state_ptrs: Sequence[int], out_device_ptr: int, stream: int = 0) -> None:
+    """The allocation-free one-call detector (include/rad.h): every pointer DEVICE; out [n_dir][n_omega] fp64."""
+    lib = load()
+    st = lib.rad_spectrum_static(n_dir, dirs_device_ptr, n_omega, omega_device_ptr, dt, t0, scale, state_dtype,
+                                 first_step_index, n_steps, n_particles, step_stride, *state_ptrs, out_device_ptr, stream)
+    if st != RAD_OK:
+        raise RadError(st, (lib.rad_static_last_error() or b"").decode())
 
 
 # ------------------------------------------------------------------ convenience wrapper

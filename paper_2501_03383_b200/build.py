@@ -17,7 +17,7 @@ ROOT = PKG.parent
 CSRC = PKG / "csrc"
 LIB = PKG / "librad.so"
 UBENCH_LIB = PKG / "librad_ubench.so"
-SOURCES = ["rad_api.cu", "rad_kernels.cu", "rad_stream.cu", "rad_finalize.cu", "rad_gridded.cu"]
+SOURCES = ["rad_api.cu", "rad_kernels.cu", "rad_stream.cu", "rad_finalize.cu", "rad_gridded.cu", "rad_static.cu"]
 UBENCH_SOURCES = ["rad_ubench.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "--use_fast_math", "-Xcompiler", "-fPIC,-fvisibility=hidden,-O2", "-shared",
