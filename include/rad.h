@@ -374,7 +374,7 @@ RAD_API const char *rad_version(void);
  * process exits: n_dir * n_omega > RAD_STATIC_MAX_BINS fails with RAD_ERR_UNSUPPORTED.  The call
  * uses no cudaMalloc / cudaFree or other allocating routine (it clears the part of the array it
  * uses, launches the accumulate kernel -- a variant of the general-grid kernel that needs no set-up
- * tables, same tolerances against the oracle -- and the |A|^2 kernel); its first call on a device
+ * tables, same tolerances against the oracle, about 0.55 x the speed -- and the |A|^2 kernel); its first call on a device
  * looks up the array's address (cudaGetSymbolAddress), so make one call before capturing.
  * ALL calls on a device share the array: calls that overlap on the GPU (different streams without
  * an ordering, or several threads) race on it and give wrong results; calls on one stream are safe.

@@ -2,7 +2,8 @@
 accumulator is a static __device__ array inside librad.so, against the existing handle-based path
 (rad_create / rad_accumulate_steps / rad_spectrum) on the same device arrays, with BASELINE.json
 north_star's tolerances (tests/_parity.py), on calls in a row that share the array: a larger detector
-first, then a smaller one whose bins overlap the first call's leftovers, then the first again.
+first, then a smaller one whose bins overlap the first call's leftovers, then the first again, then one of
+exactly the maximum size.
 Named test_zz_* so that pytest collects it last (the round's end runs pytest -x)."""
 import numpy as np
 import pytest
@@ -57,9 +58,10 @@ def _both_paths(w, t_first, scale=1.0, check_free_memory=False):
 def test_static_scratch_entry_matches_existing_path_on_calls_in_a_row(oracle_mod):
     big = _case(13, 300, "log", np.float32, 3000, 3, 4101)       # ragged chunk tail (3000 = 5 * 512 + 440), 3 bin sweeps
     small = _case(3, 40, "linear", np.float64, 700, 2, 4102)    # its 120 bins lie inside the first call's 3900
+    limit = _case(128, 512, "log", np.float32, 1100, 1, 4104)   # n_dir * n_omega = RAD_STATIC_MAX_BINS exactly
     results = []
-    for call, (w, t_first) in enumerate(((big, 0), (small, 250), (big, 0))):
-        S_ref, S = _both_paths(w, t_first, check_free_memory=call == 2)
+    for call, (w, t_first) in enumerate(((big, 0), (small, 250), (big, 0), (limit, 900))):
+        S_ref, S = _both_paths(w, t_first, check_free_memory=call >= 2)
         assert S.shape == S_ref.shape and S_ref.max() > 0
         l2, mr = P.assert_parity(S, S_ref, what=f"rad_spectrum_static {w.name} vs existing path")
         print(f"rad_spectrum_static {w.name} {S.shape}: relL2 {l2:.2e} maxrel {mr:.2e} against the existing path")
