@@ -121,6 +121,37 @@ def test_no_cpu_fallback_without_gpu(lib):
     assert ei.value.status == binding.RAD_ERR_CUDA
 
 
+@pytest.mark.parametrize("kw,status,msg", [
+    (dict(n_dir=257, n_omega=256), 5, "RAD_STATIC_MAX_BINS"),       # beyond the static scratch: RAD_ERR_UNSUPPORTED
+    (dict(n_dir=0), 1, "n_dir"),
+    (dict(out=0), 1, "out_device"),
+    (dict(dt=0.0), 1, "dt"),
+    (dict(scale=float("nan")), 1, "scale"),
+    (dict(state_dtype=3), 1, "state_dtype"),
+    (dict(n_particles=5, step_stride=4), 1, "step_stride"),
+    (dict(n_particles=5, step_stride=5), 1, "NULL particle array"),
+])
+def test_spectrum_static_rejects_bad_arguments_without_a_device(lib, kw, status, msg):
+    """rad_spectrum_static checks sizes and scalars before it touches the device (the pointers here are never read)."""
+    from paper_2501_03383_b200 import binding
+    a = dict(n_dir=2, n_omega=8, dt=1e-17, scale=1.0, state_dtype=binding.RAD_F32, n_particles=0, step_stride=0, out=256)
+    a.update(kw)
+    with pytest.raises(binding.RadError) as ei:
+        binding.rad_spectrum_static(a["n_dir"], 256, a["n_omega"], 256, a["dt"], 0.0, a["scale"], a["state_dtype"], 0, 1,
+                                    a["n_particles"], a["step_stride"], [0] * 10, a["out"])
+    assert ei.value.status == status and msg in str(ei.value)
+
+
+def test_spectrum_static_has_no_cpu_fallback(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA device present")
+    from paper_2501_03383_b200 import binding
+    with pytest.raises(binding.RadError) as ei:
+        binding.rad_spectrum_static(2, 256, 8, 256, 1e-17, 0.0, 1.0, binding.RAD_F32, 0, 1, 0, 0, [0] * 10, 256)
+    assert ei.value.status == binding.RAD_ERR_CUDA
+
+
 def test_product_path_never_touches_the_oracle():
     """The package must not import, read or link anything under oracle/ (or _work/)."""
     pkg = ROOT / "paper_2501_03383_b200"
