@@ -73,6 +73,28 @@ def test_static_scratch_entry_matches_existing_path_on_calls_in_a_row(oracle_mod
     P.assert_parity(results[1], o.spectrum(), what="rad_spectrum_static vs oracle")
 
 
+@pytest.mark.parametrize("case", range(10))
+def test_static_scratch_entry_drawn_shapes(case):
+    """Drawn detector shapes (one bin, one direction, bin counts around the 128-lane tile), particle counts around the
+    512-particle chunk, both state dtypes, the SI default scale: against the existing path."""
+    rng = np.random.default_rng(6600 + case)
+    D = int(rng.choice([1, 2, 5, 40]))
+    W = int(rng.choice([1, 3, 17, 64, 127, 129, 300]))
+    n = int(rng.choice([1, 31, 512, 513, 1500]))
+    T = int(rng.integers(1, 4))
+    dtype = np.float64 if case % 2 else np.float32
+    w = _case(D, max(W, 2), str(rng.choice(["log", "linear"])), dtype, n, T, 6600 + case)
+    w.omega = w.omega[:W]
+    scale = 0.0 if case % 3 == 0 else 1.0
+    S_ref, S = _both_paths(w, int(rng.choice([0, 40, 900])), scale=scale)
+    assert S.shape == (D, W) and S_ref.max() > 0
+    what = f"rad_spectrum_static drawn case {case}: {D}x{W} n={n} T={T} {np.dtype(dtype).name}"
+    l2, mr = P.assert_parity(S, S_ref, what=what)
+    print(f"{what}: relL2 {l2:.2e} maxrel {mr:.2e} worst direction {max(P.max_rel(S[k], S_ref[k]) for k in range(D)):.2e}")
+    for k in range(D):                                   # every direction on its own (its own peak)
+        assert P.max_rel(S[k], S_ref[k]) <= P.MAX_REL_TOL, f"case {case} direction {k}"
+
+
 def test_static_scratch_entry_empty_input_and_limits():
     import torch
     from paper_2501_03383_b200 import binding
