@@ -190,6 +190,10 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    if int(os.environ.get("WORLD_SIZE", "1")) > 1 and "TORCHELASTIC_RUN_ID" in os.environ:
+        # torchrun exports OMP_NUM_THREADS=1 to every rank when N > 1; the other ranks do no work here, so rank 0
+        # times the oracle on all the host cores it may run on, as at N = 1 (set before the OpenMP runtime loads)
+        os.environ["OMP_NUM_THREADS"] = str(len(os.sched_getaffinity(0)))
     from oracle import oracle
     w = wl.make_workload(args.config)
     n = args.particles or w.n_particles
