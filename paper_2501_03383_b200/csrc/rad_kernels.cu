@@ -127,6 +127,11 @@ __device__ __forceinline__ bool decode_task(const AccumParams &P, int warp, int 
 // GRID: evaluation of the fast gridded path (rad.h RAD_FLAG_FAST_GRIDDED) -- the "particles" are the
 // points of the per-direction retarded-time grids: point m of direction n has phase s32 = g_s0[n] +
 // m g_hs and amplitude g_master[n][m]; the sweep and the phase arithmetic are those of the general grid.
+// Uniform-grid chain in packed form: sign s_n of y_n = s_n z_(MID+n) forwards (n >= 0: + + - - + + ...) and of
+// y'_m = s'_m z_(MID-m) backwards (m >= 0: + - - + + - ...); with them s_(n+1) / s_(n-1) = -1, so the three-term
+// recurrence has no subtraction.
+__host__ __device__ constexpr int uni_sign(int n) { return (n & 3) >= 2 ? -1 : 1; }
+__host__ __device__ constexpr int uni_sign_b(int m) { return ((m + 1) & 3) >= 2 ? -1 : 1; }
 constexpr int kDyadChain = 2;  // dyadic grids: bins per squaring chain (1 anchor + kDyadChain - 1 squarings)
 
 template <typename ST, int LW, int S, int MINB, bool UNI, bool NYQ, bool FF, bool GRID = false, int DY = 0, bool SPLIT = false,
@@ -294,23 +299,56 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
                 // (2 FFMA per bin instead of the 4 FMA-pipe instructions of a complex product).  A rounding error
                 // delta grows like sin(n theta) / sin(theta) <= n over n <= S/2 steps from the anchor.
                 const float c2 = rot.x + rot.x;
-                float pr = zr0, pi = zi0;
-                float zr = fmaf(zr0, rot.x, -zi0 * rot.y), zi = fmaf(zi0, rot.x, zr0 * rot.y);
-                const float br = fmaf(c2, zr0, -zr), bi = fmaf(c2, zi0, -zi);  // z_(MID-1)
-                add(MID + 1, zr, zi);
+                const float fr = fmaf(zr0, rot.x, -zi0 * rot.y), fi = fmaf(zi0, rot.x, zr0 * rot.y);  // z_(MID+1)
+                if constexpr (!FF) {
+                    // Packed form, one fma.rn.f32x2 per bin and no negation: the chain carries y = s z with the
+                    // signs s = + + - - + ... (uni_sign), for which y_(n+1) = (+-2c) y_n + y_(n-1); the bins with
+                    // s = -1 accumulate -A and get their sign back after the sweep (below).
+                    const unsigned long long Cp = pack2(c2, c2), Cn = pack2(-c2, -c2);
+                    const unsigned long long Y0 = pack2(zr0, zi0);
+                    auto addp = [&](const int i, const unsigned long long Y) {
+                        fma2(accA[i], A1b, Y);
+                        fma2(accB[i], A2b, Y);
+                    };
+                    unsigned long long P0 = Y0, Y = pack2(fr, fi);  // forwards: n = 1
+                    addp(MID + 1, Y);
 #pragma unroll
-                for (int i = MID + 2; i < S; ++i) {  // forwards
-                    const float nr = fmaf(c2, zr, -pr), ni = fmaf(c2, zi, -pi);
-                    pr = zr; pi = zi; zr = nr; zi = ni;
-                    add(i, zr, zi);
-                }
-                if (MID >= 1) add(MID - 1, br, bi);
-                pr = zr0; pi = zi0; zr = br; zi = bi;
+                    for (int i = MID + 2; i < S; ++i) {
+                        const int n = i - MID;  // y_n from y_(n-1), y_(n-2): factor 2c s_n / s_(n-1)
+                        const unsigned long long N = fma2r(uni_sign(n) == uni_sign(n - 1) ? Cp : Cn, Y, P0);
+                        P0 = Y; Y = N;
+                        addp(i, Y);
+                    }
+                    if (MID >= 1) {
+                        P0 = Y0;
+                        Y = fma2r(Cn, Y0, pack2(fr, fi));  // backwards: m = 1, y'_1 = -z_(MID-1) = -2c z_MID + z_(MID+1)
+                        addp(MID - 1, Y);
 #pragma unroll
-                for (int i = MID - 2; i >= 0; --i) {  // backwards
-                    const float nr = fmaf(c2, zr, -pr), ni = fmaf(c2, zi, -pi);
-                    pr = zr; pi = zi; zr = nr; zi = ni;
-                    add(i, zr, zi);
+                        for (int i = MID - 2; i >= 0; --i) {
+                            const int m = MID - i;
+                            const unsigned long long N = fma2r(uni_sign_b(m) == uni_sign_b(m - 1) ? Cp : Cn, Y, P0);
+                            P0 = Y; Y = N;
+                            addp(i, Y);
+                        }
+                    }
+                } else {
+                    float pr = zr0, pi = zi0, zr = fr, zi = fi;
+                    const float br = fmaf(c2, zr0, -zr), bi = fmaf(c2, zi0, -zi);  // z_(MID-1)
+                    add(MID + 1, zr, zi);
+#pragma unroll
+                    for (int i = MID + 2; i < S; ++i) {  // forwards
+                        const float nr = fmaf(c2, zr, -pr), ni = fmaf(c2, zi, -pi);
+                        pr = zr; pi = zi; zr = nr; zi = ni;
+                        add(i, zr, zi);
+                    }
+                    if (MID >= 1) add(MID - 1, br, bi);
+                    pr = zr0; pi = zi0; zr = br; zi = bi;
+#pragma unroll
+                    for (int i = MID - 2; i >= 0; --i) {  // backwards
+                        const float nr = fmaf(c2, zr, -pr), ni = fmaf(c2, zi, -pi);
+                        pr = zr; pi = zi; zr = nr; zi = ni;
+                        add(i, zr, zi);
+                    }
                 }
             }
         } else {
@@ -440,6 +478,10 @@ __global__ void __launch_bounds__(kThreads, MINB) rad_accum(const AccumParams P)
         for (int i = 0; i < S; ++i) {
             unpack2(accA[i], acc[i][0], acc[i][1]);
             unpack2(accB[i], acc[i][2], acc[i][3]);
+            if (UNI && (i >= MID ? uni_sign(i - MID) : uni_sign_b(MID - i)) < 0) {  // bins whose chain carried -z
+#pragma unroll
+                for (int c = 0; c < 4; ++c) acc[i][c] = -acc[i][c];
+            }
         }
     }
     if (SPLIT) {  // particle split: sum the lane groups of a direction (fixed order), group 0 folds
