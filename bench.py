@@ -43,7 +43,8 @@ HEADLINE = "2"
 MUFU_LANES_PER_SM = 16
 FP32_LANES_PER_SM = 128
 MUFU_PER_UPDATE = 2         # sin + cos: no recurrence exists on a non-uniform grid
-FP32_PER_UPDATE_UNIFORM = 8  # 4 (complex rotation) + 4 (accumulate) FMA-pipe instructions
+FP32_PER_UPDATE_UNIFORM = 6  # 2 (three-term recurrence of the rotation: one packed FMA) + 4 (accumulate) FP32 FMAs
+FP32_PER_UPDATE_UNIFORM_SURVEY = 8  # SURVEY.md section 8(d)'s R_lin: a 4-FMA complex rotation + 4 accumulate FMAs
 L2_BYTES = 126 * 2 ** 20
 # short legs run after the headline: (config, timed steps, warm-up steps)
 LEGS = (("1", 50, 3), ("3a", 10, 3), ("3b", 10, 3), ("3c", 10, 3), ("3d", 10, 3), ("4", 3, 1), ("4b", 200, 3),
@@ -388,9 +389,9 @@ def measure(cfg, K, W, args, ctx, headline):
                     "frac": hbm_achieved / hbm_peak, "traffic": traffic,
                     "peak_how": f"MEASURED_PEAKS.json hbm_gbs ({peaks_src})"}
     else:
-        if variant == "uniform":  # rotation recurrence: 4 FP32 rotate + 4 FMA accumulate per update
-            per_clk_sm, pipe = FP32_LANES_PER_SM / FP32_PER_UPDATE_UNIFORM, "FP32 (8 FMA-pipe instr per update)"
-            measured = peaks_alu["ffma_per_clk_sm"] / FP32_PER_UPDATE_UNIFORM if peaks_alu else None
+        if variant == "uniform":  # rotation recurrence: 2 FP32 FMA rotate (three-term) + 4 FMA accumulate per update
+            per_clk_sm, pipe = FP32_LANES_PER_SM / FP32_PER_UPDATE_UNIFORM, "FP32 (6 FMAs per update: 3 fma.rn.f32x2)"
+            measured = peaks_alu["ffma2_fma_per_clk_sm"] / FP32_PER_UPDATE_UNIFORM if peaks_alu else None
         elif variant == "general+precise":
             # RAD_FLAG_PRECISE: every sincos by the fp32 polynomial: 23 + 4 accumulate + ~1 loop / load instructions per
             # update on the FMA and ALU pipes, no MUFU: bound by issue slots
@@ -417,10 +418,15 @@ def measure(cfg, K, W, args, ctx, headline):
             peak_m = n_sm * measured * sm_max * 1e6 / 1e9
             roofline.update({"peak_measured_pipe": peak_m, "frac_of_measured_pipe": achieved / peak_m,
                              "peak_measured_how": f"{n_sm} SMs x {measured:.3f} updates/clk/SM (alu_peaks) x {sm_max:.0f} MHz"})
-        if variant == "uniform" and peaks_alu and peaks_alu.get("ffma_var_per_clk_sm"):
-            # the sweep's FMAs read three different registers each: what the register file feeds the
-            # FMA pipe without operand reuse (alu_peaks ffma_var) is the rate the kernel actually sits on
-            peak_v = n_sm * peaks_alu["ffma_var_per_clk_sm"] / FP32_PER_UPDATE_UNIFORM * sm_max * 1e6 / 1e9
+        if variant == "uniform":
+            # SURVEY.md section 8(d) defines R_lin with a 4-FMA complex rotation (8 FMAs per update); the kernel's
+            # three-term recurrence needs 6, so `peak` above is the (higher) bound of what the kernel computes
+            peak_s = n_sm * FP32_LANES_PER_SM / FP32_PER_UPDATE_UNIFORM_SURVEY * sm_max * 1e6 / 1e9
+            roofline.update({"peak_survey_r_lin": peak_s, "frac_of_survey_r_lin": achieved / peak_s})
+        if variant == "uniform" and peaks_alu and peaks_alu.get("ffma2_var_fma_per_clk_sm"):
+            # the sweep's packed FMAs read three different register pairs each: what the register file feeds the
+            # FMA pipe without operand reuse (alu_peaks ffma2_var_fma) is the rate the kernel actually sits on
+            peak_v = n_sm * peaks_alu["ffma2_var_fma_per_clk_sm"] / FP32_PER_UPDATE_UNIFORM * sm_max * 1e6 / 1e9
             roofline.update({"peak_measured_no_operand_reuse": peak_v, "frac_of_measured_no_operand_reuse": achieved / peak_v})
         if clocks.get("sm_mhz"):
             roofline["frac_at_sampled_clock"] = roofline["frac"] * sm_max / clocks["sm_mhz"]

@@ -105,12 +105,14 @@ __device__ __forceinline__ bool decode_task(const AccumParams &P, int warp, int 
 // ------------------------------------------------------------------------------------------
 // a2 (UNI = false): general (non-uniform) frequency grid.  Per update: 1 IMAD + 1 LEA.HI + 3 FP32
 // for the phase, FMUL + MUFU.SIN + MUFU.COS, 4 FFMA.
-// a2' (UNI = true): uniform grid w_j = w_0 + j dw.  A thread's bins are LW dw apart, so
-// z_{i+1} = z_i * rot with rot = exp(i LW dw tau) staged once per (particle, direction); the
-// chain is anchored at the thread's middle bin by a direct integer-phase sincos and runs S/2
-// steps forwards (rot) and S/2-1 backwards (conj rot): 1 sincos + (S-1) complex rotations per S
-// updates instead of S sincos.  Chain length <= S/2 keeps the recurrence drift (~6e-8 per
-// rotation) below the MUFU error, which is the periodic re-anchoring BASELINE.json asks for.
+// a2' (UNI = true): uniform grid w_j = w_0 + j dw.  A thread's bins are LW dw apart, so they are
+// the powers of rot = exp(i LW dw tau), staged once per (particle, direction).  The chain is
+// anchored at the thread's middle bin by a direct integer-phase sincos; the next bin is one
+// complex product with rot, and every other bin follows from the three-term recurrence
+// z_(i+1) = 2 cos(theta) z_i - z_(i-1) (one packed FMA), S/2 steps forwards and S/2-1 backwards:
+// 1 sincos + 1 complex product + (S-2) packed FMAs per S updates instead of S sincos.  Chain
+// length <= S/2 keeps the recurrence drift (an error grows at most n-fold over n steps) below the
+// MUFU error, which is the periodic re-anchoring BASELINE.json asks for.
 // NYQ (general grid only): Nyquist limiter -- the staging lane also finds, per (particle,
 // direction), how many bins lie below the cut-off (nyquist_count); the sweep accumulates bin j
 // only if j < that count (one ISETP per update, the four FFMAs are predicated).
