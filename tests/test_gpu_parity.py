@@ -72,6 +72,30 @@ def test_uniform_grid_padded_anchor_shapes(oracle_mod, D, W, dtype):
     assert P.base_variant(vg) == "general" and P.rel_l2(S, Sg) < 1e-5
 
 
+@pytest.mark.parametrize("frac", [0.0, 1.0 / 64.0, 0.5, 0.25 + 1e-4])
+def test_uniform_grid_recurrence_degenerate_angles(oracle_mod, frac):
+    """The uniform-grid kernel reaches the bins of a strip by the three-term recurrence z(i+1) = 2 cos(theta) z(i) - z(i-1)
+    with theta = LW dw tau, whose error growth is worst at the double root sin(theta) = 0.  Here
+    every particle sits where dw tau = 2 pi (m + frac) with an integer m of up to 3000 turns, so that all chains of the
+    sweep run at one angle: theta = 0 (frac 0; 1/2 with an even LW), pi (1/64 with 32 lanes along frequency), or close to
+    pi / 2's multiples; fp64 state so that the positions carry the angle.  All bins against the oracle."""
+    W, n = 256, 900
+    omega = np.linspace(2e15, 4e17, W)
+    dw = omega[1] - omega[0]
+    w = wl.Workload("uni_deg", n, 1, 1e-17, np.array([[0.0, 0.6, 0.8]]), omega, np.float64, wl.BASE_SEED + 31, "khi")
+    (_, st), = list(w.steps(n_steps=1))
+    st = [np.array(a, dtype=np.float64) for a in st]
+    rng = np.random.default_rng(4242)
+    tau = 2.0 * np.pi * (rng.integers(0, 3000, size=n) + frac) / dw      # retarded time of each particle at t = 0
+    for c in range(3):
+        st[c] = -wl.C_LIGHT * tau * w.dirs[0, c]                          # tau = t0 + t dt - n.r / c with t0 = t = 0
+    steps = [(0, st)]
+    S, variant = P.run_gpu(w, steps)
+    assert P.base_variant(variant) == "uniform"
+    ref = P.run_oracle(oracle_mod, w, steps).spectrum()
+    P.assert_parity(S, ref, what=f"uniform degenerate angle frac={frac}")
+
+
 def test_precise_flag_all_polynomial_sincos(oracle_mod):
     """RAD_FLAG_PRECISE: every sin/cos by the fp32 polynomial on the general-grid kernel, whatever the grid (log,
     linear, few bins).  (a) parity on the usual shapes; (b) the dark-bin case a 1200-case random hunt found
